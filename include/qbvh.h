@@ -1,0 +1,139 @@
+/* qbvh.h — C-ABI of libqbvh.so: quantized-BVH Verlet neighbor lists on NVIDIA B200 (sm_100a).
+ *
+ * Method: Howard et al., "Quantized bounding volume hierarchies for neighbor search in molecular
+ * simulations on graphics processing units", arXiv:1901.08088.  Citations are lines of
+ * /root/reference/PAPER.md ("PAPER.md:<line>") plus the section / equation / algorithm they fall in.
+ *
+ * The library solves the problem stated in PAPER.md:31 (§1): "determine the subset of particles
+ * within a distance r_c of a given particle ... saved to construct a Verlet (neighbor) list", under
+ * periodic boundaries with lattice-vector images, fp32 particle data
+ * (PAPER.md:154, 176).  Every step runs in CUDA kernels; there is no CPU fallback.
+ *
+ * Conventions
+ *   - All functions return int (or int64 where noted): >= 0 success, < 0 one of QBVH_ERR_*.
+ *     No exceptions, no aborts, no printing.
+ *   - "DEVICE" pointers are CUDA device pointers valid on the current device; "HOST" pointers are
+ *     ordinary host memory.  The library never allocates device memory: the caller supplies one
+ *     workspace (qbvh_set_workspace) that holds the tree and all scratch.
+ *   - One process-global context: the last built tree.  qbvh_neighbors may be called any number of
+ *     times per build (different r_list, larger capacity on retry).  Not thread-safe.
+ *   - All work is enqueued on the stream given to qbvh_set_stream (default: stream 0).
+ *     qbvh_build is fully asynchronous.  qbvh_neighbors synchronises that stream once, to read
+ *     back 8 bytes (max count, error flags).
+ *   - Determinism: the same inputs give a bit-identical node array and identical rows as sets;
+ *     the order of entries within a row is unspecified (sorted build => deterministic).
+ */
+#ifndef QBVH_H
+#define QBVH_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define QBVH_OK 0
+#define QBVH_ERR_INVALID_ARG (-1)      /* NULL pointer, N < 0, N >= 2^30, max_neigh < 0, bad box, bad option      */
+#define QBVH_ERR_NOT_BUILT (-2)        /* qbvh_neighbors / export before a successful qbvh_build                   */
+#define QBVH_ERR_WORKSPACE (-3)        /* workspace missing, misaligned (256 B) or smaller than qbvh_workspace_bytes */
+#define QBVH_ERR_CUTOFF_TOO_LARGE (-4) /* some padded r_ij >= L_d/2: a pair could be seen through two images       */
+#define QBVH_ERR_TYPE_RANGE (-5)       /* a type id outside [0, T) was seen by the build (reported by qbvh_neighbors) */
+#define QBVH_ERR_CUDA (-6)             /* a CUDA runtime call failed; text via qbvh_error_string(QBVH_ERR_CUDA)    */
+
+#define QBVH_MAX_TYPES 4 /* type id lives in bits 30-31 of the 32-bit sort key above the 30-bit Morton code */
+
+/* ---- set-up -------------------------------------------------------------------------------- */
+
+/* Stream for all subsequent work.  cuda_stream: a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream). */
+int qbvh_set_stream(void *cuda_stream);
+
+/* Number of particle types T in [1, QBVH_MAX_TYPES] for subsequent builds (default 1).  One BVH per type,
+ * queried across types with per-pair cutoffs (reading R14 in DESIGN.md). */
+int qbvh_set_num_types(int32_t T);
+
+/* Bytes of DEVICE workspace needed for N particles and T types (tree + scratch), a multiple of 256. */
+int64_t qbvh_workspace_bytes(int64_t N, int32_t T);
+
+/* Caller-owned DEVICE workspace, 256-byte aligned; must stay valid until the next qbvh_set_workspace.
+ * Invalidates the current tree. */
+int qbvh_set_workspace(void *dev_ptr, int64_t bytes);
+
+/* Options (all take effect at the next qbvh_build unless noted). */
+#define QBVH_OPT_LEAF_COLLAPSE 1 /* k in [1,15]: the traversal stops at nodes covering <= k consecutive Z-order
+                                    particles and distance-checks that range directly ("subtree
+                                    collapse").  k = 1 is exactly the paper's one-particle-per-leaf tree. Default 4. */
+#define QBVH_OPT_STATS 2         /* 0/1: qbvh_neighbors runs the instrumented traversal and fills qbvh_get_stats
+                                    (takes effect immediately; slower — never use when timing). Default 0.        */
+int qbvh_set_option(int32_t key, int32_t value);
+int qbvh_get_option(int32_t key);
+
+/* ---- the hot path --------------------------------------------------------------------------- */
+
+/* Build the quantized linear BVH(s).  PAPER.md:61-67 (§2.1: Morton codes in the box divided into 2^10-1 bins
+ * per axis, sort along the Z-order curve, Karras hierarchy, bounding boxes fit by walking up from the leaves),
+ * PAPER.md:69,75 (left child + rope per node for stackless traversal), PAPER.md:89 (§2.2: bounds snapped
+ * outward onto 2^10-1 bins per axis of the ROOT-node box, 3 x 10 bits per bound word, 16-byte node).
+ *   pos   DEVICE  N x 3 fp32 row-major xyz; expected wrapped into [lo_d, lo_d + L_d).  Not referenced after
+ *                 the call's kernels have run (the tree keeps its own Z-ordered copy in the workspace).
+ *   type  DEVICE  N int32 in [0, T), or NULL => all particles type 0.
+ *   N     0 <= N < 2^30.  N = 0 is a valid (empty) build.
+ *   box   HOST    6 floats {lo_x, lo_y, lo_z, L_x, L_y, L_z}: orthorhombic cell, periodic in x, y, z; L_d > 0 finite.
+ * Positions outside the box never corrupt the tree (Morton bins clamp, boxes are fit to actual coordinates)
+ * but periodic images are then wrong. */
+int qbvh_build(const float *pos, const int32_t *type, int64_t N, const float *box);
+
+/* Traverse the tree(s) once per particle (Algorithm 1: bitset of the 27 periodic images whose
+ * search sphere overlaps the root, stackless left/rope walk, sphere-AABB test of eq. 2 PAPER.md:144-146 on the
+ * decompressed box) and emit the exact Verlet list: a leaf hit is kept iff the canonical fp32 minimum-image
+ * predicate d2 <= r_ij^2 holds and j != i.
+ *   r_list_ij HOST    T x T fp32 row-major, symmetric; r_ij <= 0 => that pair of types is skipped.
+ *   nlist     DEVICE  N x max_neigh int32 row-major; row i = neighbors of ORIGINAL particle i as ORIGINAL
+ *                     indices, in unspecified order; entries past n_neigh[i] are not written.
+ *   n_neigh   DEVICE  N int32; the true number of neighbors of particle i (may exceed max_neigh).
+ *   max_neigh row capacity, >= 0.
+ * Returns M = max_i n_neigh[i] (>= 0).  M <= max_neigh: all rows complete.  M > max_neigh: OVERFLOW — rows with
+ * n_neigh[i] > max_neigh hold max_neigh true neighbors; re-allocate with capacity >= M and call again. */
+int qbvh_neighbors(const float *r_list_ij, int32_t *nlist, int32_t *n_neigh, int32_t max_neigh);
+
+/* ---- the same two calls with HOST buffers (end-to-end path: copies are part of the call) ------------------ */
+
+/* Bytes of DEVICE staging the *_host calls need for N particles with row capacity max_neigh. */
+int64_t qbvh_staging_bytes(int64_t N, int32_t max_neigh);
+int qbvh_set_staging(void *dev_ptr, int64_t bytes);
+/* pos, type: HOST (pinned memory makes the copies asynchronous).  Otherwise as qbvh_build. */
+int qbvh_build_host(const float *pos, const int32_t *type, int64_t N, const float *box);
+/* nlist, n_neigh: HOST.  Copies N x max_neigh + N int32 back after the traversal.  Otherwise as qbvh_neighbors. */
+int qbvh_neighbors_host(const float *r_list_ij, int32_t *nlist, int32_t *n_neigh, int32_t max_neigh);
+
+/* ---- inspection ----------------------------------------------------------------------------- */
+
+typedef struct qbvh_stats {
+    uint64_t node_tests;    /* sphere-AABB tests of Algorithm 1 line 12 (root tests of line 4 excluded)           */
+    uint64_t leaf_overlaps; /* tests that hit a leaf (one-particle or collapsed range)                             */
+    uint64_t dist_checks;   /* exact pair-predicate evaluations                                                    */
+    uint64_t neighbors;     /* accepted pairs (= sum of n_neigh)                                                   */
+    uint64_t images;        /* set bits of the image bitset, Algorithm 1 line 4, summed over particles and trees   */
+} qbvh_stats;
+/* Counters of the last qbvh_neighbors call made with QBVH_OPT_STATS = 1. */
+int qbvh_get_stats(qbvh_stats *out);
+
+/* Debug export of build products (for parity tests of steps a1..a6).  Copies min(bytes, available) bytes into
+ * HOST memory `dst` after synchronising the stream; returns the number of bytes available, or < 0. */
+#define QBVH_EXPORT_KEYS_SORTED 1 /* uint32 [N]: type << 30 | 30-bit Morton code, ascending                       */
+#define QBVH_EXPORT_PERM 2        /* uint32 [N]: original index of the particle at sorted position k              */
+#define QBVH_EXPORT_NODES 3       /* int32 [2N-1][4] = {lo, hi, left, rope}; internal node i at i (Karras
+                                     numbering), leaf of sorted position k at N-1+k; left >= 0: left child,
+                                     left < 0: ~first sorted position; rope = -1: END           */
+#define QBVH_EXPORT_PARENT 4      /* int32 [2N-1]: parent node, -1 for roots and unused slots                     */
+#define QBVH_EXPORT_FRAMES 5      /* float [4][12]: {lo_xyz, hi_xyz, delta_xyz, 0,0,0} quantization frame per type */
+#define QBVH_EXPORT_SEGMENTS 6    /* int32 [10]: seg[0..4] = first sorted position of each type (seg[4] = N),
+                                     then roots[0..3] (-1 for an empty type), then 0                             */
+#define QBVH_EXPORT_SORTED_POS 7  /* float [N][4]: x, y, z, bits of the original index                            */
+int64_t qbvh_debug_export(int32_t what, void *dst, int64_t bytes);
+
+const char *qbvh_error_string(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* QBVH_H */

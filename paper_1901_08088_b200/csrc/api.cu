@@ -1,0 +1,341 @@
+// api.cu — the C-ABI of libqbvh.so (include/qbvh.h): argument checks, workspace carving, launches.
+#include <cfenv>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+
+#include "../../include/qbvh.h"
+#include "qbvh_internal.cuh"
+
+namespace {
+
+struct Context {
+    cudaStream_t stream = nullptr;
+    void *ws = nullptr;
+    int64_t ws_bytes = 0;
+    void *staging = nullptr;
+    int64_t staging_bytes = 0;
+    int T = 1;
+    int K = 4;          // leaf-collapse option for the next build
+    int K_built = 1;
+    bool stats = false;
+    bool built = false;
+    int64_t N = 0;
+    float box[6] = {0, 0, 0, 0, 0, 0};
+    BuildBuffers buf{};
+    int32_t *pinned = nullptr;   // 2 ints: max_count, err_flags
+    qbvh_stats last_stats{};
+    char cuda_msg[256] = "no CUDA error recorded";
+} g;
+
+inline int64_t align256(int64_t x) { return (x + 255) & ~int64_t(255); }
+
+struct Layout {
+    int64_t meta, key_a, key_b, idx_a, idx_b, status0, status1, sorted_pos, nodes, parent, slot, total;
+};
+
+Layout make_layout(int64_t N) {
+    Layout L{};
+    const int64_t n1 = N > 0 ? N : 1;
+    const int64_t tiles = (n1 + SORT_TILE - 1) / SORT_TILE;
+    int64_t off = 0;
+    auto take = [&](int64_t bytes) {
+        int64_t o = off;
+        off += align256(bytes);
+        return o;
+    };
+    L.meta = take(sizeof(TreeMeta));
+    L.key_a = take(4 * n1);
+    L.key_b = take(4 * n1);
+    L.idx_a = take(4 * n1);
+    L.idx_b = take(4 * n1);
+    L.status0 = take(4 * 256 * tiles);
+    L.status1 = take(4 * 256 * tiles);
+    L.sorted_pos = take(16 * n1);
+    L.nodes = take(16 * (2 * n1 - 1));
+    L.parent = take(4 * (2 * n1 - 1));
+    L.slot = take(8 * n1);
+    L.total = off;
+    return L;
+}
+
+int cuda_fail(cudaError_t e, const char *where) {
+    snprintf(g.cuda_msg, sizeof(g.cuda_msg), "%s: %s", where, cudaGetErrorString(e));
+    return QBVH_ERR_CUDA;
+}
+
+float mul_ru(float a, float b) {
+    std::fesetround(FE_UPWARD);
+    volatile float r = a * b;
+    std::fesetround(FE_TONEAREST);
+    return r;
+}
+
+// padded pruning radius: r_pad = add_ru(mul_ru(r, 1 + 2^-20), 8 ulp32(M)), M = max_d(|lo_d| + 2 L_d)
+float padded_radius(float r, const float *box) {
+    double M = 0.0;
+    for (int d = 0; d < 3; ++d) M = std::fmax(M, std::fabs((double)box[d]) + 2.0 * (double)box[3 + d]);
+    int e;
+    std::frexp(M, &e);
+    const float pad_abs = (float)std::ldexp(8.0, (e - 1) - 23);
+    std::fesetround(FE_UPWARD);
+    volatile float a = r * (1.0f + 0x1p-20f);
+    volatile float b = a + pad_abs;
+    std::fesetround(FE_TONEAREST);
+    return b;
+}
+
+int neighbors_impl(const float *r_list, int32_t *nlist, int32_t *n_neigh, int32_t max_neigh) {
+    if (!g.built) return QBVH_ERR_NOT_BUILT;
+    if (!r_list || max_neigh < 0) return QBVH_ERR_INVALID_ARG;
+    if (g.N > 0 && (!n_neigh || (!nlist && max_neigh > 0))) return QBVH_ERR_INVALID_ARG;
+    TraverseParams P{};
+    for (int d = 0; d < 3; ++d) P.L[d] = g.box[3 + d];
+    for (int k = 0; k < QBVH_TMAX * QBVH_TMAX; ++k) P.r2[k] = P.R2[k] = -1.0f;
+    for (int a = 0; a < g.T; ++a)
+        for (int b = 0; b < g.T; ++b) {
+            const float r = r_list[a * g.T + b];
+            if (!(r > 0.0f)) continue;
+            if (!std::isfinite(r)) return QBVH_ERR_INVALID_ARG;
+            const float rp = padded_radius(r, g.box);
+            for (int d = 0; d < 3; ++d)
+                if (!(rp < 0.5f * g.box[3 + d])) return QBVH_ERR_CUTOFF_TOO_LARGE;
+            volatile float r2 = r * r;
+            P.r2[a * QBVH_TMAX + b] = r2;
+            P.R2[a * QBVH_TMAX + b] = mul_ru(rp, rp);
+        }
+    P.N = (int32_t)g.N;
+    P.max_neigh = max_neigh;
+    P.K = g.K_built;
+    cudaError_t e;
+    // reset max_count (+ stats) of the previous traversal
+    e = cudaMemsetAsync(&g.buf.meta->max_count, 0, sizeof(int32_t), g.stream);
+    if (e != cudaSuccess) return cuda_fail(e, "memset max_count");
+    if (g.stats) {
+        e = cudaMemsetAsync(g.buf.meta->stats, 0, sizeof(g.buf.meta->stats), g.stream);
+        if (e != cudaSuccess) return cuda_fail(e, "memset stats");
+    }
+    e = launch_traverse(P, g.buf, nlist, n_neigh, g.stats, g.stream);
+    if (e != cudaSuccess) return cuda_fail(e, "traverse launch");
+    e = cudaMemcpyAsync(g.pinned, &g.buf.meta->max_count, 2 * sizeof(int32_t), cudaMemcpyDeviceToHost, g.stream);
+    if (e != cudaSuccess) return cuda_fail(e, "copy max_count");
+    if (g.stats) {
+        e = cudaMemcpyAsync(&g.last_stats, g.buf.meta->stats, sizeof(qbvh_stats), cudaMemcpyDeviceToHost, g.stream);
+        if (e != cudaSuccess) return cuda_fail(e, "copy stats");
+    }
+    return QBVH_OK;
+}
+
+int finish_neighbors() {
+    cudaError_t e = cudaStreamSynchronize(g.stream);
+    if (e != cudaSuccess) return cuda_fail(e, "stream synchronize");
+    if (g.pinned[1] & 1) return QBVH_ERR_TYPE_RANGE;
+    return g.pinned[0];
+}
+
+}  // namespace
+
+extern "C" {
+
+int qbvh_set_stream(void *cuda_stream) {
+    g.stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+    return QBVH_OK;
+}
+
+int qbvh_set_num_types(int32_t T) {
+    if (T < 1 || T > QBVH_MAX_TYPES) return QBVH_ERR_INVALID_ARG;
+    g.T = T;
+    g.built = false;
+    return QBVH_OK;
+}
+
+int64_t qbvh_workspace_bytes(int64_t N, int32_t T) {
+    if (N < 0 || N >= (int64_t(1) << 30) || T < 1 || T > QBVH_MAX_TYPES) return QBVH_ERR_INVALID_ARG;
+    return make_layout(N).total;
+}
+
+int qbvh_set_workspace(void *dev_ptr, int64_t bytes) {
+    g.built = false;
+    if (dev_ptr && ((reinterpret_cast<uintptr_t>(dev_ptr) & 255) || bytes <= 0)) return QBVH_ERR_WORKSPACE;
+    g.ws = dev_ptr;
+    g.ws_bytes = dev_ptr ? bytes : 0;
+    return QBVH_OK;
+}
+
+int qbvh_set_option(int32_t key, int32_t value) {
+    switch (key) {
+        case QBVH_OPT_LEAF_COLLAPSE:
+            if (value < 1 || value > 15) return QBVH_ERR_INVALID_ARG;
+            g.K = value;
+            return QBVH_OK;
+        case QBVH_OPT_STATS:
+            g.stats = value != 0;
+            return QBVH_OK;
+        default:
+            return QBVH_ERR_INVALID_ARG;
+    }
+}
+
+int qbvh_get_option(int32_t key) {
+    switch (key) {
+        case QBVH_OPT_LEAF_COLLAPSE: return g.K;
+        case QBVH_OPT_STATS: return g.stats ? 1 : 0;
+        default: return QBVH_ERR_INVALID_ARG;
+    }
+}
+
+int qbvh_build(const float *pos, const int32_t *type, int64_t N, const float *box) {
+    g.built = false;
+    if (N < 0 || N >= (int64_t(1) << 30) || !box || (N > 0 && !pos)) return QBVH_ERR_INVALID_ARG;
+    for (int d = 0; d < 3; ++d)
+        if (!std::isfinite(box[d]) || !std::isfinite(box[3 + d]) || !(box[3 + d] > 0.0f)) return QBVH_ERR_INVALID_ARG;
+    const Layout L = make_layout(N);
+    if (!g.ws || g.ws_bytes < L.total) return QBVH_ERR_WORKSPACE;
+    if (!g.pinned) {
+        cudaError_t e = cudaHostAlloc(reinterpret_cast<void **>(&g.pinned), 2 * sizeof(int32_t), cudaHostAllocDefault);
+        if (e != cudaSuccess) return cuda_fail(e, "cudaHostAlloc");
+        g.pinned[0] = g.pinned[1] = 0;
+    }
+    char *w = static_cast<char *>(g.ws);
+    g.buf.meta = reinterpret_cast<TreeMeta *>(w + L.meta);
+    g.buf.key_a = reinterpret_cast<uint32_t *>(w + L.key_a);
+    g.buf.key_b = reinterpret_cast<uint32_t *>(w + L.key_b);
+    g.buf.idx_a = reinterpret_cast<uint32_t *>(w + L.idx_a);
+    g.buf.idx_b = reinterpret_cast<uint32_t *>(w + L.idx_b);
+    g.buf.status[0] = reinterpret_cast<uint32_t *>(w + L.status0);
+    g.buf.status[1] = reinterpret_cast<uint32_t *>(w + L.status1);
+    g.buf.sorted_pos = reinterpret_cast<float4 *>(w + L.sorted_pos);
+    g.buf.nodes = reinterpret_cast<int4 *>(w + L.nodes);
+    g.buf.parent = reinterpret_cast<int32_t *>(w + L.parent);
+    g.buf.slot = reinterpret_cast<unsigned long long *>(w + L.slot);
+    std::memcpy(g.box, box, sizeof(g.box));
+    float scale[3];
+    for (int d = 0; d < 3; ++d) {
+        volatile float s = 1023.0f / box[3 + d];   // fp32 RN
+        scale[d] = s;
+    }
+    const int T = type ? g.T : 1;
+    cudaError_t e = launch_build(pos, type, (int)N, T, g.K, box, scale, g.buf, g.stream);
+    if (e != cudaSuccess) return cuda_fail(e, "build launch");
+    g.N = N;
+    g.K_built = g.K;
+    g.built = true;
+    return QBVH_OK;
+}
+
+int qbvh_neighbors(const float *r_list_ij, int32_t *nlist, int32_t *n_neigh, int32_t max_neigh) {
+    int rc = neighbors_impl(r_list_ij, nlist, n_neigh, max_neigh);
+    if (rc != QBVH_OK) return rc;
+    return finish_neighbors();
+}
+
+int64_t qbvh_staging_bytes(int64_t N, int32_t max_neigh) {
+    if (N < 0 || max_neigh < 0) return QBVH_ERR_INVALID_ARG;
+    const int64_t n1 = N > 0 ? N : 1;
+    return align256(12 * n1) + align256(4 * n1) + align256(4 * n1 * (int64_t)(max_neigh > 0 ? max_neigh : 1)) + align256(4 * n1);
+}
+
+int qbvh_set_staging(void *dev_ptr, int64_t bytes) {
+    if (dev_ptr && ((reinterpret_cast<uintptr_t>(dev_ptr) & 255) || bytes <= 0)) return QBVH_ERR_WORKSPACE;
+    g.staging = dev_ptr;
+    g.staging_bytes = dev_ptr ? bytes : 0;
+    return QBVH_OK;
+}
+
+int qbvh_build_host(const float *pos, const int32_t *type, int64_t N, const float *box) {
+    if (N < 0 || (N > 0 && !pos)) return QBVH_ERR_INVALID_ARG;
+    const int64_t n1 = N > 0 ? N : 1;
+    if (!g.staging || g.staging_bytes < align256(12 * n1) + align256(4 * n1)) return QBVH_ERR_WORKSPACE;
+    char *s = static_cast<char *>(g.staging);
+    float *dpos = reinterpret_cast<float *>(s);
+    int32_t *dtype = reinterpret_cast<int32_t *>(s + align256(12 * n1));
+    cudaError_t e;
+    if (N > 0) {
+        e = cudaMemcpyAsync(dpos, pos, 12 * N, cudaMemcpyHostToDevice, g.stream);
+        if (e != cudaSuccess) return cuda_fail(e, "H2D pos");
+        if (type) {
+            e = cudaMemcpyAsync(dtype, type, 4 * N, cudaMemcpyHostToDevice, g.stream);
+            if (e != cudaSuccess) return cuda_fail(e, "H2D type");
+        }
+    }
+    return qbvh_build(dpos, type ? dtype : nullptr, N, box);
+}
+
+int qbvh_neighbors_host(const float *r_list_ij, int32_t *nlist, int32_t *n_neigh, int32_t max_neigh) {
+    if (!g.built) return QBVH_ERR_NOT_BUILT;
+    if (max_neigh < 0) return QBVH_ERR_INVALID_ARG;
+    const int64_t N = g.N, n1 = N > 0 ? N : 1;
+    if (!g.staging || g.staging_bytes < qbvh_staging_bytes(N, max_neigh)) return QBVH_ERR_WORKSPACE;
+    char *s = static_cast<char *>(g.staging);
+    int32_t *dlist = reinterpret_cast<int32_t *>(s + align256(12 * n1) + align256(4 * n1));
+    int32_t *dcnt = reinterpret_cast<int32_t *>(s + align256(12 * n1) + align256(4 * n1) +
+                                                align256(4 * n1 * (int64_t)(max_neigh > 0 ? max_neigh : 1)));
+    int rc = neighbors_impl(r_list_ij, dlist, dcnt, max_neigh);
+    if (rc != QBVH_OK) return rc;
+    if (N > 0) {
+        if (!n_neigh || (!nlist && max_neigh > 0)) return QBVH_ERR_INVALID_ARG;
+        cudaError_t e = cudaMemcpyAsync(n_neigh, dcnt, 4 * N, cudaMemcpyDeviceToHost, g.stream);
+        if (e != cudaSuccess) return cuda_fail(e, "D2H n_neigh");
+        if (max_neigh > 0) {
+            e = cudaMemcpyAsync(nlist, dlist, 4 * N * (int64_t)max_neigh, cudaMemcpyDeviceToHost, g.stream);
+            if (e != cudaSuccess) return cuda_fail(e, "D2H nlist");
+        }
+    }
+    return finish_neighbors();
+}
+
+int qbvh_get_stats(qbvh_stats *out) {
+    if (!out) return QBVH_ERR_INVALID_ARG;
+    *out = g.last_stats;
+    return QBVH_OK;
+}
+
+int64_t qbvh_debug_export(int32_t what, void *dst, int64_t bytes) {
+    if (!g.built) return QBVH_ERR_NOT_BUILT;
+    if (bytes < 0 || (bytes > 0 && !dst)) return QBVH_ERR_INVALID_ARG;
+    const int64_t N = g.N;
+    const void *src = nullptr;
+    int64_t avail = 0;
+    int32_t segroots[10];
+    switch (what) {
+        case QBVH_EXPORT_KEYS_SORTED: src = g.buf.key_a; avail = 4 * N; break;
+        case QBVH_EXPORT_PERM: src = g.buf.idx_a; avail = 4 * N; break;
+        case QBVH_EXPORT_NODES: src = g.buf.nodes; avail = N > 0 ? 16 * (2 * N - 1) : 0; break;
+        case QBVH_EXPORT_PARENT: src = g.buf.parent; avail = N > 0 ? 4 * (2 * N - 1) : 0; break;
+        case QBVH_EXPORT_FRAMES: src = g.buf.meta->frames; avail = sizeof(float) * QBVH_TMAX * 12; break;
+        case QBVH_EXPORT_SORTED_POS: src = g.buf.sorted_pos; avail = 16 * N; break;
+        case QBVH_EXPORT_SEGMENTS: avail = sizeof(segroots); break;
+        default: return QBVH_ERR_INVALID_ARG;
+    }
+    cudaError_t e = cudaStreamSynchronize(g.stream);
+    if (e != cudaSuccess) return cuda_fail(e, "export synchronize");
+    const int64_t n = bytes < avail ? bytes : avail;
+    if (what == QBVH_EXPORT_SEGMENTS) {
+        std::memset(segroots, 0, sizeof(segroots));
+        e = cudaMemcpy(segroots, g.buf.meta->seg, sizeof(int32_t) * 5, cudaMemcpyDeviceToHost);
+        if (e == cudaSuccess) e = cudaMemcpy(segroots + 5, g.buf.meta->roots, sizeof(int32_t) * 4, cudaMemcpyDeviceToHost);
+        if (e != cudaSuccess) return cuda_fail(e, "export copy");
+        std::memcpy(dst, segroots, (size_t)n);
+        return avail;
+    }
+    if (n > 0) {
+        e = cudaMemcpy(dst, src, (size_t)n, cudaMemcpyDeviceToHost);
+        if (e != cudaSuccess) return cuda_fail(e, "export copy");
+    }
+    return avail;
+}
+
+const char *qbvh_error_string(int code) {
+    switch (code) {
+        case QBVH_OK: return "ok";
+        case QBVH_ERR_INVALID_ARG: return "invalid argument";
+        case QBVH_ERR_NOT_BUILT: return "no tree: call qbvh_build first";
+        case QBVH_ERR_WORKSPACE: return "workspace/staging missing, misaligned or too small";
+        case QBVH_ERR_CUTOFF_TOO_LARGE: return "padded cutoff is not below half the shortest box length";
+        case QBVH_ERR_TYPE_RANGE: return "a particle type id is outside [0, T)";
+        case QBVH_ERR_CUDA: return g.cuda_msg;
+        default: return code > 0 ? "ok (positive return value)" : "unknown error code";
+    }
+}
+
+}  // extern "C"

@@ -1,0 +1,451 @@
+// build_kernels.cu — steps a1..a6 of the hot path, hand-written for sm_100a.
+//   a1  morton_hist_kernel : Morton keys in the periodic box + digit histograms of all four
+//                            radix passes + per-type root AABB (the quantization frame)
+//       finalize_kernel    : exclusive scans of the histograms, type segments, roots, frames
+//   a2  onesweep_kernel    : stable LSD radix sort, 8-bit digits, one kernel per pass with chained-scan
+//                            decoupled look-back between tiles (the paper used CUB)
+//   a3+a4 hierarchy_kernel : Karras binary radix tree + ropes in closed form
+//   a2'+a5+a6 fit_kernel   : gather into Z-order, quantize each leaf onto the 1023-bin grid of its tree's root
+//                            box with outward rounding, then bottom-up union with atomic
+//                            hand-over directly on the packed 10-bit integers
+#include "qbvh_internal.cuh"
+
+// ------------------------------------------------------------------------------------------------------------
+// a1. Morton keys.  b_d = clamp(floor((p_d - lo_d) * s_d), 0, 1023), s_d = 1023/L_d (fp32 RN, computed on the
+// host); code = 30-bit interleave with x in the most significant position of each triple; key = type<<30 | code.
+// ------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t spread10(uint32_t v) {  // bit t -> bit 3t
+    v &= 0x3FFu;
+    v = (v | (v << 16)) & 0x030000FFu;
+    v = (v | (v << 8)) & 0x0300F00Fu;
+    v = (v | (v << 4)) & 0x030C30C3u;
+    v = (v | (v << 2)) & 0x09249249u;
+    return v;
+}
+
+__device__ __forceinline__ uint32_t morton_bin(float p, float lo, float s) {
+    float u = __fmul_rn(__fsub_rn(p, lo), s);
+    float f = floorf(u);
+    f = fminf(fmaxf(f, 0.0f), 1023.0f);   // fmaxf(NaN,0) = 0
+    return (uint32_t)f;
+}
+
+template <int NT>
+__global__ void __launch_bounds__(256) morton_hist_kernel(const float *__restrict__ pos,
+                                                           const int32_t *__restrict__ type, int N, float3 lo,
+                                                           float3 scale, uint32_t *__restrict__ key_out,
+                                                           TreeMeta *__restrict__ meta,
+                                                           uint32_t *__restrict__ status0, int status_words) {
+    __shared__ uint32_t s_hist[4][256];
+    for (int i = threadIdx.x; i < 1024; i += blockDim.x) (&s_hist[0][0])[i] = 0;
+    __syncthreads();
+    const int stride = gridDim.x * blockDim.x;
+    const int gtid = blockIdx.x * blockDim.x + threadIdx.x;
+    // the look-back status buffer of the first sort pass must be zero before that pass starts
+    for (int i = gtid; i < status_words; i += stride) status0[i] = 0;
+
+    float mn[NT][3], mx[NT][3];
+#pragma unroll
+    for (int t = 0; t < NT; ++t)
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            mn[t][d] = INFINITY;
+            mx[t][d] = -INFINITY;
+        }
+    bool bad_type = false;
+    for (int i = gtid; i < N; i += stride) {
+        float x = pos[3 * (size_t)i + 0], y = pos[3 * (size_t)i + 1], z = pos[3 * (size_t)i + 2];
+        uint32_t t = 0;
+        if (NT > 1 || type != nullptr) {
+            int tt = type ? type[i] : 0;
+            if (tt < 0 || tt >= NT) {
+                bad_type = true;
+                tt = 0;
+            }
+            t = (uint32_t)tt;
+        }
+        uint32_t code = (spread10(morton_bin(x, lo.x, scale.x)) << 2) | (spread10(morton_bin(y, lo.y, scale.y)) << 1) |
+                        spread10(morton_bin(z, lo.z, scale.z));
+        uint32_t key = (t << 30) | code;
+        key_out[i] = key;
+        atomicAdd(&s_hist[0][key & 255u], 1u);
+        atomicAdd(&s_hist[1][(key >> 8) & 255u], 1u);
+        atomicAdd(&s_hist[2][(key >> 16) & 255u], 1u);
+        atomicAdd(&s_hist[3][key >> 24], 1u);
+#pragma unroll
+        for (int tt = 0; tt < NT; ++tt) {
+            bool m = (NT == 1) || (t == (uint32_t)tt);
+            mn[tt][0] = m ? fminf(mn[tt][0], x) : mn[tt][0];
+            mn[tt][1] = m ? fminf(mn[tt][1], y) : mn[tt][1];
+            mn[tt][2] = m ? fminf(mn[tt][2], z) : mn[tt][2];
+            mx[tt][0] = m ? fmaxf(mx[tt][0], x) : mx[tt][0];
+            mx[tt][1] = m ? fmaxf(mx[tt][1], y) : mx[tt][1];
+            mx[tt][2] = m ? fmaxf(mx[tt][2], z) : mx[tt][2];
+        }
+    }
+    // per-type min/max: warp reduce on the order-preserving encoding, one global atomic per warp and value
+#pragma unroll
+    for (int t = 0; t < NT; ++t)
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            uint32_t a = __reduce_max_sync(0xFFFFFFFFu, ~f2ord(mn[t][d]));
+            uint32_t b = __reduce_max_sync(0xFFFFFFFFu, f2ord(mx[t][d]));
+            if ((threadIdx.x & 31) == 0) {
+                if (a != ~f2ord(INFINITY)) atomicMax(&meta->mm_enc[t][d], a);
+                if (b != f2ord(-INFINITY)) atomicMax(&meta->mm_enc[t][3 + d], b);
+            }
+        }
+    if (bad_type) atomicOr(&meta->err_flags, 1);
+    __syncthreads();
+    for (int i = threadIdx.x; i < 1024; i += blockDim.x) {
+        uint32_t c = (&s_hist[0][0])[i];
+        if (c) atomicAdd(&meta->hist[0][0] + i, c);
+    }
+}
+
+// One block of 256 threads: histograms -> exclusive offsets; segments, roots, frames.
+__global__ void __launch_bounds__(256) finalize_kernel(TreeMeta *__restrict__ meta, int N, int T) {
+    __shared__ uint32_t s_scan[256];
+    __shared__ uint32_t s_ws[8];
+    const int d = threadIdx.x, lane = d & 31, warp = d >> 5;
+    for (int p = 0; p < 4; ++p) {
+        uint32_t c = meta->hist[p][d];
+        uint32_t inc = c;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t v = __shfl_up_sync(0xFFFFFFFFu, inc, o);
+            if (lane >= o) inc += v;
+        }
+        if (lane == 31) s_ws[warp] = inc;
+        __syncthreads();
+        uint32_t base = 0;
+        for (int w = 0; w < warp; ++w) base += s_ws[w];
+        uint32_t excl = base + inc - c;
+        meta->hist[p][d] = excl;
+        if (p == 3) s_scan[d] = excl;
+        __syncthreads();
+    }
+    if (d <= QBVH_TMAX) {
+        // type t owns top-digit values [64 t, 64 t + 63]
+        int s = (d < QBVH_TMAX) ? (int)s_scan[64 * d] : N;
+        meta->seg[d] = s;
+    }
+    __syncthreads();
+    if (d < QBVH_TMAX) {
+        int s = (int)s_scan[64 * d];
+        int e1 = (d + 1 < QBVH_TMAX) ? (int)s_scan[64 * (d + 1)] : N;
+        int n = e1 - s;
+        meta->roots[d] = (n <= 0) ? -1 : (n == 1 ? (N - 1 + s) : s);
+        float *fr = meta->frames[d];
+        if (n > 0) {
+            for (int a = 0; a < 3; ++a) {
+                float lo = ord2f(~meta->mm_enc[d][a]);
+                float hi = ord2f(meta->mm_enc[d][3 + a]);
+                fr[a] = lo;
+                fr[3 + a] = hi;
+                // Delta = div_ru(sub_ru(hi, lo), 1023): the 1023-bin grid spans at least the root box
+                fr[6 + a] = __fdiv_ru(__fsub_ru(hi, lo), QBVH_NBINS);
+            }
+        } else {
+            for (int a = 0; a < 9; ++a) fr[a] = 0.0f;
+        }
+        fr[9] = fr[10] = fr[11] = 0.0f;
+    }
+    (void)T;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// a2. One pass of the LSD radix sort (8-bit digit).  A tile of 4096 keys per block; ranks inside a warp by
+// match_any, warps and digits combined by block scans, tiles chained by decoupled look-back on one status word
+// per (tile, digit).  Stable: ties keep their input order at every level.  FIRST: values are implicit (= index).
+// ------------------------------------------------------------------------------------------------------------
+template <bool FIRST>
+__global__ void __launch_bounds__(SORT_THREADS) onesweep_kernel(const uint32_t *__restrict__ kin,
+                                                                 const uint32_t *__restrict__ vin,
+                                                                 uint32_t *__restrict__ kout,
+                                                                 uint32_t *__restrict__ vout, int N, int shift,
+                                                                 const uint32_t *__restrict__ hist_excl,
+                                                                 volatile uint32_t *status,
+                                                                 uint32_t *__restrict__ status_next,
+                                                                 uint32_t *__restrict__ tile_counter) {
+    __shared__ uint32_t s_whist[SORT_WARPS][256];
+    __shared__ uint32_t s_keys[SORT_TILE];
+    __shared__ uint32_t s_vals[SORT_TILE];
+    __shared__ uint32_t s_dstart[256];
+    __shared__ uint32_t s_gbase[256];
+    __shared__ uint32_t s_ws[SORT_WARPS];
+    __shared__ uint32_t s_tile;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tid == 0) s_tile = atomicAdd(tile_counter, 1u);
+    for (int i = tid; i < SORT_WARPS * 256; i += SORT_THREADS) (&s_whist[0][0])[i] = 0;
+    __syncthreads();
+    const uint32_t tile = s_tile;
+    const int base = (int)tile * SORT_TILE;
+    const int nvalid = min(SORT_TILE, N - base);
+    status_next[(size_t)tile * 256 + tid] = 0;   // the other buffer: used by the next pass, idle now
+
+    uint32_t key[SORT_IPT];
+    uint32_t rank[SORT_IPT];
+    const int wbase = warp * (32 * SORT_IPT);
+#pragma unroll
+    for (int r = 0; r < SORT_IPT; ++r) {
+        int li = wbase + r * 32 + lane;
+        key[r] = (li < nvalid) ? kin[base + li] : 0xFFFFFFFFu;
+    }
+    const uint32_t lt_mask = (1u << lane) - 1u;
+#pragma unroll
+    for (int r = 0; r < SORT_IPT; ++r) {
+        int li = wbase + r * 32 + lane;
+        bool valid = li < nvalid;
+        uint32_t d = (key[r] >> shift) & 255u;
+        uint32_t m = __match_any_sync(0xFFFFFFFFu, valid ? d : 256u);
+        uint32_t before = s_whist[warp][d];
+        __syncwarp();
+        if (valid && (m & lt_mask) == 0) s_whist[warp][d] = before + __popc(m);
+        __syncwarp();
+        rank[r] = before + __popc(m & lt_mask);
+    }
+    __syncthreads();
+    // thread d owns digit d: exclusive scan over warps, then over digits, then over tiles (look-back)
+    {
+        const int d = tid;
+        uint32_t run = 0;
+#pragma unroll
+        for (int w = 0; w < SORT_WARPS; ++w) {
+            uint32_t c = s_whist[w][d];
+            s_whist[w][d] = run;
+            run += c;
+        }
+        const uint32_t count = run;
+        uint32_t inc = count;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t v = __shfl_up_sync(0xFFFFFFFFu, inc, o);
+            if (lane >= o) inc += v;
+        }
+        if (lane == 31) s_ws[warp] = inc;
+        __syncthreads();
+        uint32_t wb = 0;
+        for (int w = 0; w < warp; ++w) wb += s_ws[w];
+        const uint32_t dstart = wb + inc - count;
+        s_dstart[d] = dstart;
+        uint32_t excl = 0;
+        if (tile == 0) {
+            status[d] = count | ST_PRE;
+        } else {
+            status[(size_t)tile * 256 + d] = count | ST_AGG;
+            int p = (int)tile - 1;
+            while (true) {
+                uint32_t v = status[(size_t)p * 256 + d];
+                if (v & ST_PRE) {
+                    excl += v & ST_VAL;
+                    break;
+                }
+                if (v & ST_AGG) {
+                    excl += v & ST_VAL;
+                    --p;
+                }
+            }
+            status[(size_t)tile * 256 + d] = (excl + count) | ST_PRE;
+        }
+        s_gbase[d] = hist_excl[d] + excl - dstart;   // wraps mod 2^32; final index is exact
+    }
+    __syncthreads();
+#pragma unroll
+    for (int r = 0; r < SORT_IPT; ++r) {
+        int li = wbase + r * 32 + lane;
+        if (li < nvalid) {
+            uint32_t d = (key[r] >> shift) & 255u;
+            uint32_t p = s_dstart[d] + s_whist[warp][d] + rank[r];
+            s_keys[p] = key[r];
+            s_vals[p] = FIRST ? (uint32_t)(base + li) : vin[base + li];
+        }
+    }
+    __syncthreads();
+    for (int p = tid; p < nvalid; p += SORT_THREADS) {
+        uint32_t k = s_keys[p];
+        uint32_t g = s_gbase[(k >> shift) & 255u] + (uint32_t)p;
+        kout[g] = k;
+        vout[g] = s_vals[p];
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// a3 + a4. One thread per sorted position k: leaf k's node words and (if it exists) internal node k.
+// delta(i,j) = length of the common prefix of the augmented keys (key, position); -1 outside the type segment.
+// Rope of a node covering [f,l] (pinned in tests/test_oracle_tree.py): END if l is the segment
+// end, else with m = l+1: internal node m if its range starts at m, else leaf m.
+// ------------------------------------------------------------------------------------------------------------
+struct SegDelta {
+    const uint32_t *key;
+    int s, e;
+    __device__ __forceinline__ int operator()(int i, uint32_t ki, long long j) const {
+        if (j < s || j > e) return -1;
+        uint32_t x = ki ^ __ldg(key + j);
+        return x ? __clz(x) : 32 + __clz((uint32_t)i ^ (uint32_t)j);
+    }
+};
+
+__global__ void __launch_bounds__(256) hierarchy_kernel(const uint32_t *__restrict__ key, int N,
+                                                         const TreeMeta *__restrict__ meta, int4 *__restrict__ nodes,
+                                                         int32_t *__restrict__ parent,
+                                                         unsigned long long *__restrict__ slot, int K) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= N) return;
+    const uint32_t ki = key[k];
+    const int t = ki >> 30;
+    SegDelta delta{key, meta->seg[t], meta->seg[t + 1] - 1};
+    const int s = delta.s, e = delta.e;
+    auto rope_of = [&](int l) -> int {
+        if (l == e) return -1;
+        const int m = l + 1;
+        const uint32_t km = __ldg(key + m);
+        if (m <= e - 1 && delta(m, km, m + 1) > delta(m, km, m - 1)) return m;
+        return N - 1 + m;
+    };
+    int2 *nodes_lr = reinterpret_cast<int2 *>(nodes);   // {left, rope} = second half of the 16-byte node
+    // leaf k
+    nodes_lr[2 * (size_t)(N - 1 + k) + 1] = make_int2(~k, rope_of(k));
+    if (s == e) parent[N - 1 + k] = -1;                 // a one-particle tree: the leaf is the root
+    if (k == e) {                                       // no internal node carries the index of a segment end
+        if (k < N - 1) {
+            nodes[k] = make_int4(0, 0, 0, -1);
+            parent[k] = -1;
+            slot[k] = SLOT_EMPTY;
+        }
+        return;
+    }
+    // internal node k (Karras)
+    const int dl = delta(k, ki, (long long)k - 1), dr = delta(k, ki, (long long)k + 1);
+    const int d = (dr > dl) ? 1 : -1;
+    const int dmin = (dr > dl) ? dl : dr;
+    long long lmax = 2;
+    while (delta(k, ki, k + lmax * d) > dmin) lmax <<= 1;
+    long long l = 0;
+    for (long long tt = lmax >> 1; tt >= 1; tt >>= 1)
+        if (delta(k, ki, k + (l + tt) * d) > dmin) l += tt;
+    const int j = (int)(k + l * d);
+    const int dnode = delta(k, ki, j);
+    long long sp = 0, tt = l;
+    do {
+        tt = (tt + 1) >> 1;
+        if (delta(k, ki, k + (sp + tt) * d) > dnode) sp += tt;
+    } while (tt > 1);
+    const int gamma = (int)(k + sp * d + (d < 0 ? -1 : 0));
+    const int f = min(k, j), la = max(k, j);
+    const int lc = (f == gamma) ? (N - 1 + gamma) : gamma;
+    const int rc = (la == gamma + 1) ? (N - 1 + gamma + 1) : (gamma + 1);
+    parent[lc] = k;
+    parent[rc] = k;
+    if (k == s) parent[k] = -1;
+    const int size = la - f + 1;
+    const int leftword = (K > 1 && size <= K) ? ~f : lc;   // collapsed range leaf: first sorted position
+    nodes_lr[2 * (size_t)k + 1] = make_int2(leftword, rope_of(la));
+    slot[k] = SLOT_EMPTY;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// a2' + a5 + a6.  Quantizer defined by its decompressor:
+//   D_lo(q) = fma_rd(q, Delta, lo)   D_hi(q) = fma_ru(q, Delta, lo)
+//   q_lo(a) = max{q : D_lo(q) <= a}  q_hi(b) = min{q : D_hi(q) >= b}     (bisection: D_lo, D_hi are monotone)
+// q_lo/q_hi are monotone, so the union of boxes is the per-field integer min/max of the packed words.
+// ------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t quant_lo(float a, float lo, float delta) {
+    uint32_t q = 0;
+#pragma unroll
+    for (uint32_t bit = 512; bit; bit >>= 1) {
+        uint32_t c = q | bit;
+        if (__fmaf_rd((float)c, delta, lo) <= a) q = c;
+    }
+    return q;
+}
+__device__ __forceinline__ uint32_t quant_hi(float b, float lo, float delta) {
+    uint32_t q = 0;
+#pragma unroll
+    for (uint32_t bit = 512; bit; bit >>= 1) {
+        uint32_t c = q + bit;
+        if (__fmaf_ru((float)(c - 1), delta, lo) < b) q = c;
+    }
+    return q;
+}
+__device__ __forceinline__ uint32_t pack_min(uint32_t a, uint32_t b) {
+    return min(a & 0x3FFu, b & 0x3FFu) | min(a & 0xFFC00u, b & 0xFFC00u) | min(a & 0x3FF00000u, b & 0x3FF00000u);
+}
+__device__ __forceinline__ uint32_t pack_max(uint32_t a, uint32_t b) {
+    return max(a & 0x3FFu, b & 0x3FFu) | max(a & 0xFFC00u, b & 0xFFC00u) | max(a & 0x3FF00000u, b & 0x3FF00000u);
+}
+
+__global__ void __launch_bounds__(256) fit_kernel(const float *__restrict__ pos, const uint32_t *__restrict__ idx_sorted,
+                                                   const uint32_t *__restrict__ key_sorted, int N,
+                                                   const TreeMeta *__restrict__ meta, float4 *__restrict__ sorted_pos,
+                                                   int4 *__restrict__ nodes, const int32_t *__restrict__ parent,
+                                                   unsigned long long *__restrict__ slot, int K) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= N) return;
+    const uint32_t idx = idx_sorted[k];
+    const float x = pos[3 * (size_t)idx], y = pos[3 * (size_t)idx + 1], z = pos[3 * (size_t)idx + 2];
+    sorted_pos[k] = make_float4(x, y, z, __uint_as_float(idx));
+    const float *fr = meta->frames[key_sorted[k] >> 30];
+    uint32_t wlo = quant_lo(x, fr[0], fr[6]) | (quant_lo(y, fr[1], fr[7]) << 10) | (quant_lo(z, fr[2], fr[8]) << 20);
+    uint32_t whi = quant_hi(x, fr[0], fr[6]) | (quant_hi(y, fr[1], fr[7]) << 10) | (quant_hi(z, fr[2], fr[8]) << 20);
+    int2 *nodes_b = reinterpret_cast<int2 *>(nodes);    // {lo, hi} = first half of the 16-byte node
+    nodes_b[2 * (size_t)(N - 1 + k)] = make_int2((int)wlo, (int)whi);
+    uint32_t cnt = 0;                                    // (leaves under the node) - 1, saturating at 15
+    int n = parent[N - 1 + k];
+    while (n >= 0) {
+        // hand-over through one 64-bit atomic: the first child to arrive deposits its box, the second merges
+        unsigned long long mine = (unsigned long long)(wlo | ((cnt & 3u) << 30)) |
+                                  ((unsigned long long)(whi | ((cnt >> 2) << 30)) << 32);
+        unsigned long long other = atomicExch(slot + n, mine);
+        if (other == SLOT_EMPTY) break;
+        uint32_t olo = (uint32_t)other, ohi = (uint32_t)(other >> 32);
+        uint32_t ocnt = (olo >> 30) | ((ohi >> 30) << 2);
+        wlo = pack_min(wlo, olo);
+        whi = pack_max(whi, ohi);
+        cnt = min(cnt + ocnt + 1u, 15u);
+        uint32_t slo = wlo, shi = whi;
+        if (K > 1) {                                    // spare bits carry the leaf count for collapsed ranges
+            slo |= (cnt & 3u) << 30;
+            shi |= (cnt >> 2) << 30;
+        }
+        nodes_b[2 * (size_t)n] = make_int2((int)slo, (int)shi);
+        n = parent[n];
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+cudaError_t launch_build(const float *pos, const int32_t *type, int N, int T, int K, const float *box_lo,
+                         const float *box_scale, const BuildBuffers &b, cudaStream_t st) {
+    cudaError_t err = cudaMemsetAsync(b.meta, 0, sizeof(TreeMeta), st);
+    if (err != cudaSuccess) return err;
+    if (N == 0) {
+        finalize_kernel<<<1, 256, 0, st>>>(b.meta, 0, T);
+        return cudaGetLastError();
+    }
+    const int tiles = (N + SORT_TILE - 1) / SORT_TILE;
+    const int status_words = tiles * 256;
+    const float3 lo = make_float3(box_lo[0], box_lo[1], box_lo[2]);
+    const float3 sc = make_float3(box_scale[0], box_scale[1], box_scale[2]);
+    int mblocks = (N + 255) / 256;
+    if (mblocks > 148 * 8) mblocks = 148 * 8;
+    switch (T) {
+        case 1: morton_hist_kernel<1><<<mblocks, 256, 0, st>>>(pos, type, N, lo, sc, b.key_a, b.meta, b.status[0], status_words); break;
+        case 2: morton_hist_kernel<2><<<mblocks, 256, 0, st>>>(pos, type, N, lo, sc, b.key_a, b.meta, b.status[0], status_words); break;
+        case 3: morton_hist_kernel<3><<<mblocks, 256, 0, st>>>(pos, type, N, lo, sc, b.key_a, b.meta, b.status[0], status_words); break;
+        default: morton_hist_kernel<4><<<mblocks, 256, 0, st>>>(pos, type, N, lo, sc, b.key_a, b.meta, b.status[0], status_words); break;
+    }
+    finalize_kernel<<<1, 256, 0, st>>>(b.meta, N, T);
+    // four passes a -> b -> a -> b -> a
+    onesweep_kernel<true><<<tiles, SORT_THREADS, 0, st>>>(b.key_a, nullptr, b.key_b, b.idx_b, N, 0, b.meta->hist[0],
+                                                          b.status[0], b.status[1], &b.meta->tile_counter[0]);
+    onesweep_kernel<false><<<tiles, SORT_THREADS, 0, st>>>(b.key_b, b.idx_b, b.key_a, b.idx_a, N, 8, b.meta->hist[1],
+                                                           b.status[1], b.status[0], &b.meta->tile_counter[1]);
+    onesweep_kernel<false><<<tiles, SORT_THREADS, 0, st>>>(b.key_a, b.idx_a, b.key_b, b.idx_b, N, 16, b.meta->hist[2],
+                                                           b.status[0], b.status[1], &b.meta->tile_counter[2]);
+    onesweep_kernel<false><<<tiles, SORT_THREADS, 0, st>>>(b.key_b, b.idx_b, b.key_a, b.idx_a, N, 24, b.meta->hist[3],
+                                                           b.status[1], b.status[0], &b.meta->tile_counter[3]);
+    const int nb = (N + 255) / 256;
+    hierarchy_kernel<<<nb, 256, 0, st>>>(b.key_a, N, b.meta, b.nodes, b.parent, b.slot, K);
+    fit_kernel<<<nb, 256, 0, st>>>(pos, b.idx_a, b.key_a, N, b.meta, b.sorted_pos, b.nodes, b.parent, b.slot, K);
+    return cudaGetLastError();
+}

@@ -1,0 +1,69 @@
+// qbvh_internal.cuh — device-side data layout shared by the build and traversal kernels (sm_100a only).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#define QBVH_TMAX 4            // types live in key bits 30-31
+#define QBVH_NBINS 1023.0f     // 2^10 - 1 bins per axis
+
+// Device-resident bookkeeping of one build (lives at the start of the workspace; zeroed by a memset per build).
+struct TreeMeta {
+    uint32_t hist[4][256];     // per-pass digit histograms, turned into exclusive offsets by finalize_kernel
+    uint32_t tile_counter[4];  // dynamic tile ids of the four onesweep passes
+    uint32_t mm_enc[QBVH_TMAX][6];  // per type: ~enc(min xyz) (so atomicMax computes the min), enc(max xyz)
+    int32_t seg[QBVH_TMAX + 1];     // first sorted position of each type; seg[T..4] = N
+    int32_t roots[QBVH_TMAX];       // root node per type, -1 if empty
+    float frames[QBVH_TMAX][12];    // lo xyz, hi xyz, delta xyz, 0 0 0
+    int32_t max_count;              // max_i n_neigh[i] of the last traversal
+    int32_t err_flags;              // bit 0: type id out of range
+    unsigned long long stats[8];    // node_tests, leaf_overlaps, dist_checks, neighbors, images
+};
+
+// order-preserving map float -> uint32 (NaN excluded)
+__host__ __device__ inline uint32_t f2ord(float f) {
+#ifdef __CUDA_ARCH__
+    uint32_t b = __float_as_uint(f);
+#else
+    union { float f; uint32_t u; } c; c.f = f; uint32_t b = c.u;
+#endif
+    return (b & 0x80000000u) ? ~b : (b | 0x80000000u);
+}
+__device__ inline float ord2f(uint32_t o) {
+    uint32_t b = (o & 0x80000000u) ? (o & 0x7FFFFFFFu) : ~o;
+    return __uint_as_float(b);
+}
+
+#define SLOT_EMPTY 0xFFFFFFFFFFFFFFFFull
+
+// ---- sort geometry ----
+constexpr int SORT_THREADS = 256;
+constexpr int SORT_WARPS = SORT_THREADS / 32;
+constexpr int SORT_IPT = 16;                          // keys per thread
+constexpr int SORT_TILE = SORT_THREADS * SORT_IPT;    // 4096 keys per tile
+constexpr uint32_t ST_AGG = 1u << 30;                 // tile status: aggregate (own count) available
+constexpr uint32_t ST_PRE = 1u << 31;                 // tile status: inclusive prefix available
+constexpr uint32_t ST_VAL = (1u << 30) - 1;
+
+struct TraverseParams {
+    float L[3];
+    float r2[QBVH_TMAX * QBVH_TMAX];   // r_ij^2 (fp32 RN), <0 => skipped
+    float R2[QBVH_TMAX * QBVH_TMAX];   // padded pruning radius squared (rounded up)
+    int32_t N;
+    int32_t max_neigh;
+    int32_t K;                         // leaf-collapse threshold used by the build
+};
+
+// launchers (build_kernels.cu / traverse_kernels.cu)
+struct BuildBuffers {
+    TreeMeta *meta;
+    uint32_t *key_a, *key_b, *idx_a, *idx_b;
+    uint32_t *status[2];
+    float4 *sorted_pos;
+    int4 *nodes;
+    int32_t *parent;
+    unsigned long long *slot;
+};
+cudaError_t launch_build(const float *pos, const int32_t *type, int N, int T, int K, const float *box_lo,
+                         const float *box_scale, const BuildBuffers &b, cudaStream_t st);
+cudaError_t launch_traverse(const TraverseParams &p, const BuildBuffers &b, int32_t *nlist, int32_t *n_neigh,
+                            bool stats, cudaStream_t st);

@@ -1,0 +1,214 @@
+"""ctypes binding of libqbvh.so — same names as include/qbvh.h, argument marshalling only.
+
+Every step of the path runs in the CUDA kernels behind the C-ABI.  PyTorch is used for device memory
+and streams.  Importing this module fails loudly if the CUDA library has not been built; there is no
+CPU fallback.  Nothing here imports ``oracle/``.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libqbvh.so")
+
+OK = 0
+ERR_INVALID_ARG, ERR_NOT_BUILT, ERR_WORKSPACE, ERR_CUTOFF_TOO_LARGE, ERR_TYPE_RANGE, ERR_CUDA = -1, -2, -3, -4, -5, -6
+MAX_TYPES = 4
+OPT_LEAF_COLLAPSE, OPT_STATS = 1, 2
+EXPORT_KEYS_SORTED, EXPORT_PERM, EXPORT_NODES, EXPORT_PARENT, EXPORT_FRAMES, EXPORT_SEGMENTS, EXPORT_SORTED_POS = range(1, 8)
+
+# every symbol include/qbvh.h declares
+SYMBOLS = ("qbvh_set_stream", "qbvh_set_num_types", "qbvh_workspace_bytes", "qbvh_set_workspace",
+           "qbvh_set_option", "qbvh_get_option", "qbvh_build", "qbvh_neighbors", "qbvh_staging_bytes",
+           "qbvh_set_staging", "qbvh_build_host", "qbvh_neighbors_host", "qbvh_get_stats", "qbvh_debug_export",
+           "qbvh_error_string")
+
+
+class QbvhStats(C.Structure):
+    _fields_ = [("node_tests", C.c_uint64), ("leaf_overlaps", C.c_uint64), ("dist_checks", C.c_uint64),
+                ("neighbors", C.c_uint64), ("images", C.c_uint64)]
+
+
+class QbvhError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        super().__init__(f"{where}: {qbvh_error_string(code)} ({code})")
+
+
+if not os.path.exists(LIB_PATH):
+    raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_1901_08088_b200.build` "
+                      "(there is no CPU fallback)")
+_lib = C.CDLL(LIB_PATH)
+_vp, _i32, _i64 = C.c_void_p, C.c_int32, C.c_int64
+_lib.qbvh_set_stream.argtypes = [_vp]
+_lib.qbvh_set_num_types.argtypes = [_i32]
+_lib.qbvh_workspace_bytes.argtypes = [_i64, _i32]
+_lib.qbvh_workspace_bytes.restype = _i64
+_lib.qbvh_set_workspace.argtypes = [_vp, _i64]
+_lib.qbvh_set_option.argtypes = [_i32, _i32]
+_lib.qbvh_get_option.argtypes = [_i32]
+_lib.qbvh_build.argtypes = [_vp, _vp, _i64, _vp]
+_lib.qbvh_neighbors.argtypes = [_vp, _vp, _vp, _i32]
+_lib.qbvh_staging_bytes.argtypes = [_i64, _i32]
+_lib.qbvh_staging_bytes.restype = _i64
+_lib.qbvh_set_staging.argtypes = [_vp, _i64]
+_lib.qbvh_build_host.argtypes = [_vp, _vp, _i64, _vp]
+_lib.qbvh_neighbors_host.argtypes = [_vp, _vp, _vp, _i32]
+_lib.qbvh_get_stats.argtypes = [C.POINTER(QbvhStats)]
+_lib.qbvh_debug_export.argtypes = [_i32, _vp, _i64]
+_lib.qbvh_debug_export.restype = _i64
+_lib.qbvh_error_string.argtypes = [C.c_int]
+_lib.qbvh_error_string.restype = C.c_char_p
+
+
+def _ptr(x):
+    """Device/host pointer of a torch tensor, numpy array, int or None."""
+    if x is None:
+        return None
+    if isinstance(x, int):
+        return x
+    if isinstance(x, np.ndarray):
+        assert x.flags["C_CONTIGUOUS"]
+        return x.ctypes.data
+    assert x.is_contiguous()
+    return x.data_ptr()
+
+
+def _host_f32(a, n):
+    a = np.ascontiguousarray(a, dtype=np.float32).reshape(-1)
+    assert a.size == n, (a.size, n)
+    return a
+
+
+def qbvh_error_string(code: int) -> str:
+    return _lib.qbvh_error_string(int(code)).decode()
+
+
+def _check(rc: int, where: str) -> int:
+    if rc < 0:
+        raise QbvhError(int(rc), where)
+    return int(rc)
+
+
+def qbvh_set_stream(cuda_stream: int) -> int:
+    return _check(_lib.qbvh_set_stream(cuda_stream), "qbvh_set_stream")
+
+
+def qbvh_set_num_types(T: int) -> int:
+    return _check(_lib.qbvh_set_num_types(T), "qbvh_set_num_types")
+
+
+def qbvh_workspace_bytes(N: int, T: int = 1) -> int:
+    return _check(_lib.qbvh_workspace_bytes(N, T), "qbvh_workspace_bytes")
+
+
+def qbvh_set_workspace(buf, nbytes: int | None = None) -> int:
+    if nbytes is None:
+        nbytes = 0 if buf is None else buf.numel() * buf.element_size()
+    return _check(_lib.qbvh_set_workspace(_ptr(buf), nbytes), "qbvh_set_workspace")
+
+
+def qbvh_set_option(key: int, value: int) -> int:
+    return _check(_lib.qbvh_set_option(key, value), "qbvh_set_option")
+
+
+def qbvh_get_option(key: int) -> int:
+    return _check(_lib.qbvh_get_option(key), "qbvh_get_option")
+
+
+def qbvh_build(pos, type, N: int, box) -> int:
+    """pos, type: DEVICE tensors (float32 N x 3, int32 N or None); box: 6 host floats."""
+    box = _host_f32(box, 6)
+    return _check(_lib.qbvh_build(_ptr(pos), _ptr(type), N, box.ctypes.data), "qbvh_build")
+
+
+def qbvh_neighbors(r_list_ij, nlist, n_neigh, max_neigh: int, T: int | None = None) -> int:
+    """r_list_ij: host T x T; nlist, n_neigh: DEVICE int32 tensors.  Returns M = max n_neigh (overflow iff M > max_neigh)."""
+    r = np.ascontiguousarray(r_list_ij, dtype=np.float32)
+    return _check(_lib.qbvh_neighbors(r.ctypes.data, _ptr(nlist), _ptr(n_neigh), max_neigh), "qbvh_neighbors")
+
+
+def qbvh_staging_bytes(N: int, max_neigh: int) -> int:
+    return _check(_lib.qbvh_staging_bytes(N, max_neigh), "qbvh_staging_bytes")
+
+
+def qbvh_set_staging(buf, nbytes: int | None = None) -> int:
+    if nbytes is None:
+        nbytes = 0 if buf is None else buf.numel() * buf.element_size()
+    return _check(_lib.qbvh_set_staging(_ptr(buf), nbytes), "qbvh_set_staging")
+
+
+def qbvh_build_host(pos, type, N: int, box) -> int:
+    """pos, type: HOST buffers (numpy arrays or pinned CPU torch tensors)."""
+    box = _host_f32(box, 6)
+    return _check(_lib.qbvh_build_host(_ptr(pos), _ptr(type), N, box.ctypes.data), "qbvh_build_host")
+
+
+def qbvh_neighbors_host(r_list_ij, nlist, n_neigh, max_neigh: int) -> int:
+    r = np.ascontiguousarray(r_list_ij, dtype=np.float32)
+    return _check(_lib.qbvh_neighbors_host(r.ctypes.data, _ptr(nlist), _ptr(n_neigh), max_neigh), "qbvh_neighbors_host")
+
+
+def qbvh_get_stats() -> dict:
+    s = QbvhStats()
+    _check(_lib.qbvh_get_stats(C.byref(s)), "qbvh_get_stats")
+    return {k: int(getattr(s, k)) for k, _ in QbvhStats._fields_}
+
+
+def qbvh_debug_export(what: int, N: int) -> np.ndarray:
+    """Host copy of a build product (see QBVH_EXPORT_* in include/qbvh.h)."""
+    shapes = {EXPORT_KEYS_SORTED: (np.uint32, (N,)), EXPORT_PERM: (np.uint32, (N,)),
+              EXPORT_NODES: (np.int32, (max(2 * N - 1, 0), 4)), EXPORT_PARENT: (np.int32, (max(2 * N - 1, 0),)),
+              EXPORT_FRAMES: (np.float32, (4, 12)), EXPORT_SEGMENTS: (np.int32, (10,)),
+              EXPORT_SORTED_POS: (np.float32, (N, 4))}
+    dt, shp = shapes[what]
+    out = np.zeros(shp, dt)
+    avail = _check(_lib.qbvh_debug_export(what, out.ctypes.data, out.nbytes), "qbvh_debug_export")
+    assert avail == out.nbytes, (avail, out.nbytes)
+    return out
+
+
+# ---------------------------------------------------------------------------------------------------------
+# Convenience wrapper: owns the torch workspace, retries on overflow.  Plumbing only — no arithmetic.
+# ---------------------------------------------------------------------------------------------------------
+class NeighborList:
+    """Device-resident Verlet list builder.
+
+    >>> nl = NeighborList(N, T=1, max_neigh=128)
+    >>> nl.build(pos_cuda, None, box)              # qbvh_build
+    >>> M = nl.neighbors(r_list)                   # qbvh_neighbors (+ re-allocation and retry on overflow)
+    >>> nl.nlist, nl.n_neigh                       # int32 CUDA tensors
+    """
+
+    def __init__(self, N: int, T: int = 1, max_neigh: int = 128, device="cuda:0"):
+        import torch
+        self.torch = torch
+        self.device = torch.device(device)
+        self.N, self.T, self.max_neigh = int(N), int(T), int(max_neigh)
+        self.workspace = torch.empty(qbvh_workspace_bytes(N, T), dtype=torch.uint8, device=self.device)
+        self.nlist = torch.empty((max(N, 1), max(max_neigh, 1)), dtype=torch.int32, device=self.device)
+        self.n_neigh = torch.zeros(max(N, 1), dtype=torch.int32, device=self.device)
+        self.retries = 0
+
+    def _activate(self):
+        qbvh_set_stream(self.torch.cuda.current_stream(self.device).cuda_stream)
+        qbvh_set_num_types(self.T)
+
+    def build(self, pos, type, box):
+        assert pos.is_cuda and pos.dtype == self.torch.float32 and tuple(pos.shape) == (self.N, 3)
+        assert type is None or (type.is_cuda and type.dtype == self.torch.int32)
+        self._activate()
+        qbvh_set_workspace(self.workspace)
+        return qbvh_build(pos, type, self.N, box)
+
+    def neighbors(self, r_list, retry: bool = True) -> int:
+        M = qbvh_neighbors(r_list, self.nlist, self.n_neigh, self.max_neigh)
+        while retry and M > self.max_neigh:
+            self.retries += 1
+            self.max_neigh = int((M + 7) // 8 * 8)
+            self.nlist = self.torch.empty((max(self.N, 1), self.max_neigh), dtype=self.torch.int32, device=self.device)
+            M = qbvh_neighbors(r_list, self.nlist, self.n_neigh, self.max_neigh)
+        return M

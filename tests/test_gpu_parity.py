@@ -1,0 +1,246 @@
+"""-m gpu parity tests: the CUDA path, called through the C-ABI binding, against the CPU oracle.
+
+Bar (BASELINE.json north_star): bit-exact integer work (keys, permutation, node words, links); neighbor sets
+identical after sorting except pairs within 1e-5 sigma of r_list (counted; <= 1e-6 of all pairs) — here both sides
+evaluate the same fp32 predicate, so the tests additionally assert ZERO mismatches.
+"""
+import numpy as np
+import pytest
+
+from oracle import neighbors as ON
+from oracle import tree as OT
+from paper_1901_08088_b200 import workloads as W
+
+from gpu_util import compare_with_oracle, gpu_run
+
+pytestmark = pytest.mark.gpu
+
+
+def expected_nodes(t, K):
+    """Oracle tree -> the node array the CUDA path must produce for leaf-collapse option K."""
+    nodes = t.nodes_int4().copy()
+    if K > 1:
+        N = t.N
+        size = (t.last - t.first + 1).astype(np.int64)
+        internal = np.arange(2 * N - 1) < N - 1
+        real = t.first >= 0
+        coll = internal & real & (size <= K)
+        nodes[coll, 2] = ~t.first[coll]
+        cnt = np.minimum(size - 1, 15).astype(np.uint32)
+        inner = internal & real
+        nodes[inner, 0] = (t.wlo[inner] | ((cnt[inner] & 3) << 30)).view(np.int32)
+        nodes[inner, 1] = (t.whi[inner] | ((cnt[inner] >> 2) << 30)).view(np.int32)
+    return nodes
+
+
+def check_build(w, K):
+    out = gpu_run(w, K=K, export=True)
+    t = OT.build(w.pos, w.type, w.box, T=w.T)
+    N = w.N
+    assert np.array_equal(out["keys_sorted"], t.key_sorted)                      # a1 + a2 keys
+    assert np.array_equal(out["perm"].astype(np.int64), t.perm)                  # a2 stable permutation
+    seg, roots = out["segments"][:5], out["segments"][5:9]
+    assert np.array_equal(seg[: w.T + 1], t.seg) and np.all(seg[w.T:] == N)
+    assert np.array_equal(roots[: w.T], t.roots) and np.all(roots[w.T:] == -1)
+    for tb in range(w.T):
+        if t.roots[tb] >= 0:
+            assert np.array_equal(out["frames"][tb, :9], t.frames[tb])           # root boxes + Delta (bitwise)
+    assert np.array_equal(out["sorted_pos"][:, :3], t.pos_sorted)               # a2' gather
+    assert np.array_equal(out["sorted_pos"][:, 3].view(np.uint32).astype(np.int64), t.perm)
+    exp = expected_nodes(t, K)
+    real = np.ones(2 * N - 1, bool)
+    real[: N - 1] = t.first[: N - 1] >= 0                                        # skip unused internal slots
+    assert np.array_equal(out["nodes"][real], exp[real])                         # a3..a6: 16-byte nodes, bitwise
+    assert np.array_equal(out["nodes"][~real], np.tile([0, 0, 0, -1], ((~real).sum(), 1)))
+    assert np.array_equal(out["parent"][real], t.parent[real])
+    return out, t
+
+
+@pytest.mark.parametrize("K", [1, 4])
+@pytest.mark.parametrize("cid", [1, 2, 3, 4, 5])
+def test_build_parity_small(cid, K):
+    check_build(W.make_config(cid, small=True), K)
+
+
+@pytest.mark.parametrize("N", [1, 2, 3, 31, 32, 33, 255, 4095, 4096, 4097, 8193, 70001])
+def test_build_sizes_and_ragged_tiles(N):
+    """Sort tiles are 4096 keys: sizes around the tile edge, one warp, one element."""
+    w = W.lj_uniform(N=N, rho=min(0.85, N / 64.0), r_list=1.2, config_id=40)   # L >= 4 > 2 r_list
+    out, t = check_build(w, 1)
+    compare_with_oracle(w, out, ON.neighbor_list(w.pos, None, w.box, w.r_list))
+
+
+def _line(N, reverse=False, dup=1):
+    """Particles on the body diagonal -> strictly increasing Morton keys (already sorted / reversed / duplicated)."""
+    L = 64.0
+    t = (np.arange(N) // dup) / max(1, (N - 1) // dup + 1)
+    p = np.repeat(t[:, None], 3, 1) * L
+    if reverse:
+        p = p[::-1]
+    return W._finish(np.ascontiguousarray(p), L)
+
+
+@pytest.mark.parametrize("case", ["sorted", "reverse", "dups", "all_equal"])
+def test_sort_degenerate_orders(case):
+    N = 20000
+    if case == "all_equal":
+        pos, box = W._finish(np.full((N, 3), 3.25), 64.0)
+    else:
+        pos, box = _line(N, reverse=(case == "reverse"), dup=(7 if case == "dups" else 1))
+    w = W.Workload(case, pos, None, box, np.array([[0.5]], np.float32), 64)
+    out, t = check_build(w, 4)
+    if case == "all_equal":
+        assert np.array_equal(out["perm"], np.arange(N))   # stability: equal keys keep input order
+
+
+@pytest.mark.parametrize("K", [1, 4, 8, 15])
+@pytest.mark.parametrize("cid", [1, 2, 3, 4, 5])
+def test_neighbors_parity_small(cid, K):
+    w = W.make_config(cid, small=True)
+    out = gpu_run(w, K=K)
+    rep = compare_with_oracle(w, out, ON.neighbor_list(w.pos, w.type, w.box, w.r_list))
+    assert rep["rows_checked"] == w.N
+
+
+@pytest.mark.parametrize("cid", [2, 3, 4, 5])
+def test_neighbors_parity_full_size(cid):
+    """BASELINE.json's full sizes, in the launch configuration bench.py times (default options)."""
+    w = W.make_config(cid)
+    out = gpu_run(w, K=4)
+    rep = compare_with_oracle(w, out, ON.neighbor_list(w.pos, w.type, w.box, w.r_list, method="cell"))
+    assert rep["rows_checked"] == w.N and rep["pairs"] > 0
+
+
+def test_overflow_detection_and_retry():
+    w = W.lj_uniform()
+    csr = ON.neighbor_list(w.pos, None, w.box, w.r_list)
+    true_max = int(np.diff(csr[0]).max())
+    out = gpu_run(w, max_neigh=64)                     # too small: mean count is ~87
+    assert out["M"] == true_max > 64
+    compare_with_oracle(w, out, csr, allow_overflow=True)
+    out = gpu_run(w, max_neigh=64, retry=True)         # wrapper re-allocates with capacity >= M and calls again
+    assert out["retries"] == 1 and out["max_neigh"] >= true_max
+    compare_with_oracle(w, out, csr)
+    out = gpu_run(w, max_neigh=0)                      # count-only use
+    assert np.array_equal(out["n_neigh"], np.diff(csr[0]))
+
+
+def test_edge_cases():
+    import torch
+    from paper_1901_08088_b200 import qbvh
+    box = np.array([-5, -5, -5, 10, 10, 10], np.float32)
+    # N = 0
+    nl = qbvh.NeighborList(0, 1, 8)
+    nl.build(torch.zeros((0, 3), device="cuda"), None, box)
+    assert nl.neighbors(np.array([[1.0]], np.float32)) == 0
+    # N = 1: the tree is one leaf that is also the root
+    w = W.Workload("one", np.array([[1, 2, 3]], np.float32), None, box, np.array([[2.0]], np.float32), 4)
+    out = gpu_run(w, export=True)
+    assert out["M"] == 0 and out["n_neigh"].tolist() == [0] and out["segments"][5] == 0
+    # two coincident particles are neighbors of each other; self excluded by index
+    w = W.Workload("two", np.array([[1, 2, 3], [1, 2, 3]], np.float32), None, box, np.array([[0.1]], np.float32), 4)
+    out = gpu_run(w)
+    assert out["n_neigh"].tolist() == [1, 1] and out["nlist"][0, 0] == 1 and out["nlist"][1, 0] == 0
+    # all particles share one coordinate (zero root extent along x) and faces
+    rng = np.random.default_rng(5)
+    p = rng.random((3000, 3)) * 10
+    p[:, 0] = 2.5
+    p[:40, 1] = 0.0
+    pos, _ = W._finish(p, 10.0)
+    w = W.Workload("plane", pos, None, box, np.array([[1.1]], np.float32), 64)
+    for K in (1, 4):
+        compare_with_oracle(w, gpu_run(w, K=K), ON.neighbor_list(w.pos, None, box, w.r_list))
+    # four types, one of them empty, one with a single particle, one pair type switched off
+    p = rng.random((5000, 3)) * 10
+    pos, _ = W._finish(p, 10.0)
+    typ = rng.integers(0, 2, 5000).astype(np.int32) * 2        # types 0 and 2
+    typ[17] = 3
+    r = np.array([[1.0, 0.5, 1.4, 2.0], [0.5, 0.5, 0.5, 0.5], [1.4, 0.5, 0.0, 3.0], [2.0, 0.5, 3.0, 1.0]], np.float32)
+    w = W.Workload("types", pos, typ, box, r, 128)
+    for K in (1, 4):
+        compare_with_oracle(w, gpu_run(w, K=K), ON.neighbor_list(w.pos, typ, box, r))
+    # r just under L/2 (padded radius still below L/2)
+    w = W.Workload("halfbox", pos[:600], None, box, np.array([[4.99]], np.float32), 600)
+    compare_with_oracle(w, gpu_run(w, K=4), ON.neighbor_list(w.pos, None, box, w.r_list))
+
+
+def test_error_codes():
+    import torch
+    from paper_1901_08088_b200 import qbvh
+    w = W.lj_uniform(N=1000, config_id=41)
+    nl = qbvh.NeighborList(w.N, 1, 64)
+    pos = torch.from_numpy(w.pos).cuda()
+    nl.build(pos, None, w.box)
+    with pytest.raises(qbvh.QbvhError) as e:
+        nl.neighbors(np.array([[0.5 * float(w.box[3])]], np.float32))
+    assert e.value.code == qbvh.ERR_CUTOFF_TOO_LARGE
+    typ = torch.zeros(w.N, dtype=torch.int32, device="cuda")
+    typ[5] = 3
+    nl2 = qbvh.NeighborList(w.N, 2, 64)
+    nl2.build(pos, typ, w.box)
+    with pytest.raises(qbvh.QbvhError) as e:
+        nl2.neighbors(np.ones((2, 2), np.float32))
+    assert e.value.code == qbvh.ERR_TYPE_RANGE
+    small = torch.empty(1024, dtype=torch.uint8, device="cuda")
+    qbvh.qbvh_set_workspace(small)
+    with pytest.raises(qbvh.QbvhError) as e:
+        qbvh.qbvh_build(pos, None, w.N, w.box)
+    assert e.value.code == qbvh.ERR_WORKSPACE
+
+
+def test_determinism_and_rebuild():
+    w = W.make_config(2, small=True)
+    a = gpu_run(w, K=4, export=True)
+    b = gpu_run(w, K=4, export=True)
+    assert np.array_equal(a["nodes"], b["nodes"]) and np.array_equal(a["perm"], b["perm"])
+    assert np.array_equal(np.sort(np.where(a["nlist"] < 0, 1 << 30, a["nlist"]), 1),
+                          np.sort(np.where(b["nlist"] < 0, 1 << 30, b["nlist"]), 1))
+
+
+@pytest.mark.parametrize("cid", [1, 3, 5])
+def test_census_matches_algorithm1_replay(cid):
+    """K = 1 is the paper's tree; the instrumented traversal must take exactly the oracle's decisions:
+    same number of node tests, leaf-box overlaps and overlapping images (PAPER.md:198 census)."""
+    w = W.make_config(cid, small=True)
+    out = gpu_run(w, K=1, stats=True)
+    t = OT.build(w.pos, w.type, w.box, T=w.T)
+    tr = OT.traverse(t, w.box, w.r_list)
+    s = out["stats"]
+    assert s["node_tests"] == int(tr["n_tests"].sum())
+    assert s["leaf_overlaps"] == int(tr["n_overlap"].sum()) == s["dist_checks"]
+    assert s["images"] == int(tr["n_images"].sum())
+    assert s["neighbors"] == int(out["n_neigh"].sum())
+
+
+@pytest.mark.parametrize("rho,key", [(0.2, "false_pos_per_particle_rho0.2"), (0.8, "false_pos_per_particle_rho0.8")])
+def test_false_positive_census_vs_paper(rho, key):
+    """1.5 / 3.8 false-positive neighbors per particle (N=128,000, r_c=3.0) — measured on the GPU."""
+    from conftest import read_golden
+    paper = {k: float(v) for k, v, _ in read_golden("paper_constants.txt")}[key]
+    w = W.lj_uniform(N=128_000, rho=rho, r_list=3.0, config_id=100, max_neigh=160)
+    out = gpu_run(w, K=1, stats=True)
+    s = out["stats"]
+    fp = (s["leaf_overlaps"] - w.N - s["neighbors"]) / w.N
+    assert abs(fp - paper) / paper < 0.12, (fp, paper)
+
+
+def test_host_buffer_api_matches_device_api():
+    import torch
+    from paper_1901_08088_b200 import qbvh
+    w = W.make_config(3, small=True)
+    dev_out = gpu_run(w, K=4)
+    qbvh.qbvh_set_num_types(w.T)
+    ws = torch.empty(qbvh.qbvh_workspace_bytes(w.N, w.T), dtype=torch.uint8, device="cuda")
+    stg = torch.empty(qbvh.qbvh_staging_bytes(w.N, w.max_neigh), dtype=torch.uint8, device="cuda")
+    qbvh.qbvh_set_workspace(ws)
+    qbvh.qbvh_set_staging(stg)
+    pos = torch.from_numpy(w.pos).pin_memory()
+    typ = torch.from_numpy(w.type).pin_memory()
+    nlist = torch.empty((w.N, w.max_neigh), dtype=torch.int32).pin_memory()
+    n_neigh = torch.empty(w.N, dtype=torch.int32).pin_memory()
+    qbvh.qbvh_build_host(pos, typ, w.N, w.box)
+    M = qbvh.qbvh_neighbors_host(w.r_list, nlist, n_neigh, w.max_neigh)
+    assert M == dev_out["M"] and np.array_equal(n_neigh.numpy(), dev_out["n_neigh"])
+    out = {"M": M, "max_neigh": w.max_neigh, "nlist": nlist.numpy(), "n_neigh": n_neigh.numpy()}
+    compare_with_oracle(w, out, ON.neighbor_list(w.pos, w.type, w.box, w.r_list))
+    qbvh.qbvh_set_staging(None)
