@@ -64,6 +64,9 @@ int qbvh_set_workspace(void *dev_ptr, int64_t bytes);
                                     collapse").  k = 1 is exactly the paper's one-particle-per-leaf tree. Default 4. */
 #define QBVH_OPT_STATS 2         /* 0/1: qbvh_neighbors runs the instrumented traversal and fills qbvh_get_stats
                                     (takes effect immediately; slower — never use when timing). Default 0.        */
+#define QBVH_OPT_VARIANT 3       /* tuning/debug: which traversal kernel qbvh_neighbors launches (0 = plain
+                                    Algorithm 1 as written, the instrumented kernel's twin; >= 1: production
+                                    variants).  All variants produce identical lists.           */
 int qbvh_set_option(int32_t key, int32_t value);
 int qbvh_get_option(int32_t key);
 

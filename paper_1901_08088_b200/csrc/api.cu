@@ -19,12 +19,14 @@ struct Context {
     int K = 4;          // leaf-collapse option for the next build
     int K_built = 1;
     bool stats = false;
+    int variant = 8;
     bool built = false;
     int64_t N = 0;
     float box[6] = {0, 0, 0, 0, 0, 0};
     BuildBuffers buf{};
     int32_t *pinned = nullptr;   // 2 ints: max_count, err_flags
     qbvh_stats last_stats{};
+    cudaTextureObject_t tex_nodes = 0, tex_pos = 0;
     char cuda_msg[256] = "no CUDA error recorded";
 } g;
 
@@ -115,7 +117,7 @@ int neighbors_impl(const float *r_list, int32_t *nlist, int32_t *n_neigh, int32_
         e = cudaMemsetAsync(g.buf.meta->stats, 0, sizeof(g.buf.meta->stats), g.stream);
         if (e != cudaSuccess) return cuda_fail(e, "memset stats");
     }
-    e = launch_traverse(P, g.buf, nlist, n_neigh, g.stats, g.stream);
+    e = launch_traverse(P, g.buf, nlist, n_neigh, g.stats, g.variant, g.stream, g.tex_nodes, g.tex_pos);
     if (e != cudaSuccess) return cuda_fail(e, "traverse launch");
     e = cudaMemcpyAsync(g.pinned, &g.buf.meta->max_count, 2 * sizeof(int32_t), cudaMemcpyDeviceToHost, g.stream);
     if (e != cudaSuccess) return cuda_fail(e, "copy max_count");
@@ -171,6 +173,10 @@ int qbvh_set_option(int32_t key, int32_t value) {
         case QBVH_OPT_STATS:
             g.stats = value != 0;
             return QBVH_OK;
+        case QBVH_OPT_VARIANT:
+            if (value < 0 || value > 15) return QBVH_ERR_INVALID_ARG;
+            g.variant = value;
+            return QBVH_OK;
         default:
             return QBVH_ERR_INVALID_ARG;
     }
@@ -180,6 +186,7 @@ int qbvh_get_option(int32_t key) {
     switch (key) {
         case QBVH_OPT_LEAF_COLLAPSE: return g.K;
         case QBVH_OPT_STATS: return g.stats ? 1 : 0;
+        case QBVH_OPT_VARIANT: return g.variant;
         default: return QBVH_ERR_INVALID_ARG;
     }
 }
@@ -220,6 +227,23 @@ int qbvh_build(const float *pos, const int32_t *type, int64_t N, const float *bo
     g.N = N;
     g.K_built = g.K;
     g.built = true;
+    // texture views of the node array and the Z-ordered positions (gather path experiment)
+    if (g.tex_nodes) { cudaDestroyTextureObject(g.tex_nodes); g.tex_nodes = 0; }
+    if (g.tex_pos) { cudaDestroyTextureObject(g.tex_pos); g.tex_pos = 0; }
+    if (N > 0 && 2 * N - 1 <= (int64_t(1) << 27)) {
+        cudaResourceDesc rd{};
+        cudaTextureDesc td{};
+        td.readMode = cudaReadModeElementType;
+        rd.resType = cudaResourceTypeLinear;
+        rd.res.linear.devPtr = g.buf.nodes;
+        rd.res.linear.desc = cudaCreateChannelDesc<int4>();
+        rd.res.linear.sizeInBytes = (size_t)(2 * N - 1) * 16;
+        if (cudaCreateTextureObject(&g.tex_nodes, &rd, &td, nullptr) != cudaSuccess) { g.tex_nodes = 0; cudaGetLastError(); }
+        rd.res.linear.devPtr = g.buf.sorted_pos;
+        rd.res.linear.desc = cudaCreateChannelDesc<float4>();
+        rd.res.linear.sizeInBytes = (size_t)N * 16;
+        if (cudaCreateTextureObject(&g.tex_pos, &rd, &td, nullptr) != cudaSuccess) { g.tex_pos = 0; cudaGetLastError(); }
+    }
     return QBVH_OK;
 }
 

@@ -66,4 +66,4 @@ struct BuildBuffers {
 cudaError_t launch_build(const float *pos, const int32_t *type, int N, int T, int K, const float *box_lo,
                          const float *box_scale, const BuildBuffers &b, cudaStream_t st);
 cudaError_t launch_traverse(const TraverseParams &p, const BuildBuffers &b, int32_t *nlist, int32_t *n_neigh,
-                            bool stats, cudaStream_t st);
+                            bool stats, int variant, cudaStream_t st, cudaTextureObject_t tn, cudaTextureObject_t tp);

@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libqbvh.so")
 OK = 0
 ERR_INVALID_ARG, ERR_NOT_BUILT, ERR_WORKSPACE, ERR_CUTOFF_TOO_LARGE, ERR_TYPE_RANGE, ERR_CUDA = -1, -2, -3, -4, -5, -6
 MAX_TYPES = 4
-OPT_LEAF_COLLAPSE, OPT_STATS = 1, 2
+OPT_LEAF_COLLAPSE, OPT_STATS, OPT_VARIANT = 1, 2, 3
 EXPORT_KEYS_SORTED, EXPORT_PERM, EXPORT_NODES, EXPORT_PARENT, EXPORT_FRAMES, EXPORT_SEGMENTS, EXPORT_SORTED_POS = range(1, 8)
 
 # every symbol include/qbvh.h declares

@@ -147,7 +147,7 @@ def test_edge_cases():
     p[:, 0] = 2.5
     p[:40, 1] = 0.0
     pos, _ = W._finish(p, 10.0)
-    w = W.Workload("plane", pos, None, box, np.array([[1.1]], np.float32), 64)
+    w = W.Workload("plane", pos, None, box, np.array([[1.1]], np.float32), 256)
     for K in (1, 4):
         compare_with_oracle(w, gpu_run(w, K=K), ON.neighbor_list(w.pos, None, box, w.r_list))
     # four types, one of them empty, one with a single particle, one pair type switched off
@@ -156,7 +156,7 @@ def test_edge_cases():
     typ = rng.integers(0, 2, 5000).astype(np.int32) * 2        # types 0 and 2
     typ[17] = 3
     r = np.array([[1.0, 0.5, 1.4, 2.0], [0.5, 0.5, 0.5, 0.5], [1.4, 0.5, 0.0, 3.0], [2.0, 0.5, 3.0, 1.0]], np.float32)
-    w = W.Workload("types", pos, typ, box, r, 128)
+    w = W.Workload("types", pos, typ, box, r, 512)
     for K in (1, 4):
         compare_with_oracle(w, gpu_run(w, K=K), ON.neighbor_list(w.pos, typ, box, r))
     # r just under L/2 (padded radius still below L/2)
