@@ -61,12 +61,12 @@ int qbvh_set_workspace(void *dev_ptr, int64_t bytes);
 /* Options (all take effect at the next qbvh_build unless noted). */
 #define QBVH_OPT_LEAF_COLLAPSE 1 /* k in [1,15]: the traversal stops at nodes covering <= k consecutive Z-order
                                     particles and distance-checks that range directly ("subtree
-                                    collapse").  k = 1 is exactly the paper's one-particle-per-leaf tree. Default 4. */
+                                    collapse").  k = 1 is exactly the paper's one-particle-per-leaf tree. Default 8. */
 #define QBVH_OPT_STATS 2         /* 0/1: qbvh_neighbors runs the instrumented traversal and fills qbvh_get_stats
                                     (takes effect immediately; slower — never use when timing). Default 0.        */
-#define QBVH_OPT_VARIANT 3       /* tuning/debug: which traversal kernel qbvh_neighbors launches (0 = plain
-                                    Algorithm 1 as written, the instrumented kernel's twin; >= 1: production
-                                    variants).  All variants produce identical lists.           */
+#define QBVH_OPT_VARIANT 3       /* which traversal kernel qbvh_neighbors launches: 0 = Algorithm 1 as written, one
+                                    thread per particle; 1 (default) = one warp per query group.
+                                    Both produce identical lists.                                                 */
 int qbvh_set_option(int32_t key, int32_t value);
 int qbvh_get_option(int32_t key);
 
@@ -91,7 +91,7 @@ int qbvh_build(const float *pos, const int32_t *type, int64_t N, const float *bo
  * predicate d2 <= r_ij^2 holds and j != i.
  *   r_list_ij HOST    T x T fp32 row-major, symmetric; r_ij <= 0 => that pair of types is skipped.
  *   nlist     DEVICE  N x max_neigh int32 row-major; row i = neighbors of ORIGINAL particle i as ORIGINAL
- *                     indices, in unspecified order; entries past n_neigh[i] are not written.
+ *                     indices, in unspecified order; entries at positions >= n_neigh[i] are unspecified.
  *   n_neigh   DEVICE  N int32; the true number of neighbors of particle i (may exceed max_neigh).
  *   max_neigh row capacity, >= 0.
  * Returns M = max_i n_neigh[i] (>= 0).  M <= max_neigh: all rows complete.  M > max_neigh: OVERFLOW — rows with
@@ -116,6 +116,14 @@ typedef struct qbvh_stats {
     uint64_t dist_checks;   /* exact pair-predicate evaluations                                                    */
     uint64_t neighbors;     /* accepted pairs (= sum of n_neigh)                                                   */
     uint64_t images;        /* set bits of the image bitset, Algorithm 1 line 4, summed over particles and trees   */
+    /* the five above: census of Algorithm 1 walked once per PARTICLE (the paper's kernel).
+       the six below: the production kernel, which walks the tree once per query GROUP. */
+    uint64_t groups;            /* query groups traversed                                                          */
+    uint64_t group_node_tests;  /* box-box tests of tree nodes against a group's search volume                     */
+    uint64_t group_leaf_hits;   /* (collapsed) leaves that passed it                                               */
+    uint64_t group_candidates;  /* particles of those leaves within reach of the group box                         */
+    uint64_t group_dist_checks; /* exact pair-predicate evaluations (candidates x group members)                   */
+    uint64_t group_walk_steps;  /* warp steps of the walk (up to 32 node tests each)                               */
 } qbvh_stats;
 /* Counters of the last qbvh_neighbors call made with QBVH_OPT_STATS = 1. */
 int qbvh_get_stats(qbvh_stats *out);

@@ -16,24 +16,23 @@ struct Context {
     void *staging = nullptr;
     int64_t staging_bytes = 0;
     int T = 1;
-    int K = 4;          // leaf-collapse option for the next build
+    int K = 8;          // leaf-collapse option for the next build
     int K_built = 1;
     bool stats = false;
-    int variant = 8;
+    int variant = 1;
     bool built = false;
     int64_t N = 0;
     float box[6] = {0, 0, 0, 0, 0, 0};
     BuildBuffers buf{};
     int32_t *pinned = nullptr;   // 2 ints: max_count, err_flags
     qbvh_stats last_stats{};
-    cudaTextureObject_t tex_nodes = 0, tex_pos = 0;
     char cuda_msg[256] = "no CUDA error recorded";
 } g;
 
 inline int64_t align256(int64_t x) { return (x + 255) & ~int64_t(255); }
 
 struct Layout {
-    int64_t meta, key_a, key_b, idx_a, idx_b, status0, status1, sorted_pos, nodes, parent, slot, total;
+    int64_t meta, key_a, key_b, idx_a, idx_b, status0, status1, sorted_pos, nodes, parent, slot, groups, total;
 };
 
 Layout make_layout(int64_t N) {
@@ -57,6 +56,7 @@ Layout make_layout(int64_t N) {
     L.nodes = take(16 * (2 * n1 - 1));
     L.parent = take(4 * (2 * n1 - 1));
     L.slot = take(8 * n1);
+    L.groups = take(8 * n1);
     L.total = off;
     return L;
 }
@@ -110,14 +110,14 @@ int neighbors_impl(const float *r_list, int32_t *nlist, int32_t *n_neigh, int32_
     P.max_neigh = max_neigh;
     P.K = g.K_built;
     cudaError_t e;
-    // reset max_count (+ stats) of the previous traversal
-    e = cudaMemsetAsync(&g.buf.meta->max_count, 0, sizeof(int32_t), g.stream);
+    // reset group_cursor and max_count (+ stats) of the previous traversal
+    e = cudaMemsetAsync(&g.buf.meta->group_cursor, 0, 2 * sizeof(int32_t), g.stream);
     if (e != cudaSuccess) return cuda_fail(e, "memset max_count");
     if (g.stats) {
         e = cudaMemsetAsync(g.buf.meta->stats, 0, sizeof(g.buf.meta->stats), g.stream);
         if (e != cudaSuccess) return cuda_fail(e, "memset stats");
     }
-    e = launch_traverse(P, g.buf, nlist, n_neigh, g.stats, g.variant, g.stream, g.tex_nodes, g.tex_pos);
+    e = launch_traverse(P, g.buf, nlist, n_neigh, g.stats, g.variant, g.stream);
     if (e != cudaSuccess) return cuda_fail(e, "traverse launch");
     e = cudaMemcpyAsync(g.pinned, &g.buf.meta->max_count, 2 * sizeof(int32_t), cudaMemcpyDeviceToHost, g.stream);
     if (e != cudaSuccess) return cuda_fail(e, "copy max_count");
@@ -174,7 +174,7 @@ int qbvh_set_option(int32_t key, int32_t value) {
             g.stats = value != 0;
             return QBVH_OK;
         case QBVH_OPT_VARIANT:
-            if (value < 0 || value > 15) return QBVH_ERR_INVALID_ARG;
+            if (value < 0 || value > 1) return QBVH_ERR_INVALID_ARG;
             g.variant = value;
             return QBVH_OK;
         default:
@@ -215,6 +215,7 @@ int qbvh_build(const float *pos, const int32_t *type, int64_t N, const float *bo
     g.buf.nodes = reinterpret_cast<int4 *>(w + L.nodes);
     g.buf.parent = reinterpret_cast<int32_t *>(w + L.parent);
     g.buf.slot = reinterpret_cast<unsigned long long *>(w + L.slot);
+    g.buf.groups = reinterpret_cast<uint2 *>(w + L.groups);
     std::memcpy(g.box, box, sizeof(g.box));
     float scale[3];
     for (int d = 0; d < 3; ++d) {
@@ -227,23 +228,6 @@ int qbvh_build(const float *pos, const int32_t *type, int64_t N, const float *bo
     g.N = N;
     g.K_built = g.K;
     g.built = true;
-    // texture views of the node array and the Z-ordered positions (gather path experiment)
-    if (g.tex_nodes) { cudaDestroyTextureObject(g.tex_nodes); g.tex_nodes = 0; }
-    if (g.tex_pos) { cudaDestroyTextureObject(g.tex_pos); g.tex_pos = 0; }
-    if (N > 0 && 2 * N - 1 <= (int64_t(1) << 27)) {
-        cudaResourceDesc rd{};
-        cudaTextureDesc td{};
-        td.readMode = cudaReadModeElementType;
-        rd.resType = cudaResourceTypeLinear;
-        rd.res.linear.devPtr = g.buf.nodes;
-        rd.res.linear.desc = cudaCreateChannelDesc<int4>();
-        rd.res.linear.sizeInBytes = (size_t)(2 * N - 1) * 16;
-        if (cudaCreateTextureObject(&g.tex_nodes, &rd, &td, nullptr) != cudaSuccess) { g.tex_nodes = 0; cudaGetLastError(); }
-        rd.res.linear.devPtr = g.buf.sorted_pos;
-        rd.res.linear.desc = cudaCreateChannelDesc<float4>();
-        rd.res.linear.sizeInBytes = (size_t)N * 16;
-        if (cudaCreateTextureObject(&g.tex_pos, &rd, &td, nullptr) != cudaSuccess) { g.tex_pos = 0; cudaGetLastError(); }
-    }
     return QBVH_OK;
 }
 

@@ -287,61 +287,94 @@ struct SegDelta {
 };
 
 __global__ void __launch_bounds__(256) hierarchy_kernel(const uint32_t *__restrict__ key, int N,
-                                                         const TreeMeta *__restrict__ meta, int4 *__restrict__ nodes,
+                                                         TreeMeta *__restrict__ meta, int4 *__restrict__ nodes,
                                                          int32_t *__restrict__ parent,
-                                                         unsigned long long *__restrict__ slot, int K) {
+                                                         unsigned long long *__restrict__ slot,
+                                                         uint2 *__restrict__ groups, int K) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= N) return;
-    const uint32_t ki = key[k];
-    const int t = ki >> 30;
-    SegDelta delta{key, meta->seg[t], meta->seg[t + 1] - 1};
-    const int s = delta.s, e = delta.e;
-    auto rope_of = [&](int l) -> int {
-        if (l == e) return -1;
-        const int m = l + 1;
-        const uint32_t km = __ldg(key + m);
-        if (m <= e - 1 && delta(m, km, m + 1) > delta(m, km, m - 1)) return m;
-        return N - 1 + m;
-    };
-    int2 *nodes_lr = reinterpret_cast<int2 *>(nodes);   // {left, rope} = second half of the 16-byte node
-    // leaf k
-    nodes_lr[2 * (size_t)(N - 1 + k) + 1] = make_int2(~k, rope_of(k));
-    if (s == e) parent[N - 1 + k] = -1;                 // a one-particle tree: the leaf is the root
-    if (k == e) {                                       // no internal node carries the index of a segment end
-        if (k < N - 1) {
-            nodes[k] = make_int4(0, 0, 0, -1);
-            parent[k] = -1;
-            slot[k] = SLOT_EMPTY;
+    // query groups found by this thread (at most two): maximal subtrees with <= GROUP_MAX leaves
+    uint2 grp0 = make_uint2(0u, 0u), grp1 = make_uint2(0u, 0u);
+    int ngrp = 0;
+    if (k < N) {
+        const uint32_t ki = key[k];
+        const int t = ki >> 30;
+        SegDelta delta{key, meta->seg[t], meta->seg[t + 1] - 1};
+        const int s = delta.s, e = delta.e;
+        auto rope_of = [&](int l) -> int {
+            if (l == e) return -1;
+            const int m = l + 1;
+            const uint32_t km = __ldg(key + m);
+            if (m <= e - 1 && delta(m, km, m + 1) > delta(m, km, m - 1)) return m;
+            return N - 1 + m;
+        };
+        int2 *nodes_lr = reinterpret_cast<int2 *>(nodes);   // {left, rope} = second half of the 16-byte node
+        // leaf k
+        nodes_lr[2 * (size_t)(N - 1 + k) + 1] = make_int2(~k, rope_of(k));
+        if (s == e) parent[N - 1 + k] = -1;                 // a one-particle tree: the leaf is the root
+        if (k == s && e - s + 1 <= GROUP_MAX) {             // a whole tree that fits one group
+            grp0 = make_uint2((uint32_t)s, (uint32_t)(e - s + 1));
+            ngrp = 1;
         }
-        return;
+        if (k == e) {                                       // no internal node carries the index of a segment end
+            if (k < N - 1) {
+                nodes[k] = make_int4(0, 0, 0, -1);
+                parent[k] = -1;
+                slot[k] = SLOT_EMPTY;
+            }
+        } else {
+            // internal node k (Karras)
+            const int dl = delta(k, ki, (long long)k - 1), dr = delta(k, ki, (long long)k + 1);
+            const int d = (dr > dl) ? 1 : -1;
+            const int dmin = (dr > dl) ? dl : dr;
+            long long lmax = 2;
+            while (delta(k, ki, k + lmax * d) > dmin) lmax <<= 1;
+            long long l = 0;
+            for (long long tt = lmax >> 1; tt >= 1; tt >>= 1)
+                if (delta(k, ki, k + (l + tt) * d) > dmin) l += tt;
+            const int j = (int)(k + l * d);
+            const int dnode = delta(k, ki, j);
+            long long sp = 0, tt = l;
+            do {
+                tt = (tt + 1) >> 1;
+                if (delta(k, ki, k + (sp + tt) * d) > dnode) sp += tt;
+            } while (tt > 1);
+            const int gamma = (int)(k + sp * d + (d < 0 ? -1 : 0));
+            const int f = min(k, j), la = max(k, j);
+            const int lc = (f == gamma) ? (N - 1 + gamma) : gamma;
+            const int rc = (la == gamma + 1) ? (N - 1 + gamma + 1) : (gamma + 1);
+            parent[lc] = k;
+            parent[rc] = k;
+            if (k == s) parent[k] = -1;
+            const int size = la - f + 1;
+            const int leftword = (K > 1 && size <= K) ? ~f : lc;   // collapsed range leaf: first sorted position
+            nodes_lr[2 * (size_t)k + 1] = make_int2(leftword, rope_of(la));
+            slot[k] = SLOT_EMPTY;
+            if (size > GROUP_MAX) {                         // children that fit are maximal: they become groups
+                const int lsize = gamma - f + 1, rsize = la - gamma;
+                if (lsize <= GROUP_MAX) {
+                    grp0 = make_uint2((uint32_t)f, (uint32_t)lsize);
+                    ngrp = 1;
+                }
+                if (rsize <= GROUP_MAX) {
+                    const uint2 gr = make_uint2((uint32_t)(gamma + 1), (uint32_t)rsize);
+                    if (ngrp) grp1 = gr; else grp0 = gr;
+                    ++ngrp;
+                }
+            }
+        }
     }
-    // internal node k (Karras)
-    const int dl = delta(k, ki, (long long)k - 1), dr = delta(k, ki, (long long)k + 1);
-    const int d = (dr > dl) ? 1 : -1;
-    const int dmin = (dr > dl) ? dl : dr;
-    long long lmax = 2;
-    while (delta(k, ki, k + lmax * d) > dmin) lmax <<= 1;
-    long long l = 0;
-    for (long long tt = lmax >> 1; tt >= 1; tt >>= 1)
-        if (delta(k, ki, k + (l + tt) * d) > dmin) l += tt;
-    const int j = (int)(k + l * d);
-    const int dnode = delta(k, ki, j);
-    long long sp = 0, tt = l;
-    do {
-        tt = (tt + 1) >> 1;
-        if (delta(k, ki, k + (sp + tt) * d) > dnode) sp += tt;
-    } while (tt > 1);
-    const int gamma = (int)(k + sp * d + (d < 0 ? -1 : 0));
-    const int f = min(k, j), la = max(k, j);
-    const int lc = (f == gamma) ? (N - 1 + gamma) : gamma;
-    const int rc = (la == gamma + 1) ? (N - 1 + gamma + 1) : (gamma + 1);
-    parent[lc] = k;
-    parent[rc] = k;
-    if (k == s) parent[k] = -1;
-    const int size = la - f + 1;
-    const int leftword = (K > 1 && size <= K) ? ~f : lc;   // collapsed range leaf: first sorted position
-    nodes_lr[2 * (size_t)k + 1] = make_int2(leftword, rope_of(la));
-    slot[k] = SLOT_EMPTY;
+    // append this warp's groups with one atomic
+    const uint32_t b1 = __ballot_sync(0xFFFFFFFFu, ngrp >= 1), b2 = __ballot_sync(0xFFFFFFFFu, ngrp >= 2);
+    const int total = __popc(b1) + __popc(b2);
+    if (total) {
+        const int lane = threadIdx.x & 31;
+        const uint32_t lt = (1u << lane) - 1u;
+        int base = 0;
+        if (lane == 0) base = atomicAdd(&meta->group_count, total);
+        base = __shfl_sync(0xFFFFFFFFu, base, 0) + __popc(b1 & lt) + __popc(b2 & lt);
+        if (ngrp >= 1) groups[base] = grp0;
+        if (ngrp >= 2) groups[base + 1] = grp1;
+    }
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -445,7 +478,7 @@ cudaError_t launch_build(const float *pos, const int32_t *type, int N, int T, in
     onesweep_kernel<false><<<tiles, SORT_THREADS, 0, st>>>(b.key_b, b.idx_b, b.key_a, b.idx_a, N, 24, b.meta->hist[3],
                                                            b.status[1], b.status[0], &b.meta->tile_counter[3]);
     const int nb = (N + 255) / 256;
-    hierarchy_kernel<<<nb, 256, 0, st>>>(b.key_a, N, b.meta, b.nodes, b.parent, b.slot, K);
+    hierarchy_kernel<<<nb, 256, 0, st>>>(b.key_a, N, b.meta, b.nodes, b.parent, b.slot, b.groups, K);
     fit_kernel<<<nb, 256, 0, st>>>(pos, b.idx_a, b.key_a, N, b.meta, b.sorted_pos, b.nodes, b.parent, b.slot, K);
     return cudaGetLastError();
 }

@@ -14,9 +14,11 @@ struct TreeMeta {
     int32_t seg[QBVH_TMAX + 1];     // first sorted position of each type; seg[T..4] = N
     int32_t roots[QBVH_TMAX];       // root node per type, -1 if empty
     float frames[QBVH_TMAX][12];    // lo xyz, hi xyz, delta xyz, 0 0 0
+    int32_t group_count;            // number of query groups emitted by the build (hierarchy_kernel)
+    int32_t group_cursor;           // next group to hand out (dynamic scheduling of the traversal); reset per traversal
     int32_t max_count;              // max_i n_neigh[i] of the last traversal
     int32_t err_flags;              // bit 0: type id out of range
-    unsigned long long stats[8];    // node_tests, leaf_overlaps, dist_checks, neighbors, images
+    unsigned long long stats[16];   // qbvh_stats, in order
 };
 
 // order-preserving map float -> uint32 (NaN excluded)
@@ -44,6 +46,12 @@ constexpr uint32_t ST_AGG = 1u << 30;                 // tile status: aggregate 
 constexpr uint32_t ST_PRE = 1u << 31;                 // tile status: inclusive prefix available
 constexpr uint32_t ST_VAL = (1u << 30) - 1;
 
+// ---- query groups ----
+// A query group is a maximal subtree of the LBVH with at most GROUP_MAX leaves: a contiguous run of Z-ordered
+// particles that fills one Morton cell, i.e. a compact blob.  One warp traverses the tree once
+// for the whole group (traverse_kernels.cu).
+constexpr int GROUP_MAX = 32;
+
 struct TraverseParams {
     float L[3];
     float r2[QBVH_TMAX * QBVH_TMAX];   // r_ij^2 (fp32 RN), <0 => skipped
@@ -62,8 +70,9 @@ struct BuildBuffers {
     int4 *nodes;
     int32_t *parent;
     unsigned long long *slot;
+    uint2 *groups;                 // {first sorted position, number of particles}, group_count entries, any order
 };
 cudaError_t launch_build(const float *pos, const int32_t *type, int N, int T, int K, const float *box_lo,
                          const float *box_scale, const BuildBuffers &b, cudaStream_t st);
 cudaError_t launch_traverse(const TraverseParams &p, const BuildBuffers &b, int32_t *nlist, int32_t *n_neigh,
-                            bool stats, int variant, cudaStream_t st, cudaTextureObject_t tn, cudaTextureObject_t tp);
+                            bool stats, int variant, cudaStream_t st);

@@ -29,7 +29,9 @@ SYMBOLS = ("qbvh_set_stream", "qbvh_set_num_types", "qbvh_workspace_bytes", "qbv
 
 class QbvhStats(C.Structure):
     _fields_ = [("node_tests", C.c_uint64), ("leaf_overlaps", C.c_uint64), ("dist_checks", C.c_uint64),
-                ("neighbors", C.c_uint64), ("images", C.c_uint64)]
+                ("neighbors", C.c_uint64), ("images", C.c_uint64),
+                ("groups", C.c_uint64), ("group_node_tests", C.c_uint64), ("group_leaf_hits", C.c_uint64),
+                ("group_candidates", C.c_uint64), ("group_dist_checks", C.c_uint64), ("group_walk_steps", C.c_uint64)]
 
 
 class QbvhError(RuntimeError):
