@@ -59,7 +59,7 @@ int64_t qbvh_workspace_bytes(int64_t N, int32_t T);
 int qbvh_set_workspace(void *dev_ptr, int64_t bytes);
 
 /* Options (all take effect at the next qbvh_build unless noted). */
-#define QBVH_OPT_LEAF_COLLAPSE 1 /* k in [1,15]: the traversal stops at nodes covering <= k consecutive Z-order
+#define QBVH_OPT_LEAF_COLLAPSE 1 /* k in [1,32]: the traversal stops at nodes covering <= k consecutive Z-order
                                     particles and distance-checks that range directly ("subtree
                                     collapse").  k = 1 is exactly the paper's one-particle-per-leaf tree. Default 8. */
 #define QBVH_OPT_STATS 2         /* 0/1: qbvh_neighbors runs the instrumented traversal and fills qbvh_get_stats

@@ -23,6 +23,7 @@ struct Context {
     bool built = false;
     int64_t N = 0;
     float box[6] = {0, 0, 0, 0, 0, 0};
+    float scale[3] = {0, 0, 0};
     BuildBuffers buf{};
     int32_t *pinned = nullptr;   // 2 ints: max_count, err_flags
     qbvh_stats last_stats{};
@@ -32,7 +33,7 @@ struct Context {
 inline int64_t align256(int64_t x) { return (x + 255) & ~int64_t(255); }
 
 struct Layout {
-    int64_t meta, key_a, key_b, idx_a, idx_b, status0, status1, sorted_pos, nodes, parent, slot, groups, total;
+    int64_t meta, key_a, key_b, idx_a, idx_b, status0, status1, sorted_pos, nodes, parent, slot, groups, entry, total;
 };
 
 Layout make_layout(int64_t N) {
@@ -57,6 +58,7 @@ Layout make_layout(int64_t N) {
     L.parent = take(4 * (2 * n1 - 1));
     L.slot = take(8 * n1);
     L.groups = take(8 * n1);
+    L.entry = take(4 * (int64_t)QBVH_TMAX * ENTRY_CELLS);
     L.total = off;
     return L;
 }
@@ -92,8 +94,12 @@ int neighbors_impl(const float *r_list, int32_t *nlist, int32_t *n_neigh, int32_
     if (!r_list || max_neigh < 0) return QBVH_ERR_INVALID_ARG;
     if (g.N > 0 && (!n_neigh || (!nlist && max_neigh > 0))) return QBVH_ERR_INVALID_ARG;
     TraverseParams P{};
-    for (int d = 0; d < 3; ++d) P.L[d] = g.box[3 + d];
-    for (int k = 0; k < QBVH_TMAX * QBVH_TMAX; ++k) P.r2[k] = P.R2[k] = -1.0f;
+    for (int d = 0; d < 3; ++d) {
+        P.L[d] = g.box[3 + d];
+        P.box_lo[d] = g.box[d];
+        P.scale[d] = g.scale[d];
+    }
+    for (int k = 0; k < QBVH_TMAX * QBVH_TMAX; ++k) P.r2[k] = P.R2[k] = P.Rp[k] = -1.0f;
     for (int a = 0; a < g.T; ++a)
         for (int b = 0; b < g.T; ++b) {
             const float r = r_list[a * g.T + b];
@@ -105,6 +111,7 @@ int neighbors_impl(const float *r_list, int32_t *nlist, int32_t *n_neigh, int32_
             volatile float r2 = r * r;
             P.r2[a * QBVH_TMAX + b] = r2;
             P.R2[a * QBVH_TMAX + b] = mul_ru(rp, rp);
+            P.Rp[a * QBVH_TMAX + b] = rp;
         }
     P.N = (int32_t)g.N;
     P.max_neigh = max_neigh;
@@ -167,7 +174,7 @@ int qbvh_set_workspace(void *dev_ptr, int64_t bytes) {
 int qbvh_set_option(int32_t key, int32_t value) {
     switch (key) {
         case QBVH_OPT_LEAF_COLLAPSE:
-            if (value < 1 || value > 15) return QBVH_ERR_INVALID_ARG;
+            if (value < 1 || value > 32) return QBVH_ERR_INVALID_ARG;
             g.K = value;
             return QBVH_OK;
         case QBVH_OPT_STATS:
@@ -216,12 +223,14 @@ int qbvh_build(const float *pos, const int32_t *type, int64_t N, const float *bo
     g.buf.parent = reinterpret_cast<int32_t *>(w + L.parent);
     g.buf.slot = reinterpret_cast<unsigned long long *>(w + L.slot);
     g.buf.groups = reinterpret_cast<uint2 *>(w + L.groups);
+    g.buf.entry = reinterpret_cast<int32_t *>(w + L.entry);
     std::memcpy(g.box, box, sizeof(g.box));
     float scale[3];
     for (int d = 0; d < 3; ++d) {
         volatile float s = 1023.0f / box[3 + d];   // fp32 RN
         scale[d] = s;
     }
+    for (int d = 0; d < 3; ++d) g.scale[d] = scale[d];
     const int T = type ? g.T : 1;
     cudaError_t e = launch_build(pos, type, (int)N, T, g.K, box, scale, g.buf, g.stream);
     if (e != cudaSuccess) return cuda_fail(e, "build launch");

@@ -5,6 +5,7 @@
 //   a2  onesweep_kernel    : stable LSD radix sort, 8-bit digits, one kernel per pass with chained-scan
 //                            decoupled look-back between tiles (the paper used CUB)
 //   a3+a4 hierarchy_kernel : Karras binary radix tree + ropes in closed form
+//       entry_table_kernel : node of every cell of the 4^3 .. 32^3 Morton grids (entry points of the traversal)
 //   a2'+a5+a6 fit_kernel   : gather into Z-order, quantize each leaf onto the 1023-bin grid of its tree's root
 //                            box with outward rounding, then bottom-up union with atomic
 //                            hand-over directly on the packed 10-bit integers
@@ -412,7 +413,7 @@ __global__ void __launch_bounds__(256) fit_kernel(const float *__restrict__ pos,
                                                    const uint32_t *__restrict__ key_sorted, int N,
                                                    const TreeMeta *__restrict__ meta, float4 *__restrict__ sorted_pos,
                                                    int4 *__restrict__ nodes, const int32_t *__restrict__ parent,
-                                                   unsigned long long *__restrict__ slot, int K) {
+                                                   unsigned long long *__restrict__ slot) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= N) return;
     const uint32_t idx = idx_sorted[k];
@@ -423,27 +424,58 @@ __global__ void __launch_bounds__(256) fit_kernel(const float *__restrict__ pos,
     uint32_t whi = quant_hi(x, fr[0], fr[6]) | (quant_hi(y, fr[1], fr[7]) << 10) | (quant_hi(z, fr[2], fr[8]) << 20);
     int2 *nodes_b = reinterpret_cast<int2 *>(nodes);    // {lo, hi} = first half of the 16-byte node
     nodes_b[2 * (size_t)(N - 1 + k)] = make_int2((int)wlo, (int)whi);
-    uint32_t cnt = 0;                                    // (leaves under the node) - 1, saturating at 15
     int n = parent[N - 1 + k];
     while (n >= 0) {
         // hand-over through one 64-bit atomic: the first child to arrive deposits its box, the second merges
-        unsigned long long mine = (unsigned long long)(wlo | ((cnt & 3u) << 30)) |
-                                  ((unsigned long long)(whi | ((cnt >> 2) << 30)) << 32);
-        unsigned long long other = atomicExch(slot + n, mine);
-        if (other == SLOT_EMPTY) break;
-        uint32_t olo = (uint32_t)other, ohi = (uint32_t)(other >> 32);
-        uint32_t ocnt = (olo >> 30) | ((ohi >> 30) << 2);
-        wlo = pack_min(wlo, olo);
-        whi = pack_max(whi, ohi);
-        cnt = min(cnt + ocnt + 1u, 15u);
-        uint32_t slo = wlo, shi = whi;
-        if (K > 1) {                                    // spare bits carry the leaf count for collapsed ranges
-            slo |= (cnt & 3u) << 30;
-            shi |= (cnt >> 2) << 30;
-        }
-        nodes_b[2 * (size_t)n] = make_int2((int)slo, (int)shi);
+        const unsigned long long mine = (unsigned long long)wlo | ((unsigned long long)whi << 32);
+        const unsigned long long other = atomicExch(slot + n, mine);
+        if (other == SLOT_EMPTY) break;                 // a packed box never has bits 30, 31, 62, 63 set
+        wlo = pack_min(wlo, (uint32_t)other);
+        whi = pack_max(whi, (uint32_t)(other >> 32));
+        nodes_b[2 * (size_t)n] = make_int2((int)wlo, (int)whi);
         n = parent[n];
     }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// Entry table.  The upper levels of an LBVH over Morton codes ARE a regular grid: all particles whose code starts
+// with a given 3l-bit prefix (one cell of the 2^l x 2^l x 2^l grid over the box) form one subtree.
+// For l = 2..5 and every cell the table holds the node that roots that subtree (-1: empty cell), so a traversal
+// can enter the tree at the cells its search volume touches instead of walking down from the root.
+// The particles with prefix c are the sorted positions [a, b); the node covering exactly [a, b-1] is internal
+// node b-1 if it is a left child (its keys are closer to the right outside neighbor) and internal node a if it
+// is a right child (SURVEY.md B.1 numbering); a single particle is leaf a.
+// ------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ int lower_bound_key(const uint32_t *__restrict__ key, int N, unsigned long long v) {
+    int lo = 0, hi = N;
+    while (lo < hi) {
+        const int mid = (lo + hi) >> 1;
+        if ((unsigned long long)__ldg(key + mid) < v) lo = mid + 1; else hi = mid;
+    }
+    return lo;
+}
+
+__global__ void __launch_bounds__(256) entry_table_kernel(const uint32_t *__restrict__ key, int N,
+                                                           const TreeMeta *__restrict__ meta,
+                                                           int32_t *__restrict__ table, int T) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= T * ENTRY_CELLS) return;
+    const int t = i / ENTRY_CELLS, r = i - t * ENTRY_CELLS;
+    const int l = (r < entry_offset(3)) ? 2 : (r < entry_offset(4)) ? 3 : (r < entry_offset(5)) ? 4 : 5;
+    const unsigned long long c = (unsigned long long)(r - entry_offset(l));
+    const int shift = 30 - 3 * l;
+    const unsigned long long klo = ((unsigned long long)t << 30) | (c << shift), khi = klo + (1ull << shift);
+    const int a = lower_bound_key(key, N, klo), b = lower_bound_key(key, N, khi);
+    int node = -1;
+    if (b - a == 1) {
+        node = N - 1 + a;
+    } else if (b - a > 1) {
+        const int s = meta->seg[t], e = meta->seg[t + 1] - 1;
+        const int dl = (a - 1 < s) ? -1 : __clz(__ldg(key + a - 1) ^ __ldg(key + a));
+        const int dr = (b > e) ? -1 : __clz(__ldg(key + b - 1) ^ __ldg(key + b));
+        node = (dr > dl) ? b - 1 : a;
+    }
+    table[i] = node;
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -479,6 +511,7 @@ cudaError_t launch_build(const float *pos, const int32_t *type, int N, int T, in
                                                            b.status[1], b.status[0], &b.meta->tile_counter[3]);
     const int nb = (N + 255) / 256;
     hierarchy_kernel<<<nb, 256, 0, st>>>(b.key_a, N, b.meta, b.nodes, b.parent, b.slot, b.groups, K);
-    fit_kernel<<<nb, 256, 0, st>>>(pos, b.idx_a, b.key_a, N, b.meta, b.sorted_pos, b.nodes, b.parent, b.slot, K);
+    fit_kernel<<<nb, 256, 0, st>>>(pos, b.idx_a, b.key_a, N, b.meta, b.sorted_pos, b.nodes, b.parent, b.slot);
+    entry_table_kernel<<<(T * ENTRY_CELLS + 255) / 256, 256, 0, st>>>(b.key_a, N, b.meta, b.entry, T);
     return cudaGetLastError();
 }

@@ -52,10 +52,19 @@ constexpr uint32_t ST_VAL = (1u << 30) - 1;
 // for the whole group (traverse_kernels.cu).
 constexpr int GROUP_MAX = 32;
 
+// ---- entry table: node of every cell of the 2^l-per-axis Morton grids, l = 2..5, per type ----
+constexpr int ENTRY_LMIN = 2, ENTRY_LMAX = 5;
+__host__ __device__ constexpr int entry_offset(int l) {   // cells of the levels below l: 64 + 512 + ...
+    return l <= 2 ? 0 : (l == 3 ? 64 : (l == 4 ? 64 + 512 : 64 + 512 + 4096));
+}
+constexpr int ENTRY_CELLS = 64 + 512 + 4096 + 32768;
+
 struct TraverseParams {
     float L[3];
     float r2[QBVH_TMAX * QBVH_TMAX];   // r_ij^2 (fp32 RN), <0 => skipped
     float R2[QBVH_TMAX * QBVH_TMAX];   // padded pruning radius squared (rounded up)
+    float Rp[QBVH_TMAX * QBVH_TMAX];   // padded pruning radius
+    float box_lo[3], scale[3];         // Morton binning of the build: bin = floor((p - box_lo) * scale)
     int32_t N;
     int32_t max_neigh;
     int32_t K;                         // leaf-collapse threshold used by the build
@@ -71,6 +80,7 @@ struct BuildBuffers {
     int32_t *parent;
     unsigned long long *slot;
     uint2 *groups;                 // {first sorted position, number of particles}, group_count entries, any order
+    int32_t *entry;                // [QBVH_TMAX][ENTRY_CELLS] entry table
 };
 cudaError_t launch_build(const float *pos, const int32_t *type, int N, int T, int K, const float *box_lo,
                          const float *box_scale, const BuildBuffers &b, cudaStream_t st);

@@ -21,6 +21,14 @@ __device__ __forceinline__ void decompress(uint32_t wlo, uint32_t whi, const flo
     }
 }
 
+// Number of particles under a (collapsed) leaf node covering the sorted positions [first, last]: its rope points at
+// the node that starts at last + 1 — leaf N-1+(last+1), or the internal node numbered last+1 (a right child carries
+// the index of its first leaf) — or is END at the end of the tree's segment.
+__device__ __forceinline__ int leaf_count(const int4 nd, int N, int seg_end) {
+    const int next = (nd.w < 0) ? seg_end : (nd.w >= N - 1 ? nd.w - (N - 1) : nd.w);
+    return next - (~nd.z);
+}
+
 template <bool STATS>
 __global__ void __launch_bounds__(128) traverse_kernel(TraverseParams P, const int4 *__restrict__ nodes,
                                                         const float4 *__restrict__ sorted_pos,
@@ -44,6 +52,7 @@ __global__ void __launch_bounds__(128) traverse_kernel(TraverseParams P, const i
             const float *fr = meta->frames[tb];
             const float flo[3] = {fr[0], fr[1], fr[2]};
             const float fdl[3] = {fr[6], fr[7], fr[8]};
+            const int seg_end = meta->seg[tb + 1];
             // ---- line 4: image bitset against the root node ----
             uint32_t bset = 0;
             {
@@ -88,7 +97,7 @@ __global__ void __launch_bounds__(128) traverse_kernel(TraverseParams P, const i
                     if (d2 <= R2) {
                         if (nd.z < 0) {
                             const int first = ~nd.z;
-                            const int m = (P.K > 1) ? 1 + (int)(((uint32_t)nd.x >> 30) | (((uint32_t)nd.y >> 30) << 2)) : 1;
+                            const int m = leaf_count(nd, P.N, seg_end);
                             if (STATS) ++st_leaf;
                             for (int j = first; j < first + m; ++j) {
                                 const float4 pj = __ldg(sorted_pos + j);
@@ -180,7 +189,7 @@ __device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c) {
 
 constexpr int GW_WARPS = 4;      // warps per block
 constexpr int GW_WL = 512;       // work-list entries per warp
-constexpr int GW_LQ = 64;        // leaf-queue entries per warp
+constexpr int GW_LQ = 96;        // leaf-queue entries per warp
 constexpr int GW_TILE = 64;      // candidate tile ring per warp: two halves of 32
 constexpr int GW_RING = 32;      // staged neighbors per lane: two blocks of 16
 
@@ -188,8 +197,9 @@ struct __align__(128) GwShared {
     float tx[GW_TILE], ty[GW_TILE], tz[GW_TILE];   // candidate tile, structure of arrays
     int32_t ti[GW_TILE];                           // original particle index of each candidate
     int32_t ring[32][GW_RING];                     // per-lane staged neighbors
-    uint32_t wl[GW_WL];                            // work list: node id | (is a left child) << 31
+    uint32_t wl[GW_WL];                            // work list: node id | (also test its rope sibling) << 31
     uint2 lq[GW_LQ];                               // leaf queue: {first sorted position, count}
+    int32_t pre[36];                               // exclusive prefix sums of the counts of the leaves being gathered
 };
 
 // append one neighbor to this lane's ring: slot address = ring base | (byte offset mod 128), one LOP3
@@ -242,10 +252,37 @@ __device__ __forceinline__ void store4(int32_t *__restrict__ row, int off, int c
     }
 }
 
+
+// Morton bin of a coordinate: the build's function (build_kernels.cu, a1), restated.  It is monotone in p, which
+// is all the entry-cell selection needs.
+__device__ __forceinline__ int bin_of(float p, float lo, float s) {
+    const float f = fminf(fmaxf(floorf(__fmul_rn(__fsub_rn(p, lo), s)), 0.0f), 1023.0f);
+    return (int)f;
+}
+__device__ __forceinline__ uint32_t spread5(uint32_t v) {   // bit t -> bit 3t, t < 5
+    v = (v | (v << 8)) & 0x0000100Fu;
+    v = (v | (v << 4)) & 0x000010C3u;
+    v = (v | (v << 2)) & 0x00001249u;
+    return v;
+}
+
+// sphere-swept box test of eq. 2 in its box-box form: squared distance between the nearest
+// points of the decompressed node box and the group's box [blo, bhi] <= padded r^2
+__device__ __forceinline__ bool node_overlaps(const int4 nd, const float flo[3], const float fdl[3], const float blo[3],
+                                              const float bhi[3], float R2) {
+    float a[3], b[3];
+    decompress((uint32_t)nd.x, (uint32_t)nd.y, flo, fdl, a, b);
+    const float t0 = fmaxf(fmaxf(__fsub_rn(a[0], bhi[0]), __fsub_rn(blo[0], b[0])), 0.0f);
+    const float t1 = fmaxf(fmaxf(__fsub_rn(a[1], bhi[1]), __fsub_rn(blo[1], b[1])), 0.0f);
+    const float t2 = fmaxf(fmaxf(__fsub_rn(a[2], bhi[2]), __fsub_rn(blo[2], b[2])), 0.0f);
+    return __fmaf_rn(t2, t2, __fmaf_rn(t1, t1, __fmul_rn(t0, t0))) <= R2;
+}
+
 template <bool STATS>
 __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseParams P, const int4 *__restrict__ nodes,
                                                                         const float4 *__restrict__ sorted_pos,
                                                                         const uint2 *__restrict__ groups,
+                                                                        const int32_t *__restrict__ entry,
                                                                         TreeMeta *__restrict__ meta,
                                                                         int32_t *__restrict__ nlist,
                                                                         int32_t *__restrict__ n_neigh) {
@@ -310,25 +347,25 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
             if (!(r2u >= 0.0f)) continue;
             const float r2 = live ? r2u : -1.0f;          // idle lanes never accept
             const float R2 = P.R2[ta * QBVH_TMAX + tb];
+            const float Rp = P.Rp[ta * QBVH_TMAX + tb];
             const float *fr = meta->frames[tb];
             const float flo[3] = {fr[0], fr[1], fr[2]};
             const float fdl[3] = {fr[6], fr[7], fr[8]};
+            const int seg_end = meta->seg[tb + 1];
+            const int32_t *const etab = entry + tb * ENTRY_CELLS;
             // ---- Alg. 1 line 4: lane j tests image j of the group box against the root node; the vote is the bitset ----
             uint32_t bset;
             {
                 const int4 nd = __ldg(nodes + root);
-                float a[3], b[3];
-                decompress((uint32_t)nd.x, (uint32_t)nd.y, flo, fdl, a, b);
                 const int sh[3] = {lane % 3 - 1, (lane / 3) % 3 - 1, lane / 9 - 1};
-                float tq[3];
+                float lo_s[3], hi_s[3];
 #pragma unroll
                 for (int d = 0; d < 3; ++d) {
                     const float sL = (float)sh[d] * P.L[d];
-                    const float lo_s = __fadd_rn(glo[d], sL), hi_s = __fadd_rn(ghi[d], sL);
-                    tq[d] = fmaxf(fmaxf(__fsub_rn(a[d], hi_s), __fsub_rn(lo_s, b[d])), 0.0f);
+                    lo_s[d] = __fadd_rn(glo[d], sL);
+                    hi_s[d] = __fadd_rn(ghi[d], sL);
                 }
-                const float d2 = __fmaf_rn(tq[2], tq[2], __fmaf_rn(tq[1], tq[1], __fmul_rn(tq[0], tq[0])));
-                bset = __ballot_sync(FULL, lane < 27 && d2 <= R2);
+                bset = __ballot_sync(FULL, lane < 27 && node_overlaps(nd, flo, fdl, lo_s, hi_s, R2));
             }
             while (bset) {                                    // lines 5-9
                 const int img = __ffs(bset) - 1;
@@ -341,12 +378,47 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
                 const u64 ns0 = pk2(-s0, -s0), ns1 = pk2(-s1, -s1), ns2 = pk2(-s2, -s2);
                 const bool own_tree = (tb == ta) && !shifted;   // only then can a candidate be a group member
 
-                if (lane == 0) sm.wl[0] = (uint32_t)root;
+                // ---- line 9, "n <- root node": enter at the finest Morton grid whose cells touched by the search
+                //      volume number at most 32 (one per lane); the root itself if even the 4^3 grid has more ----
+                int wsz;
+                {
+                    int c0[3], nc[3], lvl = -1;
+                    int b0[3], b1[3];
+#pragma unroll
+                    for (int d = 0; d < 3; ++d) {
+                        b0[d] = bin_of(__fsub_rd(blo[d], Rp), P.box_lo[d], P.scale[d]);
+                        b1[d] = bin_of(__fadd_ru(bhi[d], Rp), P.box_lo[d], P.scale[d]);
+                    }
+#pragma unroll
+                    for (int l = ENTRY_LMAX; l >= ENTRY_LMIN; --l) {
+                        if (lvl < 0) {
+                            const int n0 = (b1[0] >> (10 - l)) - (b0[0] >> (10 - l)) + 1;
+                            const int n1 = (b1[1] >> (10 - l)) - (b0[1] >> (10 - l)) + 1;
+                            const int n2 = (b1[2] >> (10 - l)) - (b0[2] >> (10 - l)) + 1;
+                            if (n0 * n1 * n2 <= 32) {
+                                lvl = l;
+                                nc[0] = n0, nc[1] = n1, nc[2] = n2;
+                                c0[0] = b0[0] >> (10 - l), c0[1] = b0[1] >> (10 - l), c0[2] = b0[2] >> (10 - l);
+                            }
+                        }
+                    }
+                    int node = -1;
+                    if (lvl < 0) {
+                        if (lane == 0) node = root;
+                    } else if (lane < nc[0] * nc[1] * nc[2]) {
+                        const int ix = lane % nc[0], iy = (lane / nc[0]) % nc[1], iz = lane / (nc[0] * nc[1]);
+                        const uint32_t cell = (spread5((uint32_t)(c0[0] + ix)) << 2) | (spread5((uint32_t)(c0[1] + iy)) << 1) |
+                                              spread5((uint32_t)(c0[2] + iz));
+                        node = __ldg(etab + entry_offset(lvl) + (int)cell);
+                    }
+                    const uint32_t eb = __ballot_sync(FULL, node >= 0);
+                    if (node >= 0) sm.wl[__popc(eb & lt_mask)] = (uint32_t)node;
+                    wsz = __popc(eb);
+                }
                 __syncwarp();
-                int wsz = 1, lqn = 0;                  // work list and leaf queue fill
-                int gt = 0, gmax = 0, gfirst_l = 0, gm_l = 0;   // gather in progress: iteration, bound, my leaf
-                int tapp = 0, tproc = 0;               // candidates appended to / consumed from the tile (this image)
-                int self_lo = 0x7FFFFFFF, self_hi = -1;   // span of appended candidates that are group members
+                int lqn = 0;                           // leaf queue fill
+                int gb = 0, gT = 0, git = 0;           // gather in progress: batch base in lq, particles, iteration
+                uint32_t selfq = 0;                    // quarters of the tile ring that hold members of the group itself
 
                 while (true) {
                     if (tcount >= 32) {
@@ -354,109 +426,110 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
 #pragma unroll 1
                         for (int h = 0; h < 2; ++h) {
                             if (__any_sync(FULL, (int)(po >> 2) - flushed >= 16)) flush_blocks();
-                            const int base = thead + 16 * h, a0 = tproc + 16 * h;
+                            const int base = thead + 16 * h;
+                            const uint32_t qbit = 1u << (base >> 4);
                             if (shifted)
                                 check16<true, false>(sm, base, nmx, nmy, nmz, ns0, ns1, ns2, r2, orig_i, ring_s, po);
-                            else if (a0 < self_hi && a0 + 16 > self_lo)
+                            else if (selfq & qbit)
                                 check16<false, true>(sm, base, nmx, nmy, nmz, ns0, ns1, ns2, r2, orig_i, ring_s, po);
                             else
                                 check16<false, false>(sm, base, nmx, nmy, nmz, ns0, ns1, ns2, r2, orig_i, ring_s, po);
+                            selfq &= ~qbit;
                         }
                         if (STATS) st_checks += 32ull * (unsigned)gcnt;
                         __syncwarp();
                         thead ^= 32;
                         tcount -= 32;
-                        tproc += 32;
                         continue;
                     }
-                    if (gt < gmax) {
-                        // ---- gather: particle gt of every lane's leaf; keep those within reach of the group box ----
-                        const bool valid = gt < gm_l;
+                    if (git * 32 < gT) {
+                        // ---- gather: particles [32 git, 32 git + 32) of the batch of leaves, flattened; keep those
+                        //      within reach of the group box (point-box form of eq. 2) ----
+                        const int j = git * 32 + lane;
+                        int l = 0;
+#pragma unroll
+                        for (int stp = 16; stp >= 1; stp >>= 1)
+                            if (sm.pre[l + stp] <= j) l += stp;
                         float4 pj = make_float4(0.f, 0.f, 0.f, 0.f);
                         bool keep = false;
-                        if (valid) {
-                            pj = __ldg(sorted_pos + gfirst_l + gt);
+                        int cidx = 0;
+                        if (j < gT) {
+                            cidx = (int)sm.lq[gb + l].x + (j - sm.pre[l]);
+                            pj = __ldg(sorted_pos + cidx);
                             const float e0 = fmaxf(fmaxf(__fsub_rn(blo[0], pj.x), __fsub_rn(pj.x, bhi[0])), 0.0f);
                             const float e1 = fmaxf(fmaxf(__fsub_rn(blo[1], pj.y), __fsub_rn(pj.y, bhi[1])), 0.0f);
                             const float e2 = fmaxf(fmaxf(__fsub_rn(blo[2], pj.z), __fsub_rn(pj.z, bhi[2])), 0.0f);
                             keep = __fmaf_rn(e2, e2, __fmaf_rn(e1, e1, __fmul_rn(e0, e0))) <= R2;
                         }
                         const uint32_t kb = __ballot_sync(FULL, keep);
+                        const int slot = (thead + tcount + __popc(kb & lt_mask)) & (GW_TILE - 1);
                         if (keep) {
-                            const int slot = (thead + tcount + __popc(kb & lt_mask)) & (GW_TILE - 1);
                             sm.tx[slot] = pj.x;
                             sm.ty[slot] = pj.y;
                             sm.tz[slot] = pj.z;
                             sm.ti[slot] = __float_as_int(pj.w);
                         }
-                        if (own_tree) {
-                            const int jj = gfirst_l + gt - gfirst;
-                            const uint32_t sb = __ballot_sync(FULL, keep && jj >= 0 && jj < gcnt);
-                            if (sb) {
-                                const int lo_lane = __ffs(sb) - 1, hi_lane = 31 - __clz(sb);
-                                self_lo = min(self_lo, tapp + __popc(kb & ((1u << lo_lane) - 1u)));
-                                self_hi = max(self_hi, tapp + __popc(kb & ((2u << hi_lane) - 1u)));
-                            }
-                        }
+                        if (own_tree)
+                            selfq |= __reduce_or_sync(FULL, (keep && (unsigned)(cidx - gfirst) < (unsigned)gcnt) ? (1u << (slot >> 4)) : 0u);
                         const int nk = __popc(kb);
                         tcount += nk;
-                        tapp += nk;
                         if (STATS) st_cand += nk;
-                        ++gt;
+                        ++git;
                         __syncwarp();
                         continue;
                     }
                     if (lqn >= 32 || (wsz == 0 && lqn > 0)) {
-                        // ---- start a gather: the newest (up to) 32 queued leaves, one per lane ----
+                        // ---- start a gather: the newest (up to) 32 queued leaves; exclusive scan of their counts ----
                         const int ng = min(lqn, 32);
                         lqn -= ng;
-                        gm_l = 0;
-                        if (lane < ng) {
-                            const uint2 q = sm.lq[lqn + lane];
-                            gfirst_l = (int)q.x;
-                            gm_l = (int)q.y;
+                        gb = lqn;
+                        int incl = (lane < ng) ? (int)sm.lq[gb + lane].y : 0;
+#pragma unroll
+                        for (int o = 1; o < 32; o <<= 1) {
+                            const int v = __shfl_up_sync(FULL, incl, o);
+                            if (lane >= o) incl += v;
                         }
-                        gmax = __reduce_max_sync(FULL, gm_l);
-                        gt = 0;
+                        sm.pre[lane + 1] = incl;
+                        if (lane == 0) sm.pre[0] = 0;
+                        gT = __shfl_sync(FULL, incl, 31);
+                        git = 0;
                         __syncwarp();
                         continue;
                     }
                     if (wsz > 0) {
-                        // ---- lines 10-19, 32 nodes per step ----
-                        const int npop = (wsz > GW_WL - 128) ? 1 : min(wsz, 32);
-                        const bool active = lane < npop;
-                        bool push_sib = false, push_child = false, emit = false;
-                        int4 nd = make_int4(0, 0, 0, 0);
-                        if (active) {
+                        // ---- lines 10-19, up to 64 nodes per step: every lane pops one entry and tests that node
+                        //      and, for a left child, its rope (= right sibling) as well ----
+                        const int npop = (wsz > GW_WL - 96) ? 1 : min(wsz, 32);
+                        int pushA = 0, pushB = 0, emitA = 0, emitB = 0, pairf = 0;
+                        int4 A = make_int4(0, 0, 0, 0), B = make_int4(0, 0, 0, 0);
+                        if (lane < npop) {
                             const uint32_t ent = sm.wl[wsz - 1 - lane];
-                            nd = __ldg(nodes + (ent & 0x7FFFFFFFu));
-                            float a[3], b[3];
-                            decompress((uint32_t)nd.x, (uint32_t)nd.y, flo, fdl, a, b);
-                            const float t0 = fmaxf(fmaxf(__fsub_rn(a[0], bhi[0]), __fsub_rn(blo[0], b[0])), 0.0f);
-                            const float t1 = fmaxf(fmaxf(__fsub_rn(a[1], bhi[1]), __fsub_rn(blo[1], b[1])), 0.0f);
-                            const float t2 = fmaxf(fmaxf(__fsub_rn(a[2], bhi[2]), __fsub_rn(blo[2], b[2])), 0.0f);
-                            const float d2 = __fmaf_rn(t2, t2, __fmaf_rn(t1, t1, __fmul_rn(t0, t0)));
-                            const bool hit = d2 <= R2;
-                            push_sib = (ent >> 31) != 0;          // a left child: its rope is the right sibling
-                            push_child = hit && nd.z >= 0;
-                            emit = hit && nd.z < 0;
+                            A = __ldg(nodes + (ent & 0x7FFFFFFFu));
+                            const bool hitA = node_overlaps(A, flo, fdl, blo, bhi, R2);
+                            pushA = hitA && A.z >= 0;
+                            emitA = hitA && A.z < 0;
+                            if (ent >> 31) {
+                                pairf = 1;
+                                B = __ldg(nodes + A.w);
+                                const bool hitB = node_overlaps(B, flo, fdl, blo, bhi, R2);
+                                pushB = hitB && B.z >= 0;
+                                emitB = hitB && B.z < 0;
+                            }
                         }
                         __syncwarp();                             // all reads of the list done before it is rewritten
-                        const uint32_t b1 = __ballot_sync(FULL, push_sib);
-                        const uint32_t b2 = __ballot_sync(FULL, push_child);
-                        const uint32_t b3 = __ballot_sync(FULL, emit);
+                        const uint32_t pa = __ballot_sync(FULL, pushA), pb = __ballot_sync(FULL, pushB);
+                        const uint32_t ea = __ballot_sync(FULL, emitA), eb = __ballot_sync(FULL, emitB);
                         const int base = wsz - npop;
-                        if (push_sib) sm.wl[base + __popc(b1 & lt_mask)] = (uint32_t)nd.w;
-                        if (push_child) sm.wl[base + __popc(b1) + __popc(b2 & lt_mask)] = (uint32_t)nd.z | 0x80000000u;
-                        wsz = base + __popc(b1) + __popc(b2);
-                        if (emit) {
-                            const uint32_t m = (P.K > 1) ? 1u + (((uint32_t)nd.x >> 30) | (((uint32_t)nd.y >> 30) << 2)) : 1u;
-                            sm.lq[lqn + __popc(b3 & lt_mask)] = make_uint2((uint32_t)(~nd.z), m);
-                        }
-                        lqn += __popc(b3);
+                        if (pushA) sm.wl[base + __popc(pa & lt_mask)] = (uint32_t)A.z | 0x80000000u;
+                        if (pushB) sm.wl[base + __popc(pa) + __popc(pb & lt_mask)] = (uint32_t)B.z | 0x80000000u;
+                        wsz = base + __popc(pa) + __popc(pb);
+                        if (emitA) sm.lq[lqn + __popc(ea & lt_mask)] = make_uint2((uint32_t)(~A.z), (uint32_t)leaf_count(A, P.N, seg_end));
+                        if (emitB)
+                            sm.lq[lqn + __popc(ea) + __popc(eb & lt_mask)] = make_uint2((uint32_t)(~B.z), (uint32_t)leaf_count(B, P.N, seg_end));
+                        lqn += __popc(ea) + __popc(eb);
                         if (STATS) {
-                            st_tests += npop;
-                            st_leaf += __popc(b3);
+                            st_tests += npop + __popc(__ballot_sync(FULL, pairf));
+                            st_leaf += __popc(ea) + __popc(eb);
                             ++st_steps;
                         }
                         __syncwarp();
@@ -546,10 +619,10 @@ cudaError_t launch_traverse(const TraverseParams &p, const BuildBuffers &b, int3
         cudaError_t e = cudaMemsetAsync(&b.meta->group_cursor, 0, 2 * sizeof(int32_t), st);
         if (e != cudaSuccess) return e;
         const int gb = min(group_grid_blocks(true), (p.N + GW_WARPS - 1) / GW_WARPS);
-        traverse_group_kernel<true><<<gb, GW_WARPS * 32, 0, st>>>(p, b.nodes, b.sorted_pos, b.groups, b.meta, nlist, n_neigh);
+        traverse_group_kernel<true><<<gb, GW_WARPS * 32, 0, st>>>(p, b.nodes, b.sorted_pos, b.groups, b.entry, b.meta, nlist, n_neigh);
     } else {
         const int gb = min(group_grid_blocks(false), (p.N + GW_WARPS - 1) / GW_WARPS);
-        traverse_group_kernel<false><<<gb, GW_WARPS * 32, 0, st>>>(p, b.nodes, b.sorted_pos, b.groups, b.meta, nlist, n_neigh);
+        traverse_group_kernel<false><<<gb, GW_WARPS * 32, 0, st>>>(p, b.nodes, b.sorted_pos, b.groups, b.entry, b.meta, nlist, n_neigh);
     }
     return cudaGetLastError();
 }

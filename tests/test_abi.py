@@ -43,7 +43,7 @@ def test_host_side_validation_without_gpu(lib):
     with pytest.raises(qbvh.QbvhError):
         qbvh.qbvh_set_num_types(5)
     with pytest.raises(qbvh.QbvhError):
-        qbvh.qbvh_set_option(qbvh.OPT_LEAF_COLLAPSE, 16)
+        qbvh.qbvh_set_option(qbvh.OPT_LEAF_COLLAPSE, 33)
     with pytest.raises(qbvh.QbvhError):
         qbvh.qbvh_set_option(99, 0)
     qbvh.qbvh_set_option(qbvh.OPT_LEAF_COLLAPSE, 4)
