@@ -287,7 +287,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number 1..5 (default 2: 1M LJ)")
     ap.add_argument("--impl", default="qbvh", choices=["qbvh", "reference"])
-    ap.add_argument("--leaf-collapse", type=int, default=4)
+    ap.add_argument("--leaf-collapse", type=int, default=32)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg (profiling runs)")
     args = ap.parse_args()

@@ -61,7 +61,7 @@ int qbvh_set_workspace(void *dev_ptr, int64_t bytes);
 /* Options (all take effect at the next qbvh_build unless noted). */
 #define QBVH_OPT_LEAF_COLLAPSE 1 /* k in [1,32]: the traversal stops at nodes covering <= k consecutive Z-order
                                     particles and distance-checks that range directly ("subtree
-                                    collapse").  k = 1 is exactly the paper's one-particle-per-leaf tree. Default 8. */
+                                    collapse").  k = 1 is exactly the paper's one-particle-per-leaf tree. Default 32. */
 #define QBVH_OPT_STATS 2         /* 0/1: qbvh_neighbors runs the instrumented traversal and fills qbvh_get_stats
                                     (takes effect immediately; slower — never use when timing). Default 0.        */
 #define QBVH_OPT_VARIANT 3       /* which traversal kernel qbvh_neighbors launches: 0 = Algorithm 1 as written, one

@@ -16,7 +16,7 @@ struct Context {
     void *staging = nullptr;
     int64_t staging_bytes = 0;
     int T = 1;
-    int K = 8;          // leaf-collapse option for the next build
+    int K = 32;         // leaf-collapse option for the next build
     int K_built = 1;
     bool stats = false;
     int variant = 1;

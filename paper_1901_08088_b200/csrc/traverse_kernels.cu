@@ -192,6 +192,7 @@ constexpr int GW_WL = 512;       // work-list entries per warp
 constexpr int GW_LQ = 96;        // leaf-queue entries per warp
 constexpr int GW_TILE = 64;      // candidate tile ring per warp: two halves of 32
 constexpr int GW_RING = 32;      // staged neighbors per lane: two blocks of 16
+constexpr int GW_FLAT_K = 4;     // collapse thresholds up to here use the flattening gather, larger ones fixed slots
 
 struct __align__(128) GwShared {
     float tx[GW_TILE], ty[GW_TILE], tz[GW_TILE];   // candidate tile, structure of arrays
@@ -278,7 +279,9 @@ __device__ __forceinline__ bool node_overlaps(const int4 nd, const float flo[3],
     return __fmaf_rn(t2, t2, __fmaf_rn(t1, t1, __fmul_rn(t0, t0))) <= R2;
 }
 
-template <bool STATS>
+// WS > 0: collapsed leaves are gathered in fixed slots of WS lanes each (WS >= K, 32 / WS leaves per step) instead of
+// being flattened into dense batches by a prefix scan + binary search (WS = 0, kept for small K).
+template <bool STATS, int WS>
 __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseParams P, const int4 *__restrict__ nodes,
                                                                         const float4 *__restrict__ sorted_pos,
                                                                         const uint2 *__restrict__ groups,
@@ -442,7 +445,49 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
                         tcount -= 32;
                         continue;
                     }
-                    if (git * 32 < gT) {
+                    if (WS && lqn > 0) {
+                        // ---- gather 32 / WS leaves: lane j takes particle j % WS of leaf j / WS (a collapsed leaf has
+                        //      at most K <= WS particles); keep those within reach of the group box (point-box form
+                        //      of eq. 2) ----
+                        constexpr int NL = WS ? 32 / WS : 1;
+                        const int li = WS ? lane / WS : 0, sub = WS ? lane % WS : 0;
+                        const int take = min(lqn, NL);
+                        uint2 lf = make_uint2(0u, 0u);
+                        if (li < take) lf = sm.lq[lqn - 1 - li];
+                        lqn -= take;
+                        float4 pj = make_float4(0.f, 0.f, 0.f, 0.f);
+                        bool keep = false;
+                        const int cidx = (int)lf.x + sub;
+                        if (sub < (int)lf.y) {
+                            pj = __ldg(sorted_pos + cidx);
+                            const float e0 = fmaxf(fmaxf(__fsub_rn(blo[0], pj.x), __fsub_rn(pj.x, bhi[0])), 0.0f);
+                            const float e1 = fmaxf(fmaxf(__fsub_rn(blo[1], pj.y), __fsub_rn(pj.y, bhi[1])), 0.0f);
+                            const float e2 = fmaxf(fmaxf(__fsub_rn(blo[2], pj.z), __fsub_rn(pj.z, bhi[2])), 0.0f);
+                            keep = __fmaf_rn(e2, e2, __fmaf_rn(e1, e1, __fmul_rn(e0, e0))) <= R2;
+                        }
+                        const uint32_t kb = __ballot_sync(FULL, keep);
+                        const int slot = (thead + tcount + __popc(kb & lt_mask)) & (GW_TILE - 1);
+                        if (keep) {
+                            sm.tx[slot] = pj.x;
+                            sm.ty[slot] = pj.y;
+                            sm.tz[slot] = pj.z;
+                            sm.ti[slot] = __float_as_int(pj.w);
+                        }
+                        const int nk = __popc(kb);
+                        if (own_tree && nk) {
+                            // members of the group itself among the kept: mark every quarter of the ring just written
+                            if (__any_sync(FULL, keep && (unsigned)(cidx - gfirst) < (unsigned)gcnt)) {
+                                const int s0q = ((thead + tcount) & (GW_TILE - 1)) >> 4;
+                                const int s1q = ((thead + tcount + nk - 1) & (GW_TILE - 1)) >> 4;
+                                selfq |= (1u << s0q) | (1u << s1q) | (1u << ((s0q + 1) & 3));
+                            }
+                        }
+                        tcount += nk;
+                        if (STATS) st_cand += nk;
+                        __syncwarp();
+                        continue;
+                    }
+                    if (!WS && git * 32 < gT) {
                         // ---- gather: particles [32 git, 32 git + 32) of the batch of leaves, flattened; keep those
                         //      within reach of the group box (point-box form of eq. 2) ----
                         const int j = git * 32 + lane;
@@ -478,7 +523,7 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
                         __syncwarp();
                         continue;
                     }
-                    if (lqn >= 32 || (wsz == 0 && lqn > 0)) {
+                    if (!WS && (lqn >= 32 || (wsz == 0 && lqn > 0))) {
                         // ---- start a gather: the newest (up to) 32 queued leaves; exclusive scan of their counts ----
                         const int ng = min(lqn, 32);
                         lqn -= ng;
@@ -584,20 +629,23 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
 }
 
 // persistent grid of the group kernel: as many blocks as fit on the device at once
-static int group_grid_blocks(bool stats) {
-    static int cached[2] = {0, 0};
-    int &c = cached[stats ? 1 : 0];
+template <bool STATS, int WS>
+static int group_grid_blocks() {
+    static int c = 0;
     if (c == 0) {
         int dev = 0, sms = 148, per_sm = 1;
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        if (stats)
-            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, traverse_group_kernel<true>, GW_WARPS * 32, 0);
-        else
-            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, traverse_group_kernel<false>, GW_WARPS * 32, 0);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, traverse_group_kernel<STATS, WS>, GW_WARPS * 32, 0);
         c = sms * (per_sm > 0 ? per_sm : 1);
     }
     return c;
+}
+
+template <bool STATS, int WS>
+static void launch_group(const TraverseParams &p, const BuildBuffers &b, int32_t *nlist, int32_t *n_neigh, cudaStream_t st) {
+    const int gb = min(group_grid_blocks<STATS, WS>(), (p.N + GW_WARPS - 1) / GW_WARPS);
+    traverse_group_kernel<STATS, WS><<<gb, GW_WARPS * 32, 0, st>>>(p, b.nodes, b.sorted_pos, b.groups, b.entry, b.meta, nlist, n_neigh);
 }
 
 cudaError_t launch_traverse(const TraverseParams &p, const BuildBuffers &b, int32_t *nlist, int32_t *n_neigh,
@@ -613,16 +661,21 @@ cudaError_t launch_traverse(const TraverseParams &p, const BuildBuffers &b, int3
             traverse_kernel<false><<<blocks, threads, 0, st>>>(p, b.nodes, b.sorted_pos, b.meta, nlist, n_neigh);
         return cudaGetLastError();
     }
+    const int ws = p.K > 16 ? 32 : (p.K > 8 ? 16 : (p.K > GW_FLAT_K ? 8 : 0));
     if (stats) {
         // census of the paper's per-particle walk (stats[0..4]), then the instrumented production kernel
         traverse_kernel<true><<<blocks, threads, 0, st>>>(p, b.nodes, b.sorted_pos, b.meta, nlist, n_neigh);
         cudaError_t e = cudaMemsetAsync(&b.meta->group_cursor, 0, 2 * sizeof(int32_t), st);
         if (e != cudaSuccess) return e;
-        const int gb = min(group_grid_blocks(true), (p.N + GW_WARPS - 1) / GW_WARPS);
-        traverse_group_kernel<true><<<gb, GW_WARPS * 32, 0, st>>>(p, b.nodes, b.sorted_pos, b.groups, b.entry, b.meta, nlist, n_neigh);
+        if (ws == 32) launch_group<true, 32>(p, b, nlist, n_neigh, st);
+        else if (ws == 16) launch_group<true, 16>(p, b, nlist, n_neigh, st);
+        else if (ws == 8) launch_group<true, 8>(p, b, nlist, n_neigh, st);
+        else launch_group<true, 0>(p, b, nlist, n_neigh, st);
     } else {
-        const int gb = min(group_grid_blocks(false), (p.N + GW_WARPS - 1) / GW_WARPS);
-        traverse_group_kernel<false><<<gb, GW_WARPS * 32, 0, st>>>(p, b.nodes, b.sorted_pos, b.groups, b.entry, b.meta, nlist, n_neigh);
+        if (ws == 32) launch_group<false, 32>(p, b, nlist, n_neigh, st);
+        else if (ws == 16) launch_group<false, 16>(p, b, nlist, n_neigh, st);
+        else if (ws == 8) launch_group<false, 8>(p, b, nlist, n_neigh, st);
+        else launch_group<false, 0>(p, b, nlist, n_neigh, st);
     }
     return cudaGetLastError();
 }

@@ -89,7 +89,7 @@ def test_sort_degenerate_orders(case):
         assert np.array_equal(out["perm"], np.arange(N))   # stability: equal keys keep input order
 
 
-@pytest.mark.parametrize("K", [1, 4, 8, 32])
+@pytest.mark.parametrize("K", [1, 4, 8, 16, 32])
 @pytest.mark.parametrize("cid", [1, 2, 3, 4, 5])
 def test_neighbors_parity_small(cid, K):
     w = W.make_config(cid, small=True)
@@ -102,7 +102,7 @@ def test_neighbors_parity_small(cid, K):
 def test_neighbors_parity_full_size(cid):
     """BASELINE.json's full sizes, in the launch configuration bench.py times (default options)."""
     w = W.make_config(cid)
-    out = gpu_run(w, K=8)
+    out = gpu_run(w, K=32)
     rep = compare_with_oracle(w, out, ON.neighbor_list(w.pos, w.type, w.box, w.r_list, method="cell"))
     assert rep["rows_checked"] == w.N and rep["pairs"] > 0
 
