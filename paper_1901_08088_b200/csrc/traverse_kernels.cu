@@ -187,36 +187,42 @@ __device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c) {
     return r;
 }
 
-constexpr int GW_WARPS = 4;      // warps per block
-constexpr int GW_WL = 512;       // work-list entries per warp
+#ifndef QBVH_GW_WARPS
+#define QBVH_GW_WARPS 4
+#endif
+#ifndef QBVH_GW_RING
+#define QBVH_GW_RING 32
+#endif
+constexpr int GW_WARPS = QBVH_GW_WARPS;   // warps per block
+constexpr int GW_WL = 256;       // work-list entries per warp
 constexpr int GW_LQ = 96;        // leaf-queue entries per warp
-constexpr int GW_TILE = 64;      // candidate tile ring per warp: two halves of 32
-constexpr int GW_RING = 32;      // staged neighbors per lane: two blocks of 16
-constexpr int GW_FLAT_K = 4;     // collapse thresholds up to here use the flattening gather, larger ones fixed slots
+constexpr int GW_TILE = 128;     // candidate tile ring per warp: four tiles of 32
+constexpr int GW_RING = QBVH_GW_RING;     // staged neighbors per lane: blocks of 16
+constexpr int GW_RING_BYTES = 4 * GW_RING;
 
-struct __align__(128) GwShared {
-    float tx[GW_TILE], ty[GW_TILE], tz[GW_TILE];   // candidate tile, structure of arrays
+struct __align__(256) GwShared {
+    int32_t ring[32][GW_RING];                     // per-lane staged neighbors (256 bytes per lane)
+    float tx[GW_TILE], ty[GW_TILE], tz[GW_TILE];   // candidate tile ring, structure of arrays
     int32_t ti[GW_TILE];                           // original particle index of each candidate
-    int32_t ring[32][GW_RING];                     // per-lane staged neighbors
     uint32_t wl[GW_WL];                            // work list: node id | (also test its rope sibling) << 31
     uint2 lq[GW_LQ];                               // leaf queue: {first sorted position, count}
-    int32_t pre[36];                               // exclusive prefix sums of the counts of the leaves being gathered
 };
 
-// append one neighbor to this lane's ring: slot address = ring base | (byte offset mod 128), one LOP3
+// append one neighbor to this lane's ring: slot address = ring base | (byte offset mod 256), one LOP3
 __device__ __forceinline__ void ring_put(uint32_t ring_s, uint32_t &po, int32_t v) {
-    *static_cast<int32_t *>(__cvta_shared_to_generic((size_t)(ring_s | (po & (4 * GW_RING - 4))))) = v;
+    *static_cast<int32_t *>(__cvta_shared_to_generic((size_t)(ring_s | (po & (GW_RING_BYTES - 4))))) = v;
     po += 4;
 }
 
-// 16 candidates of the tile, starting at `base`, against this lane's particle: the canonical predicate
+// One tile of 32 candidates, starting at slot `base` of the tile ring, against this lane's particle: the
+// canonical predicate
 //   D = (p_j - p_i) [- s L];  d2 = fma(Dz, Dz, fma(Dy, Dy, Dx*Dx));  d2 <= r^2
-// evaluated for two candidates per instruction.  SELF: the tile may hold members of the group itself.
-template <bool SHIFTED, bool SELF>
-__device__ __forceinline__ void check16(const GwShared &sm, int base, u64 nmx, u64 nmy, u64 nmz, u64 ns0, u64 ns1,
+// evaluated for two candidates per instruction.  SELF: the tile holds the members of the group itself.
+template <bool SHIFTED, bool SELF, int NC>
+__device__ __forceinline__ void check_tile(const GwShared &sm, int base, u64 nmx, u64 nmy, u64 nmz, u64 ns0, u64 ns1,
                                         u64 ns2, float r2, int orig_i, uint32_t ring_s, uint32_t &po) {
 #pragma unroll
-    for (int j = 0; j < 4; ++j) {
+    for (int j = 0; j < NC / 4; ++j) {
         const float4 X = *reinterpret_cast<const float4 *>(&sm.tx[base + 4 * j]);
         const float4 Y = *reinterpret_cast<const float4 *>(&sm.ty[base + 4 * j]);
         const float4 Z = *reinterpret_cast<const float4 *>(&sm.tz[base + 4 * j]);
@@ -279,8 +285,16 @@ __device__ __forceinline__ bool node_overlaps(const int4 nd, const float flo[3],
     return __fmaf_rn(t2, t2, __fmaf_rn(t1, t1, __fmul_rn(t0, t0))) <= R2;
 }
 
-// WS > 0: collapsed leaves are gathered in fixed slots of WS lanes each (WS >= K, 32 / WS leaves per step) instead of
-// being flattened into dense batches by a prefix scan + binary search (WS = 0, kept for small K).
+// point-box form of eq. 2: is the candidate within the padded radius of the group's box
+__device__ __forceinline__ bool point_in_reach(const float4 p, const float blo[3], const float bhi[3], float R2) {
+    const float e0 = fmaxf(fmaxf(__fsub_rn(blo[0], p.x), __fsub_rn(p.x, bhi[0])), 0.0f);
+    const float e1 = fmaxf(fmaxf(__fsub_rn(blo[1], p.y), __fsub_rn(p.y, bhi[1])), 0.0f);
+    const float e2 = fmaxf(fmaxf(__fsub_rn(blo[2], p.z), __fsub_rn(p.z, bhi[2])), 0.0f);
+    return __fmaf_rn(e2, e2, __fmaf_rn(e1, e1, __fmul_rn(e0, e0))) <= R2;
+}
+
+// WS: collapsed leaves are gathered in fixed slots of WS lanes each (WS >= K, 32 / WS leaves per batch, two batches
+// per step so that two 16-byte position loads per lane are in flight).
 template <bool STATS, int WS>
 __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseParams P, const int4 *__restrict__ nodes,
                                                                         const float4 *__restrict__ sorted_pos,
@@ -294,11 +308,16 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
     const uint32_t FULL = 0xFFFFFFFFu;
     const uint32_t lt_mask = (1u << lane) - 1u;
     GwShared &sm = s_all[warp];
-    int32_t *const myring = static_cast<int32_t *>(__builtin_assume_aligned(sm.ring[lane], 128));
-    const uint32_t ring_s = (uint32_t)__cvta_generic_to_shared(myring);   // 128-byte aligned
+    int32_t *const myring = static_cast<int32_t *>(__builtin_assume_aligned(sm.ring[lane], 256));
+    const uint32_t ring_s = (uint32_t)__cvta_generic_to_shared(myring);   // 256-byte aligned
+    // every lane's ring starts at another quad, so that lanes filling at the same pace hit different banks
+    const uint32_t rot = (uint32_t)(lane & 7) << 4;
     const int ngroups = meta->group_count;
     const bool vec_ok = ((P.max_neigh & 3) == 0) && ((reinterpret_cast<uintptr_t>(nlist) & 15) == 0);
     const int cap = P.max_neigh;
+    constexpr int NL = 32 / WS;                 // leaves per gather batch
+    constexpr int CHUNK = GW_RING >= 64 ? 32 : 16;   // candidates checked between two looks at the ring fill
+    const int li = lane / WS, sub = lane % WS;
     unsigned long long st_tests = 0, st_leaf = 0, st_cand = 0, st_checks = 0, st_steps = 0, st_groups = 0;
     int wmax = 0;
 
@@ -327,19 +346,24 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
         }
         int32_t *const row = nlist + (size_t)(live ? orig_i : 0) * (size_t)cap;
         const u64 nmx = pk2(-me.x, -me.x), nmy = pk2(-me.y, -me.y), nmz = pk2(-me.z, -me.z);
-        uint32_t po = 0;                 // 4 x neighbors found so far for this lane's particle (ring byte offset)
-        int flushed = 0;                 // neighbors already written to the list row
-        int thead = 0, tcount = 0;       // candidate tile ring: first slot (0 or 32), number of candidates
+        uint32_t po = rot;               // ring byte offset: rot + 4 x neighbors found so far for this lane's particle
+        int flushed = 0;                 // neighbors already written to the list row (a multiple of 16)
+        int thead = 0, tcount = 0;       // candidate tile ring: first slot (a multiple of 32), number of candidates
         if (STATS) ++st_groups;
 
-        // lanes holding a complete 64-byte block of staged neighbors write it to their list row
+        // lanes write their complete 64-byte blocks of staged neighbors to their list rows
         auto flush_blocks = [&]() {
-            if ((int)(po >> 2) - flushed >= 16) {
-                const int32_t *src = myring + (flushed & (GW_RING - 1));
+            while (__any_sync(FULL, (int)((po - rot) >> 2) - flushed >= 16)) {
+                if ((int)((po - rot) >> 2) - flushed >= 16) {
+                    const uint32_t off = rot + 4u * (uint32_t)flushed;
 #pragma unroll
-                for (int j = 0; j < 4; ++j)
-                    store4(row, flushed + 4 * j, cap, vec_ok, *reinterpret_cast<const int4 *>(src + 4 * j));
-                flushed += 16;
+                    for (int j = 0; j < 4; ++j) {
+                        const int4 v = *static_cast<const int4 *>(
+                            __cvta_shared_to_generic((size_t)(ring_s | ((off + 16u * j) & (GW_RING_BYTES - 16)))));
+                        store4(row, flushed + 4 * j, cap, vec_ok, v);
+                    }
+                    flushed += 16;
+                }
             }
         };
 
@@ -379,7 +403,25 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
                 const float blo[3] = {__fadd_rn(glo[0], s0), __fadd_rn(glo[1], s1), __fadd_rn(glo[2], s2)};
                 const float bhi[3] = {__fadd_rn(ghi[0], s0), __fadd_rn(ghi[1], s1), __fadd_rn(ghi[2], s2)};
                 const u64 ns0 = pk2(-s0, -s0), ns1 = pk2(-s1, -s1), ns2 = pk2(-s2, -s2);
-                const bool own_tree = (tb == ta) && !shifted;   // only then can a candidate be a group member
+                // the group's own particles are found by the walk only here: in its own tree, unshifted.  They are
+                // checked first, as one tile (self excluded by index), and their leaves are skipped below.
+                const bool own_tree = (tb == ta) && !shifted;
+                if (own_tree) {
+                    sm.tx[lane] = live ? me.x : __int_as_float(0x7FC00000);   // NaN: never accepted
+                    sm.ty[lane] = me.y;
+                    sm.tz[lane] = me.z;
+                    sm.ti[lane] = orig_i;
+                    __syncwarp();
+#pragma unroll 1
+                    for (int h = 0; h < 32 / CHUNK; ++h) {
+                        check_tile<false, true, CHUNK>(sm, CHUNK * h, nmx, nmy, nmz, ns0, ns1, ns2, r2, orig_i, ring_s, po);
+                        if (__any_sync(FULL, (int)((po - rot) >> 2) - flushed >= GW_RING - CHUNK)) flush_blocks();
+                    }
+                    if (STATS) st_checks += (unsigned long long)gcnt * (unsigned)gcnt;
+                    __syncwarp();
+                    thead = 0;
+                    tcount = 0;
+                }
 
                 // ---- line 9, "n <- root node": enter at the finest Morton grid whose cells touched by the search
                 //      volume number at most 32 (one per lane); the root itself if even the 4^3 grid has more ----
@@ -420,128 +462,26 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
                 }
                 __syncwarp();
                 int lqn = 0;                           // leaf queue fill
-                int gb = 0, gT = 0, git = 0;           // gather in progress: batch base in lq, particles, iteration
-                uint32_t selfq = 0;                    // quarters of the tile ring that hold members of the group itself
 
                 while (true) {
                     if (tcount >= 32) {
-                        // ---- line 14 for every member: one tile of 32 candidates, as two halves of 16 ----
+                        // ---- line 14 for every member: one tile of 32 candidates ----
 #pragma unroll 1
-                        for (int h = 0; h < 2; ++h) {
-                            if (__any_sync(FULL, (int)(po >> 2) - flushed >= 16)) flush_blocks();
-                            const int base = thead + 16 * h;
-                            const uint32_t qbit = 1u << (base >> 4);
+                        for (int h = 0; h < 32 / CHUNK; ++h) {
                             if (shifted)
-                                check16<true, false>(sm, base, nmx, nmy, nmz, ns0, ns1, ns2, r2, orig_i, ring_s, po);
-                            else if (selfq & qbit)
-                                check16<false, true>(sm, base, nmx, nmy, nmz, ns0, ns1, ns2, r2, orig_i, ring_s, po);
+                                check_tile<true, false, CHUNK>(sm, thead + CHUNK * h, nmx, nmy, nmz, ns0, ns1, ns2, r2, orig_i, ring_s, po);
                             else
-                                check16<false, false>(sm, base, nmx, nmy, nmz, ns0, ns1, ns2, r2, orig_i, ring_s, po);
-                            selfq &= ~qbit;
+                                check_tile<false, false, CHUNK>(sm, thead + CHUNK * h, nmx, nmy, nmz, ns0, ns1, ns2, r2, orig_i, ring_s, po);
+                            // flush as soon as another chunk could overrun a ring
+                            if (__any_sync(FULL, (int)((po - rot) >> 2) - flushed >= GW_RING - CHUNK)) flush_blocks();
                         }
                         if (STATS) st_checks += 32ull * (unsigned)gcnt;
                         __syncwarp();
-                        thead ^= 32;
+                        thead = (thead + 32) & (GW_TILE - 1);
                         tcount -= 32;
                         continue;
                     }
-                    if (WS && lqn > 0) {
-                        // ---- gather 32 / WS leaves: lane j takes particle j % WS of leaf j / WS (a collapsed leaf has
-                        //      at most K <= WS particles); keep those within reach of the group box (point-box form
-                        //      of eq. 2) ----
-                        constexpr int NL = WS ? 32 / WS : 1;
-                        const int li = WS ? lane / WS : 0, sub = WS ? lane % WS : 0;
-                        const int take = min(lqn, NL);
-                        uint2 lf = make_uint2(0u, 0u);
-                        if (li < take) lf = sm.lq[lqn - 1 - li];
-                        lqn -= take;
-                        float4 pj = make_float4(0.f, 0.f, 0.f, 0.f);
-                        bool keep = false;
-                        const int cidx = (int)lf.x + sub;
-                        if (sub < (int)lf.y) {
-                            pj = __ldg(sorted_pos + cidx);
-                            const float e0 = fmaxf(fmaxf(__fsub_rn(blo[0], pj.x), __fsub_rn(pj.x, bhi[0])), 0.0f);
-                            const float e1 = fmaxf(fmaxf(__fsub_rn(blo[1], pj.y), __fsub_rn(pj.y, bhi[1])), 0.0f);
-                            const float e2 = fmaxf(fmaxf(__fsub_rn(blo[2], pj.z), __fsub_rn(pj.z, bhi[2])), 0.0f);
-                            keep = __fmaf_rn(e2, e2, __fmaf_rn(e1, e1, __fmul_rn(e0, e0))) <= R2;
-                        }
-                        const uint32_t kb = __ballot_sync(FULL, keep);
-                        const int slot = (thead + tcount + __popc(kb & lt_mask)) & (GW_TILE - 1);
-                        if (keep) {
-                            sm.tx[slot] = pj.x;
-                            sm.ty[slot] = pj.y;
-                            sm.tz[slot] = pj.z;
-                            sm.ti[slot] = __float_as_int(pj.w);
-                        }
-                        const int nk = __popc(kb);
-                        if (own_tree && nk) {
-                            // members of the group itself among the kept: mark every quarter of the ring just written
-                            if (__any_sync(FULL, keep && (unsigned)(cidx - gfirst) < (unsigned)gcnt)) {
-                                const int s0q = ((thead + tcount) & (GW_TILE - 1)) >> 4;
-                                const int s1q = ((thead + tcount + nk - 1) & (GW_TILE - 1)) >> 4;
-                                selfq |= (1u << s0q) | (1u << s1q) | (1u << ((s0q + 1) & 3));
-                            }
-                        }
-                        tcount += nk;
-                        if (STATS) st_cand += nk;
-                        __syncwarp();
-                        continue;
-                    }
-                    if (!WS && git * 32 < gT) {
-                        // ---- gather: particles [32 git, 32 git + 32) of the batch of leaves, flattened; keep those
-                        //      within reach of the group box (point-box form of eq. 2) ----
-                        const int j = git * 32 + lane;
-                        int l = 0;
-#pragma unroll
-                        for (int stp = 16; stp >= 1; stp >>= 1)
-                            if (sm.pre[l + stp] <= j) l += stp;
-                        float4 pj = make_float4(0.f, 0.f, 0.f, 0.f);
-                        bool keep = false;
-                        int cidx = 0;
-                        if (j < gT) {
-                            cidx = (int)sm.lq[gb + l].x + (j - sm.pre[l]);
-                            pj = __ldg(sorted_pos + cidx);
-                            const float e0 = fmaxf(fmaxf(__fsub_rn(blo[0], pj.x), __fsub_rn(pj.x, bhi[0])), 0.0f);
-                            const float e1 = fmaxf(fmaxf(__fsub_rn(blo[1], pj.y), __fsub_rn(pj.y, bhi[1])), 0.0f);
-                            const float e2 = fmaxf(fmaxf(__fsub_rn(blo[2], pj.z), __fsub_rn(pj.z, bhi[2])), 0.0f);
-                            keep = __fmaf_rn(e2, e2, __fmaf_rn(e1, e1, __fmul_rn(e0, e0))) <= R2;
-                        }
-                        const uint32_t kb = __ballot_sync(FULL, keep);
-                        const int slot = (thead + tcount + __popc(kb & lt_mask)) & (GW_TILE - 1);
-                        if (keep) {
-                            sm.tx[slot] = pj.x;
-                            sm.ty[slot] = pj.y;
-                            sm.tz[slot] = pj.z;
-                            sm.ti[slot] = __float_as_int(pj.w);
-                        }
-                        if (own_tree)
-                            selfq |= __reduce_or_sync(FULL, (keep && (unsigned)(cidx - gfirst) < (unsigned)gcnt) ? (1u << (slot >> 4)) : 0u);
-                        const int nk = __popc(kb);
-                        tcount += nk;
-                        if (STATS) st_cand += nk;
-                        ++git;
-                        __syncwarp();
-                        continue;
-                    }
-                    if (!WS && (lqn >= 32 || (wsz == 0 && lqn > 0))) {
-                        // ---- start a gather: the newest (up to) 32 queued leaves; exclusive scan of their counts ----
-                        const int ng = min(lqn, 32);
-                        lqn -= ng;
-                        gb = lqn;
-                        int incl = (lane < ng) ? (int)sm.lq[gb + lane].y : 0;
-#pragma unroll
-                        for (int o = 1; o < 32; o <<= 1) {
-                            const int v = __shfl_up_sync(FULL, incl, o);
-                            if (lane >= o) incl += v;
-                        }
-                        sm.pre[lane + 1] = incl;
-                        if (lane == 0) sm.pre[0] = 0;
-                        gT = __shfl_sync(FULL, incl, 31);
-                        git = 0;
-                        __syncwarp();
-                        continue;
-                    }
-                    if (wsz > 0) {
+                    if (wsz > 0 && lqn <= GW_LQ - 64) {
                         // ---- lines 10-19, up to 64 nodes per step: every lane pops one entry and tests that node
                         //      and, for a left child, its rope (= right sibling) as well ----
                         const int npop = (wsz > GW_WL - 96) ? 1 : min(wsz, 32);
@@ -550,15 +490,18 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
                         if (lane < npop) {
                             const uint32_t ent = sm.wl[wsz - 1 - lane];
                             A = __ldg(nodes + (ent & 0x7FFFFFFFu));
-                            const bool hitA = node_overlaps(A, flo, fdl, blo, bhi, R2);
-                            pushA = hitA && A.z >= 0;
-                            emitA = hitA && A.z < 0;
                             if (ent >> 31) {
                                 pairf = 1;
                                 B = __ldg(nodes + A.w);
+                            }
+                            const bool hitA = node_overlaps(A, flo, fdl, blo, bhi, R2);
+                            pushA = hitA && A.z >= 0;
+                            // leaves inside the group itself were handled above
+                            emitA = hitA && A.z < 0 && !(own_tree && (unsigned)(~A.z - gfirst) < (unsigned)gcnt);
+                            if (pairf) {
                                 const bool hitB = node_overlaps(B, flo, fdl, blo, bhi, R2);
                                 pushB = hitB && B.z >= 0;
-                                emitB = hitB && B.z < 0;
+                                emitB = hitB && B.z < 0 && !(own_tree && (unsigned)(~B.z - gfirst) < (unsigned)gcnt);
                             }
                         }
                         __syncwarp();                             // all reads of the list done before it is rewritten
@@ -580,6 +523,41 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
                         __syncwarp();
                         continue;
                     }
+                    if (lqn > 0) {
+                        // ---- gather up to 2 x 32/WS leaves: lane j takes particle j % WS of leaf j / WS of each batch (a
+                        //      collapsed leaf has at most K <= WS particles); keep those within reach of the group box ----
+                        const int take = min(lqn, 2 * NL);
+                        uint2 lfA = make_uint2(0u, 0u), lfB = make_uint2(0u, 0u);
+                        if (li < take) lfA = sm.lq[lqn - 1 - li];
+                        if (NL + li < take) lfB = sm.lq[lqn - 1 - NL - li];
+                        lqn -= take;
+                        float4 pA = make_float4(0.f, 0.f, 0.f, 0.f), pB = pA;
+                        const bool vA = sub < (int)lfA.y, vB = sub < (int)lfB.y;
+                        if (vA) pA = __ldg(sorted_pos + (int)lfA.x + sub);
+                        if (vB) pB = __ldg(sorted_pos + (int)lfB.x + sub);
+                        const bool keepA = vA && point_in_reach(pA, blo, bhi, R2);
+                        const bool keepB = vB && point_in_reach(pB, blo, bhi, R2);
+                        const uint32_t ka = __ballot_sync(FULL, keepA), kb = __ballot_sync(FULL, keepB);
+                        const int t0 = thead + tcount;
+                        if (keepA) {
+                            const int slot = (t0 + __popc(ka & lt_mask)) & (GW_TILE - 1);
+                            sm.tx[slot] = pA.x;
+                            sm.ty[slot] = pA.y;
+                            sm.tz[slot] = pA.z;
+                            sm.ti[slot] = __float_as_int(pA.w);
+                        }
+                        if (keepB) {
+                            const int slot = (t0 + __popc(ka) + __popc(kb & lt_mask)) & (GW_TILE - 1);
+                            sm.tx[slot] = pB.x;
+                            sm.ty[slot] = pB.y;
+                            sm.tz[slot] = pB.z;
+                            sm.ti[slot] = __float_as_int(pB.w);
+                        }
+                        tcount += __popc(ka) + __popc(kb);
+                        if (STATS) st_cand += __popc(ka) + __popc(kb);
+                        __syncwarp();
+                        continue;
+                    }
                     if (tcount > 0) {
                         // ---- the image's last, partial tile: pad with NaN (never accepted) and run it as a full one ----
                         if (lane >= tcount) sm.tx[(thead + lane) & (GW_TILE - 1)] = __int_as_float(0x7FC00000);
@@ -595,25 +573,27 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
         // ---- tail of every row, count, overflow word ----
         flush_blocks();
         {
-            const int rem = (int)(po >> 2) - flushed;
-            const int32_t *src = myring + (flushed & (GW_RING - 1));
+            const int cnt = (int)((po - rot) >> 2);
+            const int rem = cnt - flushed;
+            const uint32_t off = rot + 4u * (uint32_t)flushed;
 #pragma unroll
             for (int j = 0; j < 4; ++j)
                 if (4 * j < rem) {
-                    const int4 v = *reinterpret_cast<const int4 *>(src + 4 * j);
-                    const int off = flushed + 4 * j;
-                    if (vec_ok && off + 4 <= cap) {
-                        *reinterpret_cast<int4 *>(row + off) = v;    // up to 3 entries past the count: unspecified
+                    const int4 v = *static_cast<const int4 *>(
+                        __cvta_shared_to_generic((size_t)(ring_s | ((off + 16u * j) & (GW_RING_BYTES - 16)))));
+                    const int o = flushed + 4 * j;
+                    if (vec_ok && o + 4 <= cap) {
+                        *reinterpret_cast<int4 *>(row + o) = v;    // up to 3 entries past the count: unspecified
                     } else {
-                        if (4 * j + 0 < rem && off + 0 < cap) row[off + 0] = v.x;
-                        if (4 * j + 1 < rem && off + 1 < cap) row[off + 1] = v.y;
-                        if (4 * j + 2 < rem && off + 2 < cap) row[off + 2] = v.z;
-                        if (4 * j + 3 < rem && off + 3 < cap) row[off + 3] = v.w;
+                        if (4 * j + 0 < rem && o + 0 < cap) row[o + 0] = v.x;
+                        if (4 * j + 1 < rem && o + 1 < cap) row[o + 1] = v.y;
+                        if (4 * j + 2 < rem && o + 2 < cap) row[o + 2] = v.z;
+                        if (4 * j + 3 < rem && o + 3 < cap) row[o + 3] = v.w;
                     }
                 }
+            if (live) n_neigh[orig_i] = cnt;
+            wmax = max(wmax, live ? cnt : 0);
         }
-        if (live) n_neigh[orig_i] = (int)(po >> 2);
-        wmax = max(wmax, live ? (int)(po >> 2) : 0);
         __syncwarp();
     }
     wmax = __reduce_max_sync(FULL, wmax);
@@ -661,7 +641,7 @@ cudaError_t launch_traverse(const TraverseParams &p, const BuildBuffers &b, int3
             traverse_kernel<false><<<blocks, threads, 0, st>>>(p, b.nodes, b.sorted_pos, b.meta, nlist, n_neigh);
         return cudaGetLastError();
     }
-    const int ws = p.K > 16 ? 32 : (p.K > 8 ? 16 : (p.K > GW_FLAT_K ? 8 : 0));
+    const int ws = p.K > 16 ? 32 : (p.K > 8 ? 16 : 8);
     if (stats) {
         // census of the paper's per-particle walk (stats[0..4]), then the instrumented production kernel
         traverse_kernel<true><<<blocks, threads, 0, st>>>(p, b.nodes, b.sorted_pos, b.meta, nlist, n_neigh);
@@ -669,13 +649,11 @@ cudaError_t launch_traverse(const TraverseParams &p, const BuildBuffers &b, int3
         if (e != cudaSuccess) return e;
         if (ws == 32) launch_group<true, 32>(p, b, nlist, n_neigh, st);
         else if (ws == 16) launch_group<true, 16>(p, b, nlist, n_neigh, st);
-        else if (ws == 8) launch_group<true, 8>(p, b, nlist, n_neigh, st);
-        else launch_group<true, 0>(p, b, nlist, n_neigh, st);
+        else launch_group<true, 8>(p, b, nlist, n_neigh, st);
     } else {
         if (ws == 32) launch_group<false, 32>(p, b, nlist, n_neigh, st);
         else if (ws == 16) launch_group<false, 16>(p, b, nlist, n_neigh, st);
-        else if (ws == 8) launch_group<false, 8>(p, b, nlist, n_neigh, st);
-        else launch_group<false, 0>(p, b, nlist, n_neigh, st);
+        else launch_group<false, 8>(p, b, nlist, n_neigh, st);
     }
     return cudaGetLastError();
 }
