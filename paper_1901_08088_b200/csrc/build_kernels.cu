@@ -31,19 +31,80 @@ __device__ __forceinline__ uint32_t morton_bin(float p, float lo, float s) {
     return (uint32_t)f;
 }
 
+// One block of MORTON_THREADS threads: histograms -> exclusive offsets; segments, roots, frames.  Run by the last
+// block of morton_hist_kernel to finish (threads 0..255 own one digit each).
+__device__ void finalize_block(TreeMeta *__restrict__ meta, int N) {
+    __shared__ uint32_t s_scan[256];
+    __shared__ uint32_t s_ws[8];
+    const int d = threadIdx.x, lane = d & 31, warp = d >> 5;
+    for (int p = 0; p < 4; ++p) {
+        uint32_t c = 0, inc = 0;
+        if (d < 256) {
+            c = __ldcg(&meta->hist[p][d]);
+            inc = c;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                uint32_t v = __shfl_up_sync(0xFFFFFFFFu, inc, o);
+                if (lane >= o) inc += v;
+            }
+            if (lane == 31) s_ws[warp] = inc;
+        }
+        __syncthreads();
+        if (d < 256) {
+            uint32_t base = 0;
+            for (int w = 0; w < warp; ++w) base += s_ws[w];
+            uint32_t excl = base + inc - c;
+            meta->hist[p][d] = excl;
+            if (p == 3) s_scan[d] = excl;
+        }
+        __syncthreads();
+    }
+    if (d <= QBVH_TMAX) {
+        // type t owns top-digit values [64 t, 64 t + 63]
+        int s = (d < QBVH_TMAX) ? (int)s_scan[64 * d] : N;
+        meta->seg[d] = s;
+    }
+    if (d < QBVH_TMAX) {
+        int s = (int)s_scan[64 * d];
+        int e1 = (d + 1 < QBVH_TMAX) ? (int)s_scan[64 * (d + 1)] : N;
+        int n = e1 - s;
+        meta->roots[d] = (n <= 0) ? -1 : (n == 1 ? (N - 1 + s) : s);
+        float *fr = meta->frames[d];
+        if (n > 0) {
+            for (int a = 0; a < 3; ++a) {
+                float lo = ord2f(~__ldcg(&meta->mm_enc[d][a]));
+                float hi = ord2f(__ldcg(&meta->mm_enc[d][3 + a]));
+                fr[a] = lo;
+                fr[3 + a] = hi;
+                // Delta = div_ru(sub_ru(hi, lo), 1023): the 1023-bin grid spans at least the root box
+                fr[6 + a] = __fdiv_ru(__fsub_ru(hi, lo), QBVH_NBINS);
+            }
+        } else {
+            for (int a = 0; a < 9; ++a) fr[a] = 0.0f;
+        }
+        fr[9] = fr[10] = fr[11] = 0.0f;
+    }
+}
+
+constexpr int MORTON_THREADS = 512;
+
 template <int NT>
-__global__ void __launch_bounds__(256) morton_hist_kernel(const float *__restrict__ pos,
+__global__ void __launch_bounds__(MORTON_THREADS) morton_hist_kernel(const float *__restrict__ pos,
                                                            const int32_t *__restrict__ type, int N, float3 lo,
                                                            float3 scale, uint32_t *__restrict__ key_out,
                                                            TreeMeta *__restrict__ meta,
-                                                           uint32_t *__restrict__ status0, int status_words) {
+                                                           uint32_t *__restrict__ status0, int status_words,
+                                                           int32_t *__restrict__ entry, int entry_words) {
     __shared__ uint32_t s_hist[4][256];
+    __shared__ bool s_last;
     for (int i = threadIdx.x; i < 1024; i += blockDim.x) (&s_hist[0][0])[i] = 0;
     __syncthreads();
     const int stride = gridDim.x * blockDim.x;
     const int gtid = blockIdx.x * blockDim.x + threadIdx.x;
-    // the look-back status buffer of the first sort pass must be zero before that pass starts
+    // the look-back status buffer of the first sort pass must be zero before that pass starts; the entry table of
+    // the traversal starts out empty (-1) and is filled by hierarchy_kernel
     for (int i = gtid; i < status_words; i += stride) status0[i] = 0;
+    for (int i = gtid; i < entry_words; i += stride) entry[i] = -1;
 
     float mn[NT][3], mx[NT][3];
 #pragma unroll
@@ -54,35 +115,50 @@ __global__ void __launch_bounds__(256) morton_hist_kernel(const float *__restric
             mx[t][d] = -INFINITY;
         }
     bool bad_type = false;
-    for (int i = gtid; i < N; i += stride) {
-        float x = pos[3 * (size_t)i + 0], y = pos[3 * (size_t)i + 1], z = pos[3 * (size_t)i + 2];
-        uint32_t t = 0;
-        if (NT > 1 || type != nullptr) {
-            int tt = type ? type[i] : 0;
-            if (tt < 0 || tt >= NT) {
-                bad_type = true;
-                tt = 0;
-            }
-            t = (uint32_t)tt;
+    auto one = [&](float x, float y, float z, int tt) -> uint32_t {
+        if (tt < 0 || tt >= NT) {
+            bad_type = true;
+            tt = 0;
         }
+        const uint32_t t = (uint32_t)tt;
         uint32_t code = (spread10(morton_bin(x, lo.x, scale.x)) << 2) | (spread10(morton_bin(y, lo.y, scale.y)) << 1) |
                         spread10(morton_bin(z, lo.z, scale.z));
         uint32_t key = (t << 30) | code;
-        key_out[i] = key;
         atomicAdd(&s_hist[0][key & 255u], 1u);
         atomicAdd(&s_hist[1][(key >> 8) & 255u], 1u);
         atomicAdd(&s_hist[2][(key >> 16) & 255u], 1u);
         atomicAdd(&s_hist[3][key >> 24], 1u);
 #pragma unroll
-        for (int tt = 0; tt < NT; ++tt) {
-            bool m = (NT == 1) || (t == (uint32_t)tt);
-            mn[tt][0] = m ? fminf(mn[tt][0], x) : mn[tt][0];
-            mn[tt][1] = m ? fminf(mn[tt][1], y) : mn[tt][1];
-            mn[tt][2] = m ? fminf(mn[tt][2], z) : mn[tt][2];
-            mx[tt][0] = m ? fmaxf(mx[tt][0], x) : mx[tt][0];
-            mx[tt][1] = m ? fmaxf(mx[tt][1], y) : mx[tt][1];
-            mx[tt][2] = m ? fmaxf(mx[tt][2], z) : mx[tt][2];
+        for (int u = 0; u < NT; ++u) {
+            bool m = (NT == 1) || (t == (uint32_t)u);
+            mn[u][0] = m ? fminf(mn[u][0], x) : mn[u][0];
+            mn[u][1] = m ? fminf(mn[u][1], y) : mn[u][1];
+            mn[u][2] = m ? fminf(mn[u][2], z) : mn[u][2];
+            mx[u][0] = m ? fmaxf(mx[u][0], x) : mx[u][0];
+            mx[u][1] = m ? fmaxf(mx[u][1], y) : mx[u][1];
+            mx[u][2] = m ? fmaxf(mx[u][2], z) : mx[u][2];
         }
+        return key;
+    };
+    // four particles per thread and iteration: three 128-bit position loads, one 128-bit key store
+    const bool vec = ((reinterpret_cast<uintptr_t>(pos) & 15) == 0) && ((reinterpret_cast<uintptr_t>(key_out) & 15) == 0) &&
+                     (type == nullptr || (reinterpret_cast<uintptr_t>(type) & 15) == 0);
+    const int nquad = vec ? N / 4 : 0;
+    for (int q = gtid; q < nquad; q += stride) {
+        const float4 *p4 = reinterpret_cast<const float4 *>(pos) + 3 * (size_t)q;
+        const float4 a = __ldg(p4), b = __ldg(p4 + 1), c = __ldg(p4 + 2);
+        int4 tt = make_int4(0, 0, 0, 0);
+        if (type) tt = __ldg(reinterpret_cast<const int4 *>(type) + q);
+        uint4 k;
+        k.x = one(a.x, a.y, a.z, tt.x);
+        k.y = one(a.w, b.x, b.y, tt.y);
+        k.z = one(b.z, b.w, c.x, tt.z);
+        k.w = one(c.y, c.z, c.w, tt.w);
+        reinterpret_cast<uint4 *>(key_out)[q] = k;
+    }
+    for (int i = 4 * nquad + gtid; i < N; i += stride) {
+        const float x = pos[3 * (size_t)i + 0], y = pos[3 * (size_t)i + 1], z = pos[3 * (size_t)i + 2];
+        key_out[i] = one(x, y, z, type ? type[i] : 0);
     }
     // per-type min/max: warp reduce on the order-preserving encoding, one global atomic per warp and value
 #pragma unroll
@@ -102,57 +178,20 @@ __global__ void __launch_bounds__(256) morton_hist_kernel(const float *__restric
         uint32_t c = (&s_hist[0][0])[i];
         if (c) atomicAdd(&meta->hist[0][0] + i, c);
     }
+    // the last block to get here turns the histograms into offsets (segments, roots, frames)
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) s_last = atomicAdd(&meta->blocks_done, 1u) == gridDim.x - 1;
+    __syncthreads();
+    if (s_last) {
+        __threadfence();
+        finalize_block(meta, N);
+    }
 }
 
-// One block of 256 threads: histograms -> exclusive offsets; segments, roots, frames.
-__global__ void __launch_bounds__(256) finalize_kernel(TreeMeta *__restrict__ meta, int N, int T) {
-    __shared__ uint32_t s_scan[256];
-    __shared__ uint32_t s_ws[8];
-    const int d = threadIdx.x, lane = d & 31, warp = d >> 5;
-    for (int p = 0; p < 4; ++p) {
-        uint32_t c = meta->hist[p][d];
-        uint32_t inc = c;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            uint32_t v = __shfl_up_sync(0xFFFFFFFFu, inc, o);
-            if (lane >= o) inc += v;
-        }
-        if (lane == 31) s_ws[warp] = inc;
-        __syncthreads();
-        uint32_t base = 0;
-        for (int w = 0; w < warp; ++w) base += s_ws[w];
-        uint32_t excl = base + inc - c;
-        meta->hist[p][d] = excl;
-        if (p == 3) s_scan[d] = excl;
-        __syncthreads();
-    }
-    if (d <= QBVH_TMAX) {
-        // type t owns top-digit values [64 t, 64 t + 63]
-        int s = (d < QBVH_TMAX) ? (int)s_scan[64 * d] : N;
-        meta->seg[d] = s;
-    }
-    __syncthreads();
-    if (d < QBVH_TMAX) {
-        int s = (int)s_scan[64 * d];
-        int e1 = (d + 1 < QBVH_TMAX) ? (int)s_scan[64 * (d + 1)] : N;
-        int n = e1 - s;
-        meta->roots[d] = (n <= 0) ? -1 : (n == 1 ? (N - 1 + s) : s);
-        float *fr = meta->frames[d];
-        if (n > 0) {
-            for (int a = 0; a < 3; ++a) {
-                float lo = ord2f(~meta->mm_enc[d][a]);
-                float hi = ord2f(meta->mm_enc[d][3 + a]);
-                fr[a] = lo;
-                fr[3 + a] = hi;
-                // Delta = div_ru(sub_ru(hi, lo), 1023): the 1023-bin grid spans at least the root box
-                fr[6 + a] = __fdiv_ru(__fsub_ru(hi, lo), QBVH_NBINS);
-            }
-        } else {
-            for (int a = 0; a < 9; ++a) fr[a] = 0.0f;
-        }
-        fr[9] = fr[10] = fr[11] = 0.0f;
-    }
-    (void)T;
+// N = 0: only the bookkeeping
+__global__ void __launch_bounds__(MORTON_THREADS) finalize_kernel(TreeMeta *__restrict__ meta, int N) {
+    finalize_block(meta, N);
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -161,63 +200,72 @@ __global__ void __launch_bounds__(256) finalize_kernel(TreeMeta *__restrict__ me
 // per (tile, digit).  Stable: ties keep their input order at every level.  FIRST: values are implicit (= index).
 // ------------------------------------------------------------------------------------------------------------
 template <bool FIRST>
-__global__ void __launch_bounds__(SORT_THREADS) onesweep_kernel(const uint32_t *__restrict__ kin,
-                                                                 const uint32_t *__restrict__ vin,
-                                                                 uint32_t *__restrict__ kout,
-                                                                 uint32_t *__restrict__ vout, int N, int shift,
-                                                                 const uint32_t *__restrict__ hist_excl,
-                                                                 volatile uint32_t *status,
-                                                                 uint32_t *__restrict__ status_next,
-                                                                 uint32_t *__restrict__ tile_counter) {
-    __shared__ uint32_t s_whist[SORT_WARPS][256];
-    __shared__ uint32_t s_keys[SORT_TILE];
+__global__ void __launch_bounds__(SORT_THREADS, 2) onesweep_kernel(const uint32_t *__restrict__ kin,
+                                                                    const uint32_t *__restrict__ vin,
+                                                                    uint32_t *__restrict__ kout,
+                                                                    uint32_t *__restrict__ vout, int N, int shift,
+                                                                    const uint32_t *__restrict__ hist_excl,
+                                                                    volatile uint32_t *status,
+                                                                    uint32_t *__restrict__ status_next,
+                                                                    uint32_t *__restrict__ tile_counter) {
+    // per-warp digit counters while ranking; the tile's keys in output order afterwards (same storage)
+    __shared__ __align__(16) uint32_t s_buf[SORT_TILE];
     __shared__ uint32_t s_vals[SORT_TILE];
     __shared__ uint32_t s_dstart[256];
     __shared__ uint32_t s_gbase[256];
-    __shared__ uint32_t s_ws[SORT_WARPS];
+    __shared__ uint32_t s_ws[8];
     __shared__ uint32_t s_tile;
+    static_assert(SORT_WARPS * 256 <= SORT_TILE, "the per-warp counters live in the key buffer");
+    uint32_t(*s_whist)[256] = reinterpret_cast<uint32_t(*)[256]>(s_buf);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid == 0) s_tile = atomicAdd(tile_counter, 1u);
-    for (int i = tid; i < SORT_WARPS * 256; i += SORT_THREADS) (&s_whist[0][0])[i] = 0;
+    for (int i = tid; i < SORT_WARPS * 256; i += SORT_THREADS) s_buf[i] = 0;
     __syncthreads();
     const uint32_t tile = s_tile;
     const int base = (int)tile * SORT_TILE;
     const int nvalid = min(SORT_TILE, N - base);
-    status_next[(size_t)tile * 256 + tid] = 0;   // the other buffer: used by the next pass, idle now
+    if (tid < 256) status_next[(size_t)tile * 256 + tid] = 0;   // the other buffer: used by the next pass, idle now
 
-    uint32_t key[SORT_IPT];
+    uint32_t key[SORT_IPT], val[SORT_IPT];
     uint32_t rank[SORT_IPT];
     const int wbase = warp * (32 * SORT_IPT);
 #pragma unroll
     for (int r = 0; r < SORT_IPT; ++r) {
-        int li = wbase + r * 32 + lane;
+        const int li = wbase + r * 32 + lane;
         key[r] = (li < nvalid) ? kin[base + li] : 0xFFFFFFFFu;
+        val[r] = FIRST ? (uint32_t)(base + li) : ((li < nvalid) ? vin[base + li] : 0u);
     }
+    // ranks inside the warp: lanes with the same digit find each other by match.any; the lowest of them bumps the
+    // warp's counter of that digit (shared-memory atomic) and hands the old value to the others.  Rounds are
+    // ordered by the warp-wide shuffle, so equal digits keep their input order (stability).
     const uint32_t lt_mask = (1u << lane) - 1u;
 #pragma unroll
     for (int r = 0; r < SORT_IPT; ++r) {
-        int li = wbase + r * 32 + lane;
-        bool valid = li < nvalid;
-        uint32_t d = (key[r] >> shift) & 255u;
-        uint32_t m = __match_any_sync(0xFFFFFFFFu, valid ? d : 256u);
-        uint32_t before = s_whist[warp][d];
-        __syncwarp();
-        if (valid && (m & lt_mask) == 0) s_whist[warp][d] = before + __popc(m);
-        __syncwarp();
+        const int li = wbase + r * 32 + lane;
+        const bool valid = li < nvalid;
+        const uint32_t d = (key[r] >> shift) & 255u;
+        const uint32_t m = __match_any_sync(0xFFFFFFFFu, valid ? d : 256u);
+        uint32_t before = 0;
+        if (valid && (m & lt_mask) == 0) before = atomicAdd(&s_whist[warp][d], (uint32_t)__popc(m));
+        before = __shfl_sync(0xFFFFFFFFu, before, __ffs(m) - 1);
         rank[r] = before + __popc(m & lt_mask);
     }
     __syncthreads();
     // thread d owns digit d: exclusive scan over warps, then over digits, then over tiles (look-back)
-    {
+    if (tid < 256) {
         const int d = tid;
+        uint32_t c[SORT_WARPS];
+#pragma unroll
+        for (int w = 0; w < SORT_WARPS; ++w) c[w] = s_whist[w][d];
         uint32_t run = 0;
 #pragma unroll
         for (int w = 0; w < SORT_WARPS; ++w) {
-            uint32_t c = s_whist[w][d];
             s_whist[w][d] = run;
-            run += c;
+            run += c[w];
         }
         const uint32_t count = run;
+        if (tile == 0) status[d] = count | ST_PRE;
+        else status[(size_t)tile * 256 + d] = count | ST_AGG;
         uint32_t inc = count;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
@@ -225,26 +273,34 @@ __global__ void __launch_bounds__(SORT_THREADS) onesweep_kernel(const uint32_t *
             if (lane >= o) inc += v;
         }
         if (lane == 31) s_ws[warp] = inc;
-        __syncthreads();
+        asm volatile("bar.sync 1, 256;");      // the eight warps that own digits
         uint32_t wb = 0;
         for (int w = 0; w < warp; ++w) wb += s_ws[w];
         const uint32_t dstart = wb + inc - count;
         s_dstart[d] = dstart;
         uint32_t excl = 0;
-        if (tile == 0) {
-            status[d] = count | ST_PRE;
-        } else {
-            status[(size_t)tile * 256 + d] = count | ST_AGG;
+        if (tile != 0) {
+            // decoupled look-back, LB predecessors polled per round trip: all tiles of a pass are resident at once
+            // at these sizes, so the chain of prefixes advances LB tiles per L2 round trip
             int p = (int)tile - 1;
-            while (true) {
-                uint32_t v = status[(size_t)p * 256 + d];
-                if (v & ST_PRE) {
-                    excl += v & ST_VAL;
-                    break;
-                }
-                if (v & ST_AGG) {
-                    excl += v & ST_VAL;
-                    --p;
+            bool done = false;
+            while (!done) {
+                constexpr int LB = 16;
+                uint32_t v[LB];
+#pragma unroll
+                for (int u = 0; u < LB; ++u) v[u] = (p - u >= 0) ? (uint32_t)status[(size_t)(p - u) * 256 + d] : (uint32_t)(1u << 31);
+#pragma unroll
+                for (int u = 0; u < LB; ++u) {
+                    if (done) continue;
+                    if (v[u] & ST_PRE) {
+                        excl += v[u] & ST_VAL;
+                        done = true;
+                    } else if (v[u] & ST_AGG) {
+                        excl += v[u] & ST_VAL;
+                        --p;
+                    } else {
+                        break;                 // not published yet: poll again from here
+                    }
                 }
             }
             status[(size_t)tile * 256 + d] = (excl + count) | ST_PRE;
@@ -252,20 +308,25 @@ __global__ void __launch_bounds__(SORT_THREADS) onesweep_kernel(const uint32_t *
         s_gbase[d] = hist_excl[d] + excl - dstart;   // wraps mod 2^32; final index is exact
     }
     __syncthreads();
+    // position of every key inside the tile's output order
 #pragma unroll
     for (int r = 0; r < SORT_IPT; ++r) {
-        int li = wbase + r * 32 + lane;
+        const uint32_t d = (key[r] >> shift) & 255u;
+        rank[r] += s_dstart[d] + s_whist[warp][d];
+    }
+    __syncthreads();                                  // the counters are dead: their storage takes the keys
+#pragma unroll
+    for (int r = 0; r < SORT_IPT; ++r) {
+        const int li = wbase + r * 32 + lane;
         if (li < nvalid) {
-            uint32_t d = (key[r] >> shift) & 255u;
-            uint32_t p = s_dstart[d] + s_whist[warp][d] + rank[r];
-            s_keys[p] = key[r];
-            s_vals[p] = FIRST ? (uint32_t)(base + li) : vin[base + li];
+            s_buf[rank[r]] = key[r];
+            s_vals[rank[r]] = val[r];
         }
     }
     __syncthreads();
     for (int p = tid; p < nvalid; p += SORT_THREADS) {
-        uint32_t k = s_keys[p];
-        uint32_t g = s_gbase[(k >> shift) & 255u] + (uint32_t)p;
+        const uint32_t k = s_buf[p];
+        const uint32_t g = s_gbase[(k >> shift) & 255u] + (uint32_t)p;
         kout[g] = k;
         vout[g] = s_vals[p];
     }
@@ -291,7 +352,8 @@ __global__ void __launch_bounds__(256) hierarchy_kernel(const uint32_t *__restri
                                                          TreeMeta *__restrict__ meta, int4 *__restrict__ nodes,
                                                          int32_t *__restrict__ parent,
                                                          unsigned long long *__restrict__ slot,
-                                                         uint2 *__restrict__ groups, int K) {
+                                                         uint2 *__restrict__ groups, int32_t *__restrict__ entry,
+                                                         int K) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     // query groups found by this thread (at most two): maximal subtrees with <= GROUP_MAX leaves
     uint2 grp0 = make_uint2(0u, 0u), grp1 = make_uint2(0u, 0u);
@@ -309,8 +371,22 @@ __global__ void __launch_bounds__(256) hierarchy_kernel(const uint32_t *__restri
             return N - 1 + m;
         };
         int2 *nodes_lr = reinterpret_cast<int2 *>(nodes);   // {left, rope} = second half of the 16-byte node
+        // Entry table of the traversal.  The upper levels of an LBVH over Morton codes ARE a regular grid: all
+        // particles whose code starts with a given 3l-bit prefix (one cell of the 2^l-per-axis grid over the box,
+        // PAPER.md:61) form one subtree.  A node whose keys share `dnode` leading bits while its parent's share
+        // only `dpar` roots the cell of every level l with dpar < 2 + 3 l <= dnode (2 type bits, then the code).
+        int32_t *const etab = entry + t * ENTRY_CELLS;
+        auto emit_entry = [&](int dpar, int dnode, int node) {
+#pragma unroll
+            for (int l = ENTRY_LMIN; l <= ENTRY_LMAX; ++l) {
+                const int need = 2 + 3 * l;
+                if (dpar < need && need <= dnode) etab[entry_offset(l) + (int)((ki & 0x3FFFFFFFu) >> (30 - 3 * l))] = node;
+            }
+        };
+        const int dl = delta(k, ki, (long long)k - 1), dr = delta(k, ki, (long long)k + 1);
         // leaf k
         nodes_lr[2 * (size_t)(N - 1 + k) + 1] = make_int2(~k, rope_of(k));
+        emit_entry(max(dl, dr), 64, N - 1 + k);
         if (s == e) parent[N - 1 + k] = -1;                 // a one-particle tree: the leaf is the root
         if (k == s && e - s + 1 <= GROUP_MAX) {             // a whole tree that fits one group
             grp0 = make_uint2((uint32_t)s, (uint32_t)(e - s + 1));
@@ -324,7 +400,6 @@ __global__ void __launch_bounds__(256) hierarchy_kernel(const uint32_t *__restri
             }
         } else {
             // internal node k (Karras)
-            const int dl = delta(k, ki, (long long)k - 1), dr = delta(k, ki, (long long)k + 1);
             const int d = (dr > dl) ? 1 : -1;
             const int dmin = (dr > dl) ? dl : dr;
             long long lmax = 2;
@@ -346,6 +421,7 @@ __global__ void __launch_bounds__(256) hierarchy_kernel(const uint32_t *__restri
             parent[lc] = k;
             parent[rc] = k;
             if (k == s) parent[k] = -1;
+            emit_entry(dmin, dnode, k);
             const int size = la - f + 1;
             const int leftword = (K > 1 && size <= K) ? ~f : lc;   // collapsed range leaf: first sorted position
             nodes_lr[2 * (size_t)k + 1] = make_int2(leftword, rope_of(la));
@@ -438,68 +514,28 @@ __global__ void __launch_bounds__(256) fit_kernel(const float *__restrict__ pos,
 }
 
 // ------------------------------------------------------------------------------------------------------------
-// Entry table.  The upper levels of an LBVH over Morton codes ARE a regular grid: all particles whose code starts
-// with a given 3l-bit prefix (one cell of the 2^l x 2^l x 2^l grid over the box) form one subtree.
-// For l = 2..5 and every cell the table holds the node that roots that subtree (-1: empty cell), so a traversal
-// can enter the tree at the cells its search volume touches instead of walking down from the root.
-// The particles with prefix c are the sorted positions [a, b); the node covering exactly [a, b-1] is internal
-// node b-1 if it is a left child (its keys are closer to the right outside neighbor) and internal node a if it
-// is a right child (SURVEY.md B.1 numbering); a single particle is leaf a.
-// ------------------------------------------------------------------------------------------------------------
-__device__ __forceinline__ int lower_bound_key(const uint32_t *__restrict__ key, int N, unsigned long long v) {
-    int lo = 0, hi = N;
-    while (lo < hi) {
-        const int mid = (lo + hi) >> 1;
-        if ((unsigned long long)__ldg(key + mid) < v) lo = mid + 1; else hi = mid;
-    }
-    return lo;
-}
-
-__global__ void __launch_bounds__(256) entry_table_kernel(const uint32_t *__restrict__ key, int N,
-                                                           const TreeMeta *__restrict__ meta,
-                                                           int32_t *__restrict__ table, int T) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= T * ENTRY_CELLS) return;
-    const int t = i / ENTRY_CELLS, r = i - t * ENTRY_CELLS;
-    const int l = (r < entry_offset(3)) ? 2 : (r < entry_offset(4)) ? 3 : (r < entry_offset(5)) ? 4 : 5;
-    const unsigned long long c = (unsigned long long)(r - entry_offset(l));
-    const int shift = 30 - 3 * l;
-    const unsigned long long klo = ((unsigned long long)t << 30) | (c << shift), khi = klo + (1ull << shift);
-    const int a = lower_bound_key(key, N, klo), b = lower_bound_key(key, N, khi);
-    int node = -1;
-    if (b - a == 1) {
-        node = N - 1 + a;
-    } else if (b - a > 1) {
-        const int s = meta->seg[t], e = meta->seg[t + 1] - 1;
-        const int dl = (a - 1 < s) ? -1 : __clz(__ldg(key + a - 1) ^ __ldg(key + a));
-        const int dr = (b > e) ? -1 : __clz(__ldg(key + b - 1) ^ __ldg(key + b));
-        node = (dr > dl) ? b - 1 : a;
-    }
-    table[i] = node;
-}
-
-// ------------------------------------------------------------------------------------------------------------
 cudaError_t launch_build(const float *pos, const int32_t *type, int N, int T, int K, const float *box_lo,
                          const float *box_scale, const BuildBuffers &b, cudaStream_t st) {
     cudaError_t err = cudaMemsetAsync(b.meta, 0, sizeof(TreeMeta), st);
     if (err != cudaSuccess) return err;
     if (N == 0) {
-        finalize_kernel<<<1, 256, 0, st>>>(b.meta, 0, T);
+        finalize_kernel<<<1, MORTON_THREADS, 0, st>>>(b.meta, 0);
         return cudaGetLastError();
     }
     const int tiles = (N + SORT_TILE - 1) / SORT_TILE;
     const int status_words = tiles * 256;
+    const int entry_words = QBVH_TMAX * ENTRY_CELLS;
     const float3 lo = make_float3(box_lo[0], box_lo[1], box_lo[2]);
     const float3 sc = make_float3(box_scale[0], box_scale[1], box_scale[2]);
-    int mblocks = (N + 255) / 256;
-    if (mblocks > 148 * 8) mblocks = 148 * 8;
+    int mblocks = (N / 4 + MORTON_THREADS - 1) / MORTON_THREADS;
+    if (mblocks > 148 * 2) mblocks = 148 * 2;
+    if (mblocks < 1) mblocks = 1;
     switch (T) {
-        case 1: morton_hist_kernel<1><<<mblocks, 256, 0, st>>>(pos, type, N, lo, sc, b.key_a, b.meta, b.status[0], status_words); break;
-        case 2: morton_hist_kernel<2><<<mblocks, 256, 0, st>>>(pos, type, N, lo, sc, b.key_a, b.meta, b.status[0], status_words); break;
-        case 3: morton_hist_kernel<3><<<mblocks, 256, 0, st>>>(pos, type, N, lo, sc, b.key_a, b.meta, b.status[0], status_words); break;
-        default: morton_hist_kernel<4><<<mblocks, 256, 0, st>>>(pos, type, N, lo, sc, b.key_a, b.meta, b.status[0], status_words); break;
+        case 1: morton_hist_kernel<1><<<mblocks, MORTON_THREADS, 0, st>>>(pos, type, N, lo, sc, b.key_a, b.meta, b.status[0], status_words, b.entry, entry_words); break;
+        case 2: morton_hist_kernel<2><<<mblocks, MORTON_THREADS, 0, st>>>(pos, type, N, lo, sc, b.key_a, b.meta, b.status[0], status_words, b.entry, entry_words); break;
+        case 3: morton_hist_kernel<3><<<mblocks, MORTON_THREADS, 0, st>>>(pos, type, N, lo, sc, b.key_a, b.meta, b.status[0], status_words, b.entry, entry_words); break;
+        default: morton_hist_kernel<4><<<mblocks, MORTON_THREADS, 0, st>>>(pos, type, N, lo, sc, b.key_a, b.meta, b.status[0], status_words, b.entry, entry_words); break;
     }
-    finalize_kernel<<<1, 256, 0, st>>>(b.meta, N, T);
     // four passes a -> b -> a -> b -> a
     onesweep_kernel<true><<<tiles, SORT_THREADS, 0, st>>>(b.key_a, nullptr, b.key_b, b.idx_b, N, 0, b.meta->hist[0],
                                                           b.status[0], b.status[1], &b.meta->tile_counter[0]);
@@ -510,8 +546,7 @@ cudaError_t launch_build(const float *pos, const int32_t *type, int N, int T, in
     onesweep_kernel<false><<<tiles, SORT_THREADS, 0, st>>>(b.key_b, b.idx_b, b.key_a, b.idx_a, N, 24, b.meta->hist[3],
                                                            b.status[1], b.status[0], &b.meta->tile_counter[3]);
     const int nb = (N + 255) / 256;
-    hierarchy_kernel<<<nb, 256, 0, st>>>(b.key_a, N, b.meta, b.nodes, b.parent, b.slot, b.groups, K);
+    hierarchy_kernel<<<nb, 256, 0, st>>>(b.key_a, N, b.meta, b.nodes, b.parent, b.slot, b.groups, b.entry, K);
     fit_kernel<<<nb, 256, 0, st>>>(pos, b.idx_a, b.key_a, N, b.meta, b.sorted_pos, b.nodes, b.parent, b.slot);
-    entry_table_kernel<<<(T * ENTRY_CELLS + 255) / 256, 256, 0, st>>>(b.key_a, N, b.meta, b.entry, T);
     return cudaGetLastError();
 }

@@ -10,6 +10,7 @@
 struct TreeMeta {
     uint32_t hist[4][256];     // per-pass digit histograms, turned into exclusive offsets by finalize_kernel
     uint32_t tile_counter[4];  // dynamic tile ids of the four onesweep passes
+    uint32_t blocks_done;      // blocks of morton_hist_kernel that have added their histograms (the last one finalizes)
     uint32_t mm_enc[QBVH_TMAX][6];  // per type: ~enc(min xyz) (so atomicMax computes the min), enc(max xyz)
     int32_t seg[QBVH_TMAX + 1];     // first sorted position of each type; seg[T..4] = N
     int32_t roots[QBVH_TMAX];       // root node per type, -1 if empty
@@ -38,9 +39,9 @@ __device__ inline float ord2f(uint32_t o) {
 #define SLOT_EMPTY 0xFFFFFFFFFFFFFFFFull
 
 // ---- sort geometry ----
-constexpr int SORT_THREADS = 256;
+constexpr int SORT_THREADS = 512;
 constexpr int SORT_WARPS = SORT_THREADS / 32;
-constexpr int SORT_IPT = 16;                          // keys per thread
+constexpr int SORT_IPT = 8;                           // keys per thread
 constexpr int SORT_TILE = SORT_THREADS * SORT_IPT;    // 4096 keys per tile
 constexpr uint32_t ST_AGG = 1u << 30;                 // tile status: aggregate (own count) available
 constexpr uint32_t ST_PRE = 1u << 31;                 // tile status: inclusive prefix available
