@@ -193,6 +193,12 @@ __device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c) {
 #ifndef QBVH_GW_RING
 #define QBVH_GW_RING 32
 #endif
+#ifndef QBVH_GW_FETCH
+#define QBVH_GW_FETCH 1      // consecutive query groups a warp takes per visit to the cursor
+#endif
+#ifndef QBVH_GW_QUADFLUSH
+#define QBVH_GW_QUADFLUSH 0  // 1: a flush writes every complete 16-byte quad of every lane; 0: 64-byte blocks only
+#endif
 constexpr int GW_WARPS = QBVH_GW_WARPS;   // warps per block
 constexpr int GW_WL = 256;       // work-list entries per warp
 constexpr int GW_LQ = 96;        // leaf-queue entries per warp
@@ -321,12 +327,16 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
     unsigned long long st_tests = 0, st_leaf = 0, st_cand = 0, st_checks = 0, st_steps = 0, st_groups = 0;
     int wmax = 0;
 
+    int g = 0, g_end = 0;
     while (true) {
-        int g = 0;
-        if (lane == 0) g = atomicAdd(&meta->group_cursor, 1);
-        g = __shfl_sync(FULL, g, 0);
-        if (g >= ngroups) break;
+        if (g >= g_end) {
+            if (lane == 0) g = atomicAdd(&meta->group_cursor, QBVH_GW_FETCH);
+            g = __shfl_sync(FULL, g, 0);
+            g_end = min(g + QBVH_GW_FETCH, ngroups);
+            if (g >= ngroups) break;
+        }
         const uint2 grp = __ldg(groups + g);
+        ++g;
         const int gfirst = (int)grp.x, gcnt = (int)grp.y;
         const bool live = lane < gcnt;
         const float4 me = live ? __ldg(sorted_pos + gfirst + lane) : make_float4(0.f, 0.f, 0.f, 0.f);
@@ -353,6 +363,21 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
 
         // lanes write their complete 64-byte blocks of staged neighbors to their list rows
         auto flush_blocks = [&]() {
+            if (QBVH_GW_QUADFLUSH) {
+                // every lane writes all its complete quads: up to (GW_RING - 1) / 4 of them
+                const int nq = ((int)((po - rot) >> 2) - flushed) >> 2;
+                const int maxq = __reduce_max_sync(FULL, nq);
+                const uint32_t off = rot + 4u * (uint32_t)flushed;
+                for (int q = 0; q < maxq; ++q) {
+                    if (q < nq) {
+                        const int4 v = *static_cast<const int4 *>(
+                            __cvta_shared_to_generic((size_t)(ring_s | ((off + 16u * q) & (GW_RING_BYTES - 16)))));
+                        store4(row, flushed + 4 * q, cap, vec_ok, v);
+                    }
+                }
+                flushed += 4 * nq;
+                return;
+            }
             while (__any_sync(FULL, (int)((po - rot) >> 2) - flushed >= 16)) {
                 if ((int)((po - rot) >> 2) - flushed >= 16) {
                     const uint32_t off = rot + 4u * (uint32_t)flushed;
@@ -489,10 +514,15 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
                         int4 A = make_int4(0, 0, 0, 0), B = make_int4(0, 0, 0, 0);
                         if (lane < npop) {
                             const uint32_t ent = sm.wl[wsz - 1 - lane];
-                            A = __ldg(nodes + (ent & 0x7FFFFFFFu));
+                            const int ia = (int)(ent & 0x7FFFFFFFu);
+                            A = __ldg(nodes + ia);
                             if (ent >> 31) {
+                                // A is a left child; its rope is its right sibling: internal node gamma + 1 or leaf
+                                // gamma + 1 (SURVEY.md B.1 numbering).  Load both without waiting for A.
                                 pairf = 1;
-                                B = __ldg(nodes + A.w);
+                                const int gam = ia < P.N - 1 ? ia : ia - (P.N - 1);
+                                const int4 B1 = __ldg(nodes + gam + 1), B2 = __ldg(nodes + P.N + gam);
+                                B = (A.w == gam + 1) ? B1 : B2;
                             }
                             const bool hitA = node_overlaps(A, flo, fdl, blo, bhi, R2);
                             pushA = hitA && A.z >= 0;
