@@ -193,12 +193,7 @@ __device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c) {
 #ifndef QBVH_GW_RING
 #define QBVH_GW_RING 32
 #endif
-#ifndef QBVH_GW_FETCH
-#define QBVH_GW_FETCH 1      // consecutive query groups a warp takes per visit to the cursor
-#endif
-#ifndef QBVH_GW_QUADFLUSH
-#define QBVH_GW_QUADFLUSH 0  // 1: a flush writes every complete 16-byte quad of every lane; 0: 64-byte blocks only
-#endif
+
 constexpr int GW_WARPS = QBVH_GW_WARPS;   // warps per block
 constexpr int GW_WL = 256;       // work-list entries per warp
 constexpr int GW_LQ = 96;        // leaf-queue entries per warp
@@ -327,16 +322,12 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
     unsigned long long st_tests = 0, st_leaf = 0, st_cand = 0, st_checks = 0, st_steps = 0, st_groups = 0;
     int wmax = 0;
 
-    int g = 0, g_end = 0;
     while (true) {
-        if (g >= g_end) {
-            if (lane == 0) g = atomicAdd(&meta->group_cursor, QBVH_GW_FETCH);
-            g = __shfl_sync(FULL, g, 0);
-            g_end = min(g + QBVH_GW_FETCH, ngroups);
-            if (g >= ngroups) break;
-        }
+        int g = 0;
+        if (lane == 0) g = atomicAdd(&meta->group_cursor, 1);
+        g = __shfl_sync(FULL, g, 0);
+        if (g >= ngroups) break;
         const uint2 grp = __ldg(groups + g);
-        ++g;
         const int gfirst = (int)grp.x, gcnt = (int)grp.y;
         const bool live = lane < gcnt;
         const float4 me = live ? __ldg(sorted_pos + gfirst + lane) : make_float4(0.f, 0.f, 0.f, 0.f);
@@ -363,29 +354,21 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
 
         // lanes write their complete 64-byte blocks of staged neighbors to their list rows
         auto flush_blocks = [&]() {
-            if (QBVH_GW_QUADFLUSH) {
-                // every lane writes all its complete quads: up to (GW_RING - 1) / 4 of them
-                const int nq = ((int)((po - rot) >> 2) - flushed) >> 2;
-                const int maxq = __reduce_max_sync(FULL, nq);
-                const uint32_t off = rot + 4u * (uint32_t)flushed;
-                for (int q = 0; q < maxq; ++q) {
-                    if (q < nq) {
-                        const int4 v = *static_cast<const int4 *>(
-                            __cvta_shared_to_generic((size_t)(ring_s | ((off + 16u * q) & (GW_RING_BYTES - 16)))));
-                        store4(row, flushed + 4 * q, cap, vec_ok, v);
-                    }
-                }
-                flushed += 4 * nq;
-                return;
-            }
             while (__any_sync(FULL, (int)((po - rot) >> 2) - flushed >= 16)) {
                 if ((int)((po - rot) >> 2) - flushed >= 16) {
                     const uint32_t off = rot + 4u * (uint32_t)flushed;
+                    int4 v[4];
 #pragma unroll
-                    for (int j = 0; j < 4; ++j) {
-                        const int4 v = *static_cast<const int4 *>(
+                    for (int j = 0; j < 4; ++j)
+                        v[j] = *static_cast<const int4 *>(
                             __cvta_shared_to_generic((size_t)(ring_s | ((off + 16u * j) & (GW_RING_BYTES - 16)))));
-                        store4(row, flushed + 4 * j, cap, vec_ok, v);
+                    if (vec_ok && flushed + 16 <= cap) {          // the common case: four aligned 128-bit stores
+                        int4 *dst = reinterpret_cast<int4 *>(row + flushed);
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) dst[j] = v[j];
+                    } else {
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) store4(row, flushed + 4 * j, cap, false, v[j]);
                     }
                     flushed += 16;
                 }
@@ -561,10 +544,10 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
                         if (li < take) lfA = sm.lq[lqn - 1 - li];
                         if (NL + li < take) lfB = sm.lq[lqn - 1 - NL - li];
                         lqn -= take;
-                        float4 pA = make_float4(0.f, 0.f, 0.f, 0.f), pB = pA;
+                        // lanes past the end of their leaf load its first particle instead (no branch) and drop it
                         const bool vA = sub < (int)lfA.y, vB = sub < (int)lfB.y;
-                        if (vA) pA = __ldg(sorted_pos + (int)lfA.x + sub);
-                        if (vB) pB = __ldg(sorted_pos + (int)lfB.x + sub);
+                        const float4 pA = __ldg(sorted_pos + (lfA.x + (vA ? (uint32_t)sub : 0u)));
+                        const float4 pB = __ldg(sorted_pos + (lfB.x + (vB ? (uint32_t)sub : 0u)));
                         const bool keepA = vA && point_in_reach(pA, blo, bhi, R2);
                         const bool keepB = vB && point_in_reach(pB, blo, bhi, R2);
                         const uint32_t ka = __ballot_sync(FULL, keepA), kb = __ballot_sync(FULL, keepB);
