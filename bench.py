@@ -24,7 +24,7 @@ sys.path.insert(0, ROOT)
 
 METRIC = "neighbor-list build+traverse ns/particle at 1M LJ"
 UNIT = "ns/particle"
-KERNELS_PER_STEP = 8    # morton_hist (+finalize in its last block), 4 x onesweep, hierarchy (+entry table), fit, traverse_group
+KERNELS_PER_STEP = 7    # morton_hist (+finalize in its last block), 4 x onesweep, tree (hierarchy+fit+quantize), traverse_group
 
 
 def measured_peaks():

@@ -25,6 +25,8 @@ struct Context {
     float box[6] = {0, 0, 0, 0, 0, 0};
     float scale[3] = {0, 0, 0};
     BuildBuffers buf{};
+    uint32_t build_tag = 0;      // tag of the last build's meeting slots; 0: the slot area has to be cleared first
+    int64_t tag_N = -1;          // the layout (N) the slot area was cleared for
     int32_t *pinned = nullptr;   // 2 ints: max_count, err_flags
     qbvh_stats last_stats{};
     char cuda_msg[256] = "no CUDA error recorded";
@@ -56,7 +58,7 @@ Layout make_layout(int64_t N) {
     L.sorted_pos = take(16 * n1);
     L.nodes = take(16 * (2 * n1 - 1));
     L.parent = take(4 * (2 * n1 - 1));
-    L.slot = take(8 * n1);
+    L.slot = take(16 * n1);
     L.groups = take(8 * n1);
     L.entry = take(4 * (int64_t)QBVH_TMAX * ENTRY_CELLS);
     L.total = off;
@@ -165,6 +167,7 @@ int64_t qbvh_workspace_bytes(int64_t N, int32_t T) {
 
 int qbvh_set_workspace(void *dev_ptr, int64_t bytes) {
     g.built = false;
+    g.build_tag = 0;
     if (dev_ptr && ((reinterpret_cast<uintptr_t>(dev_ptr) & 255) || bytes <= 0)) return QBVH_ERR_WORKSPACE;
     g.ws = dev_ptr;
     g.ws_bytes = dev_ptr ? bytes : 0;
@@ -221,7 +224,7 @@ int qbvh_build(const float *pos, const int32_t *type, int64_t N, const float *bo
     g.buf.sorted_pos = reinterpret_cast<float4 *>(w + L.sorted_pos);
     g.buf.nodes = reinterpret_cast<int4 *>(w + L.nodes);
     g.buf.parent = reinterpret_cast<int32_t *>(w + L.parent);
-    g.buf.slot = reinterpret_cast<unsigned long long *>(w + L.slot);
+    g.buf.slot = reinterpret_cast<uint4 *>(w + L.slot);
     g.buf.groups = reinterpret_cast<uint2 *>(w + L.groups);
     g.buf.entry = reinterpret_cast<int32_t *>(w + L.entry);
     std::memcpy(g.box, box, sizeof(g.box));
@@ -232,7 +235,15 @@ int qbvh_build(const float *pos, const int32_t *type, int64_t N, const float *bo
     }
     for (int d = 0; d < 3; ++d) g.scale[d] = scale[d];
     const int T = type ? g.T : 1;
-    cudaError_t e = launch_build(pos, type, (int)N, T, g.K, box, scale, g.buf, g.stream);
+    // the meeting slots of tree_kernel carry a 24-bit build number; clear them when the layout moves or it wraps
+    if (g.build_tag == 0 || g.build_tag >= 0xFFFFFFu || g.tag_N != N) {
+        cudaError_t em = cudaMemsetAsync(g.buf.slot, 0, (size_t)16 * (size_t)(N > 0 ? N : 1), g.stream);
+        if (em != cudaSuccess) return cuda_fail(em, "memset slots");
+        g.build_tag = 0;
+        g.tag_N = N;
+    }
+    ++g.build_tag;
+    cudaError_t e = launch_build(pos, type, (int)N, T, g.K, box, scale, g.buf, g.build_tag, g.stream);
     if (e != cudaSuccess) return cuda_fail(e, "build launch");
     g.N = N;
     g.K_built = g.K;

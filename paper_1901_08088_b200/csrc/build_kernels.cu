@@ -160,7 +160,11 @@ __global__ void __launch_bounds__(MORTON_THREADS) morton_hist_kernel(const float
         const float x = pos[3 * (size_t)i + 0], y = pos[3 * (size_t)i + 1], z = pos[3 * (size_t)i + 2];
         key_out[i] = one(x, y, z, type ? type[i] : 0);
     }
-    // per-type min/max: warp reduce on the order-preserving encoding, one global atomic per warp and value
+    // per-type min/max: warp reduce on the order-preserving encoding, block reduce through shared memory, then one
+    // global atomic per block and value (same-address atomics serialise in L2)
+    __shared__ uint32_t s_mm[QBVH_TMAX][6];
+    if (threadIdx.x < QBVH_TMAX * 6) (&s_mm[0][0])[threadIdx.x] = 0u;
+    __syncthreads();
 #pragma unroll
     for (int t = 0; t < NT; ++t)
 #pragma unroll
@@ -168,25 +172,31 @@ __global__ void __launch_bounds__(MORTON_THREADS) morton_hist_kernel(const float
             uint32_t a = __reduce_max_sync(0xFFFFFFFFu, ~f2ord(mn[t][d]));
             uint32_t b = __reduce_max_sync(0xFFFFFFFFu, f2ord(mx[t][d]));
             if ((threadIdx.x & 31) == 0) {
-                if (a != ~f2ord(INFINITY)) atomicMax(&meta->mm_enc[t][d], a);
-                if (b != f2ord(-INFINITY)) atomicMax(&meta->mm_enc[t][3 + d], b);
+                if (a != ~f2ord(INFINITY)) atomicMax(&s_mm[t][d], a);
+                if (b != f2ord(-INFINITY)) atomicMax(&s_mm[t][3 + d], b);
             }
         }
+    __syncthreads();
+    if (threadIdx.x < NT * 6) {
+        const uint32_t v = (&s_mm[0][0])[threadIdx.x];
+        if (v) atomicMax(&meta->mm_enc[0][0] + threadIdx.x, v);
+    }
     if (bad_type) atomicOr(&meta->err_flags, 1);
     __syncthreads();
     for (int i = threadIdx.x; i < 1024; i += blockDim.x) {
         uint32_t c = (&s_hist[0][0])[i];
         if (c) atomicAdd(&meta->hist[0][0] + i, c);
     }
-    // the last block to get here turns the histograms into offsets (segments, roots, frames)
-    __threadfence();
+    // the last block to get here turns the histograms into offsets (segments, roots, frames).  One cumulative
+    // fence by thread 0 after the barrier orders the whole block's atomics before its ticket.
     __syncthreads();
-    if (threadIdx.x == 0) s_last = atomicAdd(&meta->blocks_done, 1u) == gridDim.x - 1;
-    __syncthreads();
-    if (s_last) {
+    if (threadIdx.x == 0) {
         __threadfence();
-        finalize_block(meta, N);
+        s_last = atomicAdd(&meta->blocks_done, 1u) == gridDim.x - 1;
+        __threadfence();
     }
+    __syncthreads();
+    if (s_last) finalize_block(meta, N);
 }
 
 // N = 0: only the bookkeeping
@@ -333,129 +343,23 @@ __global__ void __launch_bounds__(SORT_THREADS, 2) onesweep_kernel(const uint32_
 }
 
 // ------------------------------------------------------------------------------------------------------------
-// a3 + a4. One thread per sorted position k: leaf k's node words and (if it exists) internal node k.
-// delta(i,j) = length of the common prefix of the augmented keys (key, position); -1 outside the type segment.
-// Rope of a node covering [f,l] (pinned in tests/test_oracle_tree.py): END if l is the segment
-// end, else with m = l+1: internal node m if its range starts at m, else leaf m.
-// ------------------------------------------------------------------------------------------------------------
-struct SegDelta {
-    const uint32_t *key;
-    int s, e;
-    __device__ __forceinline__ int operator()(int i, uint32_t ki, long long j) const {
-        if (j < s || j > e) return -1;
-        uint32_t x = ki ^ __ldg(key + j);
-        return x ? __clz(x) : 32 + __clz((uint32_t)i ^ (uint32_t)j);
-    }
-};
-
-__global__ void __launch_bounds__(256) hierarchy_kernel(const uint32_t *__restrict__ key, int N,
-                                                         TreeMeta *__restrict__ meta, int4 *__restrict__ nodes,
-                                                         int32_t *__restrict__ parent,
-                                                         unsigned long long *__restrict__ slot,
-                                                         uint2 *__restrict__ groups, int32_t *__restrict__ entry,
-                                                         int K) {
-    const int k = blockIdx.x * blockDim.x + threadIdx.x;
-    // query groups found by this thread (at most two): maximal subtrees with <= GROUP_MAX leaves
-    uint2 grp0 = make_uint2(0u, 0u), grp1 = make_uint2(0u, 0u);
-    int ngrp = 0;
-    if (k < N) {
-        const uint32_t ki = key[k];
-        const int t = ki >> 30;
-        SegDelta delta{key, meta->seg[t], meta->seg[t + 1] - 1};
-        const int s = delta.s, e = delta.e;
-        auto rope_of = [&](int l) -> int {
-            if (l == e) return -1;
-            const int m = l + 1;
-            const uint32_t km = __ldg(key + m);
-            if (m <= e - 1 && delta(m, km, m + 1) > delta(m, km, m - 1)) return m;
-            return N - 1 + m;
-        };
-        int2 *nodes_lr = reinterpret_cast<int2 *>(nodes);   // {left, rope} = second half of the 16-byte node
-        // Entry table of the traversal.  The upper levels of an LBVH over Morton codes ARE a regular grid: all
-        // particles whose code starts with a given 3l-bit prefix (one cell of the 2^l-per-axis grid over the box,
-        // PAPER.md:61) form one subtree.  A node whose keys share `dnode` leading bits while its parent's share
-        // only `dpar` roots the cell of every level l with dpar < 2 + 3 l <= dnode (2 type bits, then the code).
-        int32_t *const etab = entry + t * ENTRY_CELLS;
-        auto emit_entry = [&](int dpar, int dnode, int node) {
-#pragma unroll
-            for (int l = ENTRY_LMIN; l <= ENTRY_LMAX; ++l) {
-                const int need = 2 + 3 * l;
-                if (dpar < need && need <= dnode) etab[entry_offset(l) + (int)((ki & 0x3FFFFFFFu) >> (30 - 3 * l))] = node;
-            }
-        };
-        const int dl = delta(k, ki, (long long)k - 1), dr = delta(k, ki, (long long)k + 1);
-        // leaf k
-        nodes_lr[2 * (size_t)(N - 1 + k) + 1] = make_int2(~k, rope_of(k));
-        emit_entry(max(dl, dr), 64, N - 1 + k);
-        if (s == e) parent[N - 1 + k] = -1;                 // a one-particle tree: the leaf is the root
-        if (k == s && e - s + 1 <= GROUP_MAX) {             // a whole tree that fits one group
-            grp0 = make_uint2((uint32_t)s, (uint32_t)(e - s + 1));
-            ngrp = 1;
-        }
-        if (k == e) {                                       // no internal node carries the index of a segment end
-            if (k < N - 1) {
-                nodes[k] = make_int4(0, 0, 0, -1);
-                parent[k] = -1;
-                slot[k] = SLOT_EMPTY;
-            }
-        } else {
-            // internal node k (Karras)
-            const int d = (dr > dl) ? 1 : -1;
-            const int dmin = (dr > dl) ? dl : dr;
-            long long lmax = 2;
-            while (delta(k, ki, k + lmax * d) > dmin) lmax <<= 1;
-            long long l = 0;
-            for (long long tt = lmax >> 1; tt >= 1; tt >>= 1)
-                if (delta(k, ki, k + (l + tt) * d) > dmin) l += tt;
-            const int j = (int)(k + l * d);
-            const int dnode = delta(k, ki, j);
-            long long sp = 0, tt = l;
-            do {
-                tt = (tt + 1) >> 1;
-                if (delta(k, ki, k + (sp + tt) * d) > dnode) sp += tt;
-            } while (tt > 1);
-            const int gamma = (int)(k + sp * d + (d < 0 ? -1 : 0));
-            const int f = min(k, j), la = max(k, j);
-            const int lc = (f == gamma) ? (N - 1 + gamma) : gamma;
-            const int rc = (la == gamma + 1) ? (N - 1 + gamma + 1) : (gamma + 1);
-            parent[lc] = k;
-            parent[rc] = k;
-            if (k == s) parent[k] = -1;
-            emit_entry(dmin, dnode, k);
-            const int size = la - f + 1;
-            const int leftword = (K > 1 && size <= K) ? ~f : lc;   // collapsed range leaf: first sorted position
-            nodes_lr[2 * (size_t)k + 1] = make_int2(leftword, rope_of(la));
-            slot[k] = SLOT_EMPTY;
-            if (size > GROUP_MAX) {                         // children that fit are maximal: they become groups
-                const int lsize = gamma - f + 1, rsize = la - gamma;
-                if (lsize <= GROUP_MAX) {
-                    grp0 = make_uint2((uint32_t)f, (uint32_t)lsize);
-                    ngrp = 1;
-                }
-                if (rsize <= GROUP_MAX) {
-                    const uint2 gr = make_uint2((uint32_t)(gamma + 1), (uint32_t)rsize);
-                    if (ngrp) grp1 = gr; else grp0 = gr;
-                    ++ngrp;
-                }
-            }
-        }
-    }
-    // append this warp's groups with one atomic
-    const uint32_t b1 = __ballot_sync(0xFFFFFFFFu, ngrp >= 1), b2 = __ballot_sync(0xFFFFFFFFu, ngrp >= 2);
-    const int total = __popc(b1) + __popc(b2);
-    if (total) {
-        const int lane = threadIdx.x & 31;
-        const uint32_t lt = (1u << lane) - 1u;
-        int base = 0;
-        if (lane == 0) base = atomicAdd(&meta->group_count, total);
-        base = __shfl_sync(0xFFFFFFFFu, base, 0) + __popc(b1 & lt) + __popc(b2 & lt);
-        if (ngrp >= 1) groups[base] = grp0;
-        if (ngrp >= 2) groups[base + 1] = grp1;
-    }
-}
-
-// ------------------------------------------------------------------------------------------------------------
-// a2' + a5 + a6.  Quantizer defined by its decompressor:
+// a2' + a3 + a4 + a5 + a6 in ONE bottom-up pass (tree_kernel).  One thread per sorted position k.
+//
+// Hierarchy (Karras' binary radix tree, "built bottom up"): every node covers a contiguous range
+// [f,l] of the sorted augmented keys (key, position).  With dL = delta(f-1,f) and dR = delta(l,l+1) the common
+// prefix lengths with the outside neighbours (-1 beyond the type segment), the node is the LEFT child of its
+// parent iff dR > dL, and then the parent splits at gamma = l; otherwise it is the RIGHT child and gamma = f-1.
+// (dL = dR only at the root, where both are -1.)  The two children of a parent meet at slot[gamma]: the first to
+// arrive leaves {its packed box, the far end of its range, its outer delta} there with ONE 128-bit atomic
+// exchange and retires; the second takes them, so it knows the parent's range, box and both outer deltas
+// without a single key load or search, writes the parent's 16-byte node and walks on ("walking up the
+// tree from the leaf nodes").  Slots are tagged with a per-build number instead of being cleared every build.
+// Numbering (pinned in tests/test_oracle_tree.py): a left child [f,gamma] is internal node gamma, a
+// right child [gamma+1,l] is internal node gamma+1, a root is the first position of its segment; leaf k is node
+// N-1+k.  Rope of a node covering [f,l]: END if l is the segment end, else with m = l+1:
+// internal node m if its range starts at m (delta(m,m+1) > delta(m,m-1)), else leaf m.
+//
+// Boxes (a5 + a6).  Quantizer defined by its decompressor:
 //   D_lo(q) = fma_rd(q, Delta, lo)   D_hi(q) = fma_ru(q, Delta, lo)
 //   q_lo(a) = max{q : D_lo(q) <= a}  q_hi(b) = min{q : D_hi(q) >= b}     (bisection: D_lo, D_hi are monotone)
 // q_lo/q_hi are monotone, so the union of boxes is the per-field integer min/max of the packed words.
@@ -485,37 +389,136 @@ __device__ __forceinline__ uint32_t pack_max(uint32_t a, uint32_t b) {
     return max(a & 0x3FFu, b & 0x3FFu) | max(a & 0xFFC00u, b & 0xFFC00u) | max(a & 0x3FF00000u, b & 0x3FF00000u);
 }
 
-__global__ void __launch_bounds__(256) fit_kernel(const float *__restrict__ pos, const uint32_t *__restrict__ idx_sorted,
-                                                   const uint32_t *__restrict__ key_sorted, int N,
-                                                   const TreeMeta *__restrict__ meta, float4 *__restrict__ sorted_pos,
-                                                   int4 *__restrict__ nodes, const int32_t *__restrict__ parent,
-                                                   unsigned long long *__restrict__ slot) {
+// 128-bit atomic exchange (sm_90+): returns the previous content of *addr
+__device__ __forceinline__ uint4 exch128(uint4 *addr, uint4 v) {
+    unsigned long long vlo = (unsigned long long)v.x | ((unsigned long long)v.y << 32);
+    unsigned long long vhi = (unsigned long long)v.z | ((unsigned long long)v.w << 32);
+    unsigned long long olo, ohi;
+    asm volatile(
+        "{\n .reg .b128 _v, _d;\n mov.b128 _v, {%2, %3};\n atom.global.relaxed.gpu.exch.b128 _d, [%4], _v;\n"
+        " mov.b128 {%0, %1}, _d;\n}"
+        : "=l"(olo), "=l"(ohi)
+        : "l"(vlo), "l"(vhi), "l"(addr)
+        : "memory");
+    return make_uint4((uint32_t)olo, (uint32_t)(olo >> 32), (uint32_t)ohi, (uint32_t)(ohi >> 32));
+}
+
+// common prefix length of the augmented keys (ka, a) and (kb, b)
+__device__ __forceinline__ int delta_aug(uint32_t ka, int a, uint32_t kb, int b) {
+    const uint32_t x = ka ^ kb;
+    return x ? __clz(x) : 32 + __clz((uint32_t)a ^ (uint32_t)b);
+}
+
+__global__ void __launch_bounds__(256) tree_kernel(const float *__restrict__ pos, const uint32_t *__restrict__ idx_sorted,
+                                                    const uint32_t *__restrict__ key, int N,
+                                                    TreeMeta *__restrict__ meta, float4 *__restrict__ sorted_pos,
+                                                    int4 *__restrict__ nodes, int32_t *__restrict__ parent,
+                                                    uint4 *__restrict__ slot, uint2 *__restrict__ groups,
+                                                    int32_t *__restrict__ entry, int K, uint32_t build_tag) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= N) return;
+    const uint32_t ki = key[k];
+    const int t = ki >> 30;
+    const int s = meta->seg[t], e = meta->seg[t + 1] - 1;
+    const float *fr = meta->frames[t];
+    // ---- a2': gather into Z-order ----
     const uint32_t idx = idx_sorted[k];
     const float x = pos[3 * (size_t)idx], y = pos[3 * (size_t)idx + 1], z = pos[3 * (size_t)idx + 2];
     sorted_pos[k] = make_float4(x, y, z, __uint_as_float(idx));
-    const float *fr = meta->frames[key_sorted[k] >> 30];
+    // ---- the leaf: outer deltas, rope, one-bin box ----
+    int dL = (k > s) ? delta_aug(ki, k, __ldg(key + k - 1), k - 1) : -1;
+    int dR = -1, rope = -1;
+    if (k < e) {
+        const uint32_t k1 = __ldg(key + k + 1);
+        dR = delta_aug(ki, k, k1, k + 1);
+        const int m = k + 1;
+        rope = (m <= e - 1 && delta_aug(k1, m, __ldg(key + m + 1), m + 1) > dR) ? m : N - 1 + m;
+    }
     uint32_t wlo = quant_lo(x, fr[0], fr[6]) | (quant_lo(y, fr[1], fr[7]) << 10) | (quant_lo(z, fr[2], fr[8]) << 20);
     uint32_t whi = quant_hi(x, fr[0], fr[6]) | (quant_hi(y, fr[1], fr[7]) << 10) | (quant_hi(z, fr[2], fr[8]) << 20);
-    int2 *nodes_b = reinterpret_cast<int2 *>(nodes);    // {lo, hi} = first half of the 16-byte node
-    nodes_b[2 * (size_t)(N - 1 + k)] = make_int2((int)wlo, (int)whi);
-    int n = parent[N - 1 + k];
-    while (n >= 0) {
-        // hand-over through one 64-bit atomic: the first child to arrive deposits its box, the second merges
-        const unsigned long long mine = (unsigned long long)wlo | ((unsigned long long)whi << 32);
-        const unsigned long long other = atomicExch(slot + n, mine);
-        if (other == SLOT_EMPTY) break;                 // a packed box never has bits 30, 31, 62, 63 set
-        wlo = pack_min(wlo, (uint32_t)other);
-        whi = pack_max(whi, (uint32_t)(other >> 32));
-        nodes_b[2 * (size_t)n] = make_int2((int)wlo, (int)whi);
-        n = parent[n];
+    nodes[N - 1 + k] = make_int4((int)wlo, (int)whi, ~k, rope);
+    if (k == e && k < N - 1) {                       // no internal node carries the index of a segment end
+        nodes[k] = make_int4(0, 0, 0, -1);
+        parent[k] = -1;
+    }
+    // Entry table of the traversal.  The upper levels of an LBVH over Morton codes ARE a regular grid: all
+    // particles whose code starts with a given 3l-bit prefix (one cell of the 2^l-per-axis grid over the box,
+    // PAPER.md:61) form one subtree.  A node whose keys share `dnode` leading bits while its parent's share
+    // only `dpar` roots the cell of every level l with dpar < 2 + 3 l <= dnode (2 type bits, then the code).
+    int32_t *const etab = entry + t * ENTRY_CELLS;
+    auto emit_entry = [&](int dpar, int dnode, int node) {
+#pragma unroll
+        for (int l = ENTRY_LMIN; l <= ENTRY_LMAX; ++l) {
+            const int need = 2 + 3 * l;
+            if (dpar < need && need <= dnode) etab[entry_offset(l) + (int)((ki & 0x3FFFFFFFu) >> (30 - 3 * l))] = node;
+        }
+    };
+    // query groups (maximal subtrees with <= GROUP_MAX leaves): appended with one atomic per converged set of lanes
+    auto emit_groups = [&](uint2 g0, uint2 g1, int n) {
+        const uint32_t act = __activemask();
+        const uint32_t two = __ballot_sync(act, n >= 2);
+        const int lane = threadIdx.x & 31;
+        const uint32_t lt = (1u << lane) - 1u;
+        const int leader = __ffs(act) - 1;
+        int base = 0;
+        if (lane == leader) base = atomicAdd(&meta->group_count, __popc(act) + __popc(two));
+        base = __shfl_sync(act, base, leader) + __popc(act & lt) + __popc(two & lt);
+        groups[base] = g0;
+        if (n >= 2) groups[base + 1] = g1;
+    };
+    emit_entry(max(dL, dR), 64, N - 1 + k);
+
+    // ---- walk up ----
+    int f = k, l = k, cur = N - 1 + k;
+    while (true) {
+        if (dL < 0 && dR < 0) {                      // the root of this type's tree
+            parent[cur] = -1;
+            if (l - f + 1 <= GROUP_MAX) emit_groups(make_uint2((uint32_t)f, (uint32_t)(l - f + 1)), make_uint2(0u, 0u), 1);
+            break;
+        }
+        const bool is_left = dR > dL;
+        const int gamma = is_left ? l : f - 1;
+        const uint4 mine = make_uint4(wlo, whi, (uint32_t)(is_left ? f : l), (build_tag << 8) | (uint32_t)((is_left ? dL : dR) + 1));
+        const uint4 other = exch128(slot + gamma, mine);
+        if ((other.w >> 8) != build_tag) break;      // first to arrive: the sibling will carry on
+        const int dsplit = is_left ? dR : dL;        // delta(gamma, gamma+1): the parent's own prefix length
+        if (is_left) {
+            l = (int)other.z;
+            dR = (int)(other.w & 255u) - 1;
+        } else {
+            f = (int)other.z;
+            dL = (int)(other.w & 255u) - 1;
+        }
+        wlo = pack_min(wlo, other.x);
+        whi = pack_max(whi, other.y);
+        const int lsize = gamma - f + 1, rsize = l - gamma, size = l - f + 1;
+        const int lc = (lsize == 1) ? (N - 1 + gamma) : gamma;
+        const int rc = (rsize == 1) ? (N + gamma) : (gamma + 1);
+        const int id = (dL < 0 && dR < 0) ? s : (dR > dL ? l : f);
+        parent[lc] = id;
+        parent[rc] = id;
+        int nrope = -1;
+        if (l < e) {
+            const int m = l + 1;
+            nrope = (m <= e - 1 && delta_aug(__ldg(key + m), m, __ldg(key + m + 1), m + 1) > dR) ? m : N - 1 + m;
+        }
+        const int leftword = (K > 1 && size <= K) ? ~f : lc;      // collapsed range leaf: first sorted position
+        nodes[id] = make_int4((int)wlo, (int)whi, leftword, nrope);
+        emit_entry(max(dL, dR), dsplit, id);
+        if (size > GROUP_MAX) {                      // children that fit are maximal: they become groups
+            const int nl = lsize <= GROUP_MAX, nr = rsize <= GROUP_MAX;
+            if (nl + nr) {
+                const uint2 gl = make_uint2((uint32_t)f, (uint32_t)lsize), gr = make_uint2((uint32_t)(gamma + 1), (uint32_t)rsize);
+                emit_groups(nl ? gl : gr, gr, nl + nr);
+            }
+        }
+        cur = id;
     }
 }
 
 // ------------------------------------------------------------------------------------------------------------
 cudaError_t launch_build(const float *pos, const int32_t *type, int N, int T, int K, const float *box_lo,
-                         const float *box_scale, const BuildBuffers &b, cudaStream_t st) {
+                         const float *box_scale, const BuildBuffers &b, uint32_t build_tag, cudaStream_t st) {
     cudaError_t err = cudaMemsetAsync(b.meta, 0, sizeof(TreeMeta), st);
     if (err != cudaSuccess) return err;
     if (N == 0) {
@@ -546,7 +549,7 @@ cudaError_t launch_build(const float *pos, const int32_t *type, int N, int T, in
     onesweep_kernel<false><<<tiles, SORT_THREADS, 0, st>>>(b.key_b, b.idx_b, b.key_a, b.idx_a, N, 24, b.meta->hist[3],
                                                            b.status[1], b.status[0], &b.meta->tile_counter[3]);
     const int nb = (N + 255) / 256;
-    hierarchy_kernel<<<nb, 256, 0, st>>>(b.key_a, N, b.meta, b.nodes, b.parent, b.slot, b.groups, b.entry, K);
-    fit_kernel<<<nb, 256, 0, st>>>(pos, b.idx_a, b.key_a, N, b.meta, b.sorted_pos, b.nodes, b.parent, b.slot);
+    tree_kernel<<<nb, 256, 0, st>>>(pos, b.idx_a, b.key_a, N, b.meta, b.sorted_pos, b.nodes, b.parent, b.slot, b.groups,
+                                    b.entry, K, build_tag);
     return cudaGetLastError();
 }

@@ -36,7 +36,6 @@ __device__ inline float ord2f(uint32_t o) {
     return __uint_as_float(b);
 }
 
-#define SLOT_EMPTY 0xFFFFFFFFFFFFFFFFull
 
 // ---- sort geometry ----
 constexpr int SORT_THREADS = 512;
@@ -79,11 +78,11 @@ struct BuildBuffers {
     float4 *sorted_pos;
     int4 *nodes;
     int32_t *parent;
-    unsigned long long *slot;
+    uint4 *slot;                   // meeting slot of the two children of the node that splits at gamma (tree_kernel)
     uint2 *groups;                 // {first sorted position, number of particles}, group_count entries, any order
     int32_t *entry;                // [QBVH_TMAX][ENTRY_CELLS] entry table
 };
 cudaError_t launch_build(const float *pos, const int32_t *type, int N, int T, int K, const float *box_lo,
-                         const float *box_scale, const BuildBuffers &b, cudaStream_t st);
+                         const float *box_scale, const BuildBuffers &b, uint32_t build_tag, cudaStream_t st);
 cudaError_t launch_traverse(const TraverseParams &p, const BuildBuffers &b, int32_t *nlist, int32_t *n_neigh,
                             bool stats, int variant, cudaStream_t st);
