@@ -1,14 +1,14 @@
 // build_kernels.cu — steps a1..a6 of the hot path, hand-written for sm_100a.
 //   a1  morton_hist_kernel : Morton keys in the periodic box + digit histograms of all four
-//                            radix passes + per-type root AABB (the quantization frame)
-//       finalize_kernel    : exclusive scans of the histograms, type segments, roots, frames
+//                            radix passes + per-type root AABB (the quantization frame); its last
+//                            block scans the histograms and writes type segments, roots and frames
 //   a2  onesweep_kernel    : stable LSD radix sort, 8-bit digits, one kernel per pass with chained-scan
 //                            decoupled look-back between tiles (the paper used CUB)
-//   a3+a4 hierarchy_kernel : Karras binary radix tree + ropes in closed form
-//       entry_table_kernel : node of every cell of the 4^3 .. 32^3 Morton grids (entry points of the traversal)
-//   a2'+a5+a6 fit_kernel   : gather into Z-order, quantize each leaf onto the 1023-bin grid of its tree's root
-//                            box with outward rounding, then bottom-up union with atomic
-//                            hand-over directly on the packed 10-bit integers
+//   a2'+a3+a4+a5+a6 tree_kernel : gather into Z-order; Karras binary radix tree built bottom up
+//                            with ropes in closed form; each leaf quantized onto the 1023-bin
+//                            grid of its tree's root box with outward rounding; boxes united
+//                            on the packed 10-bit integers while walking up with one 128-bit atomic hand-over
+//                            per node; entry table and query groups of the traversal
 #include "qbvh_internal.cuh"
 
 // ------------------------------------------------------------------------------------------------------------
@@ -102,7 +102,7 @@ __global__ void __launch_bounds__(MORTON_THREADS) morton_hist_kernel(const float
     const int stride = gridDim.x * blockDim.x;
     const int gtid = blockIdx.x * blockDim.x + threadIdx.x;
     // the look-back status buffer of the first sort pass must be zero before that pass starts; the entry table of
-    // the traversal starts out empty (-1) and is filled by hierarchy_kernel
+    // the traversal starts out empty (-1) and is filled by tree_kernel
     for (int i = gtid; i < status_words; i += stride) status0[i] = 0;
     for (int i = gtid; i < entry_words; i += stride) entry[i] = -1;
 

@@ -8,14 +8,14 @@
 
 // Device-resident bookkeeping of one build (lives at the start of the workspace; zeroed by a memset per build).
 struct TreeMeta {
-    uint32_t hist[4][256];     // per-pass digit histograms, turned into exclusive offsets by finalize_kernel
+    uint32_t hist[4][256];     // per-pass digit histograms, turned into exclusive offsets by the last block of morton_hist_kernel
     uint32_t tile_counter[4];  // dynamic tile ids of the four onesweep passes
     uint32_t blocks_done;      // blocks of morton_hist_kernel that have added their histograms (the last one finalizes)
     uint32_t mm_enc[QBVH_TMAX][6];  // per type: ~enc(min xyz) (so atomicMax computes the min), enc(max xyz)
     int32_t seg[QBVH_TMAX + 1];     // first sorted position of each type; seg[T..4] = N
     int32_t roots[QBVH_TMAX];       // root node per type, -1 if empty
     float frames[QBVH_TMAX][12];    // lo xyz, hi xyz, delta xyz, 0 0 0
-    int32_t group_count;            // number of query groups emitted by the build (hierarchy_kernel)
+    int32_t group_count;            // number of query groups emitted by the build (tree_kernel)
     int32_t group_cursor;           // next group to hand out (dynamic scheduling of the traversal); reset per traversal
     int32_t max_count;              // max_i n_neigh[i] of the last traversal
     int32_t err_flags;              // bit 0: type id out of range
