@@ -81,6 +81,22 @@ class ClockSampler(threading.Thread):
         return {"sm_mhz": med, "sm_max_mhz": self.sm_max, "reasons": sorted(self.reasons), "samples": len(self.samples)}
 
 
+def max_over_ranks(value: float, world: int, device=None) -> float:
+    """Timing of a multi-rank run = the slowest rank (replicas: no other exchange on the path)."""
+    if world <= 1:
+        return float(value)
+    import torch
+    import torch.distributed as dist
+    tt = torch.tensor([value], device=device, dtype=torch.float64)
+    dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    return float(tt.item())
+
+
+def whole_job_value(ms_per_step: float, n_per_rank: int, world: int) -> float:
+    """ns per particle of the whole job: all ranks' particles over the slowest rank's time."""
+    return 1e6 * ms_per_step / (n_per_rank * world)
+
+
 def reference_sample(cid: int):
     """Bounded sample of the workload for the oracle arm: same recipe, density, cutoff; fewer particles."""
     from paper_1901_08088_b200 import workloads as W
@@ -183,13 +199,9 @@ def run_gpu(args):
         dist.barrier()
     t_build = np.array([e[0].elapsed_time(e[1]) for e in ev])
     t_trav = np.array([e[1].elapsed_time(e[2]) for e in ev])
-    total_ms = float((t_build + t_trav).sum())
-    if world > 1:
-        tt = torch.tensor([total_ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        total_ms = float(tt.item())
+    total_ms = max_over_ranks(float((t_build + t_trav).sum()), world, dev)
     ms_per_step = total_ms / K
-    value = 1e6 * ms_per_step / (N * world)            # ns per particle, whole job
+    value = whole_job_value(ms_per_step, N, world)     # ns per particle, whole job
 
     # ---- statistics of the run (one instrumented pass, outside the timed region) ----
     qbvh.qbvh_set_option(qbvh.OPT_STATS, 1)
@@ -220,10 +232,7 @@ def run_gpu(args):
         e1.record()
         torch.cuda.synchronize()
         e2e_ms = e0.elapsed_time(e1) / Ke
-        if world > 1:
-            tt = torch.tensor([e2e_ms], device=dev, dtype=torch.float64)
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            e2e_ms = float(tt.item())
+        e2e_ms = max_over_ranks(e2e_ms, world, dev)
         qbvh.qbvh_set_staging(None)
     clocks = sampler.stop()
     h2d = 12 * N + (4 * N if w.type is not None else 0)
