@@ -64,12 +64,14 @@ __device__ void finalize_block(TreeMeta *__restrict__ meta, int N) {
         int s = (d < QBVH_TMAX) ? (int)s_scan[64 * d] : N;
         meta->seg[d] = s;
     }
+    __shared__ float s_rho[QBVH_TMAX];
     if (d < QBVH_TMAX) {
         int s = (int)s_scan[64 * d];
         int e1 = (d + 1 < QBVH_TMAX) ? (int)s_scan[64 * (d + 1)] : N;
         int n = e1 - s;
         meta->roots[d] = (n <= 0) ? -1 : (n == 1 ? (N - 1 + s) : s);
         float *fr = meta->frames[d];
+        float vol = 1.0f;
         if (n > 0) {
             for (int a = 0; a < 3; ++a) {
                 float lo = ord2f(~__ldcg(&meta->mm_enc[d][a]));
@@ -78,11 +80,25 @@ __device__ void finalize_block(TreeMeta *__restrict__ meta, int N) {
                 fr[3 + a] = hi;
                 // Delta = div_ru(sub_ru(hi, lo), 1023): the 1023-bin grid spans at least the root box
                 fr[6 + a] = __fdiv_ru(__fsub_ru(hi, lo), QBVH_NBINS);
+                vol *= hi - lo;
             }
         } else {
             for (int a = 0; a < 9; ++a) fr[a] = 0.0f;
         }
         fr[9] = fr[10] = fr[11] = 0.0f;
+        s_rho[d] = (n > 1 && vol > 0.0f) ? (float)n / vol : 0.0f;    // unknown (flat or single): treated as dense
+    }
+    __syncthreads();
+    // Query-group size per type.  One warp traverses for a whole group with the group's box as search volume, so
+    // the candidates it draws from a tree of number density rho_b grow with rho_b x (group size / rho_t): for a
+    // type far sparser than the densest one (the colloids of a colloid-solvent mixture) a full group
+    // would sweep up thousands of misses.  Groups of type t hold at most 32 rho_t / rho_max particles (>= 1).
+    if (d < QBVH_TMAX) {
+        const float rmax = fmaxf(fmaxf(s_rho[0], s_rho[1]), fmaxf(s_rho[2], s_rho[3]));
+        int gm = GROUP_MAX;
+        if (s_rho[d] > 0.0f && rmax > 0.0f)
+            gm = (int)fminf(fmaxf(floorf((float)GROUP_MAX * s_rho[d] / rmax), 1.0f), (float)GROUP_MAX);
+        meta->gmax[d] = gm;
     }
 }
 
@@ -453,7 +469,8 @@ __global__ void __launch_bounds__(256) tree_kernel(const float *__restrict__ pos
             if (dpar < need && need <= dnode) etab[entry_offset(l) + (int)((ki & 0x3FFFFFFFu) >> (30 - 3 * l))] = node;
         }
     };
-    // query groups (maximal subtrees with <= GROUP_MAX leaves): appended with one atomic per converged set of lanes
+    // query groups (maximal subtrees with <= gmax[type] leaves): appended with one atomic per converged set of lanes
+    const int gmax = meta->gmax[t];
     auto emit_groups = [&](uint2 g0, uint2 g1, int n) {
         const uint32_t act = __activemask();
         const uint32_t two = __ballot_sync(act, n >= 2);
@@ -473,7 +490,7 @@ __global__ void __launch_bounds__(256) tree_kernel(const float *__restrict__ pos
     while (true) {
         if (dL < 0 && dR < 0) {                      // the root of this type's tree
             parent[cur] = -1;
-            if (l - f + 1 <= GROUP_MAX) emit_groups(make_uint2((uint32_t)f, (uint32_t)(l - f + 1)), make_uint2(0u, 0u), 1);
+            if (l - f + 1 <= gmax) emit_groups(make_uint2((uint32_t)f, (uint32_t)(l - f + 1)), make_uint2(0u, 0u), 1);
             break;
         }
         const bool is_left = dR > dL;
@@ -505,8 +522,8 @@ __global__ void __launch_bounds__(256) tree_kernel(const float *__restrict__ pos
         const int leftword = (K > 1 && size <= K) ? ~f : lc;      // collapsed range leaf: first sorted position
         nodes[id] = make_int4((int)wlo, (int)whi, leftword, nrope);
         emit_entry(max(dL, dR), dsplit, id);
-        if (size > GROUP_MAX) {                      // children that fit are maximal: they become groups
-            const int nl = lsize <= GROUP_MAX, nr = rsize <= GROUP_MAX;
+        if (size > gmax) {                           // children that fit are maximal: they become groups
+            const int nl = lsize <= gmax, nr = rsize <= gmax;
             if (nl + nr) {
                 const uint2 gl = make_uint2((uint32_t)f, (uint32_t)lsize), gr = make_uint2((uint32_t)(gamma + 1), (uint32_t)rsize);
                 emit_groups(nl ? gl : gr, gr, nl + nr);

@@ -1,6 +1,7 @@
 // qbvh_internal.cuh — device-side data layout shared by the build and traversal kernels (sm_100a only).
 #pragma once
 #include <cuda_runtime.h>
+#include <stddef.h>
 #include <stdint.h>
 
 #define QBVH_TMAX 4            // types live in key bits 30-31
@@ -15,6 +16,8 @@ struct TreeMeta {
     int32_t seg[QBVH_TMAX + 1];     // first sorted position of each type; seg[T..4] = N
     int32_t roots[QBVH_TMAX];       // root node per type, -1 if empty
     float frames[QBVH_TMAX][12];    // lo xyz, hi xyz, delta xyz, 0 0 0
+    int32_t gmax[QBVH_TMAX];        // largest query group of each type (<= GROUP_MAX; smaller for a sparse type, see finalize)
+    int32_t pad_[38];               // the counters below, hammered by atomics, keep a 128-byte line of their own
     int32_t group_count;            // number of query groups emitted by the build (tree_kernel)
     int32_t group_cursor;           // next group to hand out (dynamic scheduling of the traversal); reset per traversal
     int32_t max_count;              // max_i n_neigh[i] of the last traversal
@@ -47,7 +50,7 @@ constexpr uint32_t ST_PRE = 1u << 31;                 // tile status: inclusive 
 constexpr uint32_t ST_VAL = (1u << 30) - 1;
 
 // ---- query groups ----
-// A query group is a maximal subtree of the LBVH with at most GROUP_MAX leaves: a contiguous run of Z-ordered
+// A query group is a maximal subtree of the LBVH with at most GROUP_MAX leaves (fewer for a sparse type, TreeMeta::gmax): a contiguous run of Z-ordered
 // particles that fills one Morton cell, i.e. a compact blob.  One warp traverses the tree once
 // for the whole group (traverse_kernels.cu).
 constexpr int GROUP_MAX = 32;
@@ -86,3 +89,4 @@ cudaError_t launch_build(const float *pos, const int32_t *type, int N, int T, in
                          const float *box_scale, const BuildBuffers &b, uint32_t build_tag, cudaStream_t st);
 cudaError_t launch_traverse(const TraverseParams &p, const BuildBuffers &b, int32_t *nlist, int32_t *n_neigh,
                             bool stats, int variant, cudaStream_t st);
+static_assert(offsetof(TreeMeta, group_count) % 128 == 0, "the atomic counters start a 128-byte line");

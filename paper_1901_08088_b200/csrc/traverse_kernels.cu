@@ -335,6 +335,7 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
         int ta = 0;
 #pragma unroll
         for (int t = 1; t < QBVH_TMAX; ++t) ta += (gfirst >= meta->seg[t]) ? 1 : 0;
+        const bool aligned = meta->gmax[ta] >= P.K;   // groups are unions of collapsed leaves (the normal case)
         // bounding box of the group (exact fp32 min / max of its members)
         float glo[3], ghi[3];
         {
@@ -413,7 +414,10 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
                 const u64 ns0 = pk2(-s0, -s0), ns1 = pk2(-s1, -s1), ns2 = pk2(-s2, -s2);
                 // the group's own particles are found by the walk only here: in its own tree, unshifted.  They are
                 // checked first, as one tile (self excluded by index), and their leaves are skipped below.
-                const bool own_tree = (tb == ta) && !shifted;
+                // (A sparse type has groups smaller than the collapsed leaves, meta->gmax < K: then a leaf may hold the
+                // group and strangers; nothing is skipped and every tile of this image excludes self by index.)
+                const bool own_image = (tb == ta) && !shifted;
+                const bool own_tree = own_image && aligned, self_all = own_image && !aligned;
                 if (own_tree) {
                     sm.tx[lane] = live ? me.x : __int_as_float(0x7FC00000);   // NaN: never accepted
                     sm.ty[lane] = me.y;
@@ -478,6 +482,8 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
                         for (int h = 0; h < 32 / CHUNK; ++h) {
                             if (shifted)
                                 check_tile<true, false, CHUNK>(sm, thead + CHUNK * h, nmx, nmy, nmz, ns0, ns1, ns2, r2, orig_i, ring_s, po);
+                            else if (self_all)
+                                check_tile<false, true, CHUNK>(sm, thead + CHUNK * h, nmx, nmy, nmz, ns0, ns1, ns2, r2, orig_i, ring_s, po);
                             else
                                 check_tile<false, false, CHUNK>(sm, thead + CHUNK * h, nmx, nmy, nmz, ns0, ns1, ns2, r2, orig_i, ring_s, po);
                             // flush as soon as another chunk could overrun a ring
