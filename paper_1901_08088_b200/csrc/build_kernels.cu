@@ -463,6 +463,7 @@ __global__ void __launch_bounds__(256) tree_kernel(const float *__restrict__ pos
     // only `dpar` roots the cell of every level l with dpar < 2 + 3 l <= dnode (2 type bits, then the code).
     int32_t *const etab = entry + t * ENTRY_CELLS;
     auto emit_entry = [&](int dpar, int dnode, int node) {
+        if (dpar >= 2 + 3 * ENTRY_LMAX || dnode < 2 + 3 * ENTRY_LMIN) return;   // below or above every grid level
 #pragma unroll
         for (int l = ENTRY_LMIN; l <= ENTRY_LMAX; ++l) {
             const int need = 2 + 3 * l;
