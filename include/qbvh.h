@@ -98,6 +98,16 @@ int qbvh_build(const float *pos, const int32_t *type, int64_t N, const float *bo
  * n_neigh[i] > max_neigh hold max_neigh true neighbors; re-allocate with capacity >= M and call again. */
 int qbvh_neighbors(const float *r_list_ij, int32_t *nlist, int32_t *n_neigh, int32_t max_neigh);
 
+/* The paper's own operating mode ("the object in the leaf node is processed as a neighbor" without a
+ * distance check, positions are not loaded; the benchmarks only count): Algorithm 1 as printed, one
+ * thread per particle in Z-order, accepting every particle whose (collapsed) leaf box overlaps the padded search
+ * sphere in some image.  With QBVH_OPT_LEAF_COLLAPSE = 1 at build time this is exactly the paper's kernel.
+ *   r_list_ij HOST    T x T fp32 as for qbvh_neighbors.
+ *   n_overlap DEVICE  N int32; for ORIGINAL particle i the number of accepted particles j != i (true neighbors plus
+ *                     the false positives of the quantized leaf boxes).
+ * Returns max_i n_overlap[i] (>= 0), or < 0. */
+int qbvh_count_overlaps(const float *r_list_ij, int32_t *n_overlap);
+
 /* ---- the same two calls with HOST buffers (end-to-end path: copies are part of the call) ------------------ */
 
 /* Bytes of DEVICE staging the *_host calls need for N particles with row capacity max_neigh. */

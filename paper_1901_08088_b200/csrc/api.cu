@@ -91,11 +91,8 @@ float padded_radius(float r, const float *box) {
     return b;
 }
 
-int neighbors_impl(const float *r_list, int32_t *nlist, int32_t *n_neigh, int32_t max_neigh) {
-    if (!g.built) return QBVH_ERR_NOT_BUILT;
-    if (!r_list || max_neigh < 0) return QBVH_ERR_INVALID_ARG;
-    if (g.N > 0 && (!n_neigh || (!nlist && max_neigh > 0))) return QBVH_ERR_INVALID_ARG;
-    TraverseParams P{};
+// r_list -> the traversal's parameter block (exact r^2, padded pruning radius, Morton binning of the build)
+int make_params(const float *r_list, TraverseParams &P) {
     for (int d = 0; d < 3; ++d) {
         P.L[d] = g.box[3 + d];
         P.box_lo[d] = g.box[d];
@@ -115,6 +112,18 @@ int neighbors_impl(const float *r_list, int32_t *nlist, int32_t *n_neigh, int32_
             P.R2[a * QBVH_TMAX + b] = mul_ru(rp, rp);
             P.Rp[a * QBVH_TMAX + b] = rp;
         }
+    P.N = (int32_t)g.N;
+    P.K = g.K_built;
+    return QBVH_OK;
+}
+
+int neighbors_impl(const float *r_list, int32_t *nlist, int32_t *n_neigh, int32_t max_neigh) {
+    if (!g.built) return QBVH_ERR_NOT_BUILT;
+    if (!r_list || max_neigh < 0) return QBVH_ERR_INVALID_ARG;
+    if (g.N > 0 && (!n_neigh || (!nlist && max_neigh > 0))) return QBVH_ERR_INVALID_ARG;
+    TraverseParams P{};
+    const int prc = make_params(r_list, P);
+    if (prc != QBVH_OK) return prc;
     P.N = (int32_t)g.N;
     P.max_neigh = max_neigh;
     P.K = g.K_built;
@@ -254,6 +263,22 @@ int qbvh_build(const float *pos, const int32_t *type, int64_t N, const float *bo
 int qbvh_neighbors(const float *r_list_ij, int32_t *nlist, int32_t *n_neigh, int32_t max_neigh) {
     int rc = neighbors_impl(r_list_ij, nlist, n_neigh, max_neigh);
     if (rc != QBVH_OK) return rc;
+    return finish_neighbors();
+}
+
+int qbvh_count_overlaps(const float *r_list_ij, int32_t *n_overlap) {
+    if (!g.built) return QBVH_ERR_NOT_BUILT;
+    if (!r_list_ij || (g.N > 0 && !n_overlap)) return QBVH_ERR_INVALID_ARG;
+    TraverseParams P{};
+    const int prc = make_params(r_list_ij, P);
+    if (prc != QBVH_OK) return prc;
+    P.max_neigh = 0;
+    cudaError_t e = cudaMemsetAsync(&g.buf.meta->group_cursor, 0, 2 * sizeof(int32_t), g.stream);
+    if (e != cudaSuccess) return cuda_fail(e, "memset max_count");
+    e = launch_count_overlaps(P, g.buf, n_overlap, g.stream);
+    if (e != cudaSuccess) return cuda_fail(e, "count launch");
+    e = cudaMemcpyAsync(g.pinned, &g.buf.meta->max_count, 2 * sizeof(int32_t), cudaMemcpyDeviceToHost, g.stream);
+    if (e != cudaSuccess) return cuda_fail(e, "copy max_count");
     return finish_neighbors();
 }
 

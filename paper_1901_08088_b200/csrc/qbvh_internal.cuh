@@ -89,4 +89,5 @@ cudaError_t launch_build(const float *pos, const int32_t *type, int N, int T, in
                          const float *box_scale, const BuildBuffers &b, uint32_t build_tag, cudaStream_t st);
 cudaError_t launch_traverse(const TraverseParams &p, const BuildBuffers &b, int32_t *nlist, int32_t *n_neigh,
                             bool stats, int variant, cudaStream_t st);
+cudaError_t launch_count_overlaps(const TraverseParams &p, const BuildBuffers &b, int32_t *n_overlap, cudaStream_t st);
 static_assert(offsetof(TreeMeta, group_count) % 128 == 0, "the atomic counters start a 128-byte line");

@@ -141,6 +141,84 @@ __global__ void __launch_bounds__(128) traverse_kernel(TraverseParams P, const i
 
 
 // ------------------------------------------------------------------------------------------------------------
+// The paper's own operating mode: Algorithm 1 with line 14 as printed — a leaf whose box
+// overlaps the search sphere is ACCEPTED, positions are never loaded, and the benchmark only counts.  One thread
+// per particle in Z-order.  n_overlap[orig_i] = particles j != i accepted (a collapsed leaf accepts its whole
+// range; the particle's own leaf always overlaps and is not counted).
+// ------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128) count_overlaps_kernel(TraverseParams P, const int4 *__restrict__ nodes,
+                                                              const float4 *__restrict__ sorted_pos,
+                                                              TreeMeta *__restrict__ meta, int32_t *__restrict__ n_overlap) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    int cnt = 0;
+    if (k < P.N) {
+        const float4 me = sorted_pos[k];
+        int ta = 0;
+#pragma unroll
+        for (int t = 1; t < QBVH_TMAX; ++t) ta += (k >= meta->seg[t]) ? 1 : 0;
+        for (int tb = 0; tb < QBVH_TMAX; ++tb) {
+            const int root = meta->roots[tb];
+            if (!(P.r2[ta * QBVH_TMAX + tb] >= 0.0f) || root < 0) continue;
+            const float R2 = P.R2[ta * QBVH_TMAX + tb];
+            const float *fr = meta->frames[tb];
+            const float flo[3] = {fr[0], fr[1], fr[2]};
+            const float fdl[3] = {fr[6], fr[7], fr[8]};
+            const int seg_end = meta->seg[tb + 1];
+            const float xme[3] = {me.x, me.y, me.z};
+            uint32_t bset = 0;                                   // line 4
+            {
+                const int4 nd = __ldg(nodes + root);
+                float a[3], b[3];
+                decompress((uint32_t)nd.x, (uint32_t)nd.y, flo, fdl, a, b);
+                float tq[3][3];
+#pragma unroll
+                for (int d = 0; d < 3; ++d)
+#pragma unroll
+                    for (int s = -1; s <= 1; ++s) {
+                        const float xs = __fadd_rn(xme[d], (float)s * P.L[d]);
+                        tq[d][s + 1] = __fsub_rn(fminf(fmaxf(xs, a[d]), b[d]), xs);
+                    }
+#pragma unroll
+                for (int img = 0; img < 27; ++img) {
+                    const float tx = tq[0][img % 3], ty = tq[1][(img / 3) % 3], tz = tq[2][img / 9];
+                    if (__fmaf_rn(tz, tz, __fmaf_rn(ty, ty, __fmul_rn(tx, tx))) <= R2) bset |= 1u << img;
+                }
+            }
+            while (bset) {                                       // lines 5-19
+                const int img = __ffs(bset) - 1;
+                bset &= bset - 1;
+                const float xs[3] = {__fadd_rn(me.x, (float)(img % 3 - 1) * P.L[0]), __fadd_rn(me.y, (float)((img / 3) % 3 - 1) * P.L[1]),
+                                     __fadd_rn(me.z, (float)(img / 9 - 1) * P.L[2])};
+                int n = root;
+                while (n >= 0) {
+                    const int4 nd = __ldg(nodes + n);
+                    float a[3], b[3];
+                    decompress((uint32_t)nd.x, (uint32_t)nd.y, flo, fdl, a, b);
+                    float tq[3];
+#pragma unroll
+                    for (int d = 0; d < 3; ++d) tq[d] = __fsub_rn(fminf(fmaxf(xs[d], a[d]), b[d]), xs[d]);
+                    const bool hit = __fmaf_rn(tq[2], tq[2], __fmaf_rn(tq[1], tq[1], __fmul_rn(tq[0], tq[0]))) <= R2;
+                    if (hit && nd.z < 0) {                       // line 14: accept the leaf's particles, self excepted
+                        const int first = ~nd.z, m = leaf_count(nd, P.N, seg_end);
+                        cnt += m - ((img == 13 && (unsigned)(k - first) < (unsigned)m) ? 1 : 0);
+                    }
+                    n = (hit && nd.z >= 0) ? nd.z : nd.w;
+                }
+            }
+        }
+        n_overlap[__float_as_int(me.w)] = cnt;
+    }
+    const int wmax = __reduce_max_sync(0xFFFFFFFFu, cnt);
+    if ((threadIdx.x & 31) == 0 && wmax > 0) atomicMax(&meta->max_count, wmax);
+}
+
+cudaError_t launch_count_overlaps(const TraverseParams &p, const BuildBuffers &b, int32_t *n_overlap, cudaStream_t st) {
+    if (p.N == 0) return cudaSuccess;
+    count_overlaps_kernel<<<(p.N + 127) / 128, 128, 0, st>>>(p, b.nodes, b.sorted_pos, b.meta, n_overlap);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------------------
 // Group traversal (the production kernel).
 //
 // Algorithm 1 is written for one thread per particle; the paper runs those threads in Z-order so that "threads

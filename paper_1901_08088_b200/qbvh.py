@@ -22,7 +22,7 @@ EXPORT_KEYS_SORTED, EXPORT_PERM, EXPORT_NODES, EXPORT_PARENT, EXPORT_FRAMES, EXP
 
 # every symbol include/qbvh.h declares
 SYMBOLS = ("qbvh_set_stream", "qbvh_set_num_types", "qbvh_workspace_bytes", "qbvh_set_workspace",
-           "qbvh_set_option", "qbvh_get_option", "qbvh_build", "qbvh_neighbors", "qbvh_staging_bytes",
+           "qbvh_set_option", "qbvh_get_option", "qbvh_build", "qbvh_neighbors", "qbvh_count_overlaps", "qbvh_staging_bytes",
            "qbvh_set_staging", "qbvh_build_host", "qbvh_neighbors_host", "qbvh_get_stats", "qbvh_debug_export",
            "qbvh_error_string")
 
@@ -54,6 +54,7 @@ _lib.qbvh_set_option.argtypes = [_i32, _i32]
 _lib.qbvh_get_option.argtypes = [_i32]
 _lib.qbvh_build.argtypes = [_vp, _vp, _i64, _vp]
 _lib.qbvh_neighbors.argtypes = [_vp, _vp, _vp, _i32]
+_lib.qbvh_count_overlaps.argtypes = [_vp, _vp]
 _lib.qbvh_staging_bytes.argtypes = [_i64, _i32]
 _lib.qbvh_staging_bytes.restype = _i64
 _lib.qbvh_set_staging.argtypes = [_vp, _i64]
@@ -131,6 +132,12 @@ def qbvh_neighbors(r_list_ij, nlist, n_neigh, max_neigh: int, T: int | None = No
     """r_list_ij: host T x T; nlist, n_neigh: DEVICE int32 tensors.  Returns M = max n_neigh (overflow iff M > max_neigh)."""
     r = np.ascontiguousarray(r_list_ij, dtype=np.float32)
     return _check(_lib.qbvh_neighbors(r.ctypes.data, _ptr(nlist), _ptr(n_neigh), max_neigh), "qbvh_neighbors")
+
+
+def qbvh_count_overlaps(r_list_ij, n_overlap) -> int:
+    """The paper's accept-on-leaf-overlap count.  n_overlap: DEVICE int32 tensor of N."""
+    r = np.ascontiguousarray(r_list_ij, dtype=np.float32)
+    return _check(_lib.qbvh_count_overlaps(r.ctypes.data, _ptr(n_overlap)), "qbvh_count_overlaps")
 
 
 def qbvh_staging_bytes(N: int, max_neigh: int) -> int:

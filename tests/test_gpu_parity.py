@@ -242,3 +242,31 @@ def test_host_buffer_api_matches_device_api():
     out = {"M": M, "max_neigh": w.max_neigh, "nlist": nlist.numpy(), "n_neigh": n_neigh.numpy()}
     compare_with_oracle(w, out, ON.neighbor_list(w.pos, w.type, w.box, w.r_list))
     qbvh.qbvh_set_staging(None)
+
+
+@pytest.mark.parametrize("cid", [1, 3, 5])
+def test_count_overlaps_is_the_papers_kernel(cid):
+    """qbvh_count_overlaps = Algorithm 1 as printed (accept on leaf-box overlap) on the paper's
+    one-particle-per-leaf tree: per particle the oracle replay's count, minus the particle's own leaf."""
+    import torch
+    from paper_1901_08088_b200 import qbvh
+    w = W.make_config(cid, small=True)
+    dev = torch.device("cuda:0")
+    qbvh.qbvh_set_option(qbvh.OPT_LEAF_COLLAPSE, 1)
+    qbvh.qbvh_set_option(qbvh.OPT_STATS, 0)
+    nl = qbvh.NeighborList(w.N, T=w.T, max_neigh=w.max_neigh, device=dev)   # owns the workspace: keep it alive
+    nl.build(torch.from_numpy(w.pos).to(dev), None if w.type is None else torch.from_numpy(w.type).to(dev), w.box)
+    t = OT.build(w.pos, w.type, w.box, T=w.T)
+    tr = OT.traverse(t, w.box, w.r_list)
+    cnt = torch.full((w.N,), -7, dtype=torch.int32, device=dev)
+    M = qbvh.qbvh_count_overlaps(w.r_list, cnt)
+    got = cnt.cpu().numpy()
+    r = np.asarray(w.r_list, np.float32).reshape(w.T, w.T)
+    ta = np.searchsorted(t.seg[1:], np.arange(w.N), side="right")        # type of sorted position k
+    own = (r[ta, ta] > 0).astype(np.int64)                                # own leaf overlaps iff its own tree is walked
+    expect = tr["n_overlap"].astype(np.int64) - own
+    assert np.array_equal(got[t.perm], expect)
+    assert M == int(expect.max())
+    # and it brackets the exact list: every true neighbor's leaf box overlaps (PAPER.md:85, 196)
+    nl.neighbors(w.r_list)
+    assert np.all(got >= nl.n_neigh.cpu().numpy()[: w.N])
