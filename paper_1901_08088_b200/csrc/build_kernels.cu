@@ -33,7 +33,7 @@ __device__ __forceinline__ uint32_t morton_bin(float p, float lo, float s) {
 
 // One block of MORTON_THREADS threads: histograms -> exclusive offsets; segments, roots, frames.  Run by the last
 // block of morton_hist_kernel to finish (threads 0..255 own one digit each).
-__device__ void finalize_block(TreeMeta *__restrict__ meta, int N) {
+__device__ void finalize_block(TreeMeta *__restrict__ meta, int N, int warp_slots) {
     __shared__ uint32_t s_scan[256];
     __shared__ uint32_t s_ws[8];
     const int d = threadIdx.x, lane = d & 31, warp = d >> 5;
@@ -65,6 +65,7 @@ __device__ void finalize_block(TreeMeta *__restrict__ meta, int N) {
         meta->seg[d] = s;
     }
     __shared__ float s_rho[QBVH_TMAX];
+    __shared__ uint32_t s_scan_count[QBVH_TMAX];
     if (d < QBVH_TMAX) {
         int s = (int)s_scan[64 * d];
         int e1 = (d + 1 < QBVH_TMAX) ? (int)s_scan[64 * (d + 1)] : N;
@@ -87,6 +88,7 @@ __device__ void finalize_block(TreeMeta *__restrict__ meta, int N) {
         }
         fr[9] = fr[10] = fr[11] = 0.0f;
         s_rho[d] = (n > 1 && vol > 0.0f) ? (float)n / vol : 0.0f;    // unknown (flat or single): treated as dense
+        s_scan_count[d] = n > 0 ? (uint32_t)n : 0u;
     }
     __syncthreads();
     // Query-group size per type.  One warp traverses for a whole group with the group's box as search volume, so
@@ -98,6 +100,10 @@ __device__ void finalize_block(TreeMeta *__restrict__ meta, int N) {
         int gm = GROUP_MAX;
         if (s_rho[d] > 0.0f && rmax > 0.0f)
             gm = (int)fminf(fmaxf(floorf((float)GROUP_MAX * s_rho[d] / rmax), 1.0f), (float)GROUP_MAX);
+        // Small systems (the regime of PAPER.md:186): with fewer groups than the device has resident warps the
+        // traversal is one group's latency, so groups shrink (down to 4) until there is about one per warp.
+        const int nt = (int)s_scan_count[d];
+        gm = min(gm, max(4, nt / max(warp_slots, 1)));
         meta->gmax[d] = gm;
     }
 }
@@ -110,7 +116,8 @@ __global__ void __launch_bounds__(MORTON_THREADS) morton_hist_kernel(const float
                                                            float3 scale, uint32_t *__restrict__ key_out,
                                                            TreeMeta *__restrict__ meta,
                                                            uint32_t *__restrict__ status0, int status_words,
-                                                           int32_t *__restrict__ entry, int entry_words) {
+                                                           int32_t *__restrict__ entry, int entry_words,
+                                                           int warp_slots) {
     __shared__ uint32_t s_hist[4][256];
     __shared__ bool s_last;
     for (int i = threadIdx.x; i < 1024; i += blockDim.x) (&s_hist[0][0])[i] = 0;
@@ -212,12 +219,12 @@ __global__ void __launch_bounds__(MORTON_THREADS) morton_hist_kernel(const float
         __threadfence();
     }
     __syncthreads();
-    if (s_last) finalize_block(meta, N);
+    if (s_last) finalize_block(meta, N, warp_slots);
 }
 
 // N = 0: only the bookkeeping
 __global__ void __launch_bounds__(MORTON_THREADS) finalize_kernel(TreeMeta *__restrict__ meta, int N) {
-    finalize_block(meta, N);
+    finalize_block(meta, N, 1);
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -546,16 +553,23 @@ cudaError_t launch_build(const float *pos, const int32_t *type, int N, int T, in
     const int tiles = (N + SORT_TILE - 1) / SORT_TILE;
     const int status_words = tiles * 256;
     const int entry_words = QBVH_TMAX * ENTRY_CELLS;
+    static int warp_slots = 0;                     // warps the traversal keeps resident on this device
+    if (warp_slots == 0) {
+        int dev = 0, sms = 148;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        warp_slots = sms * 28;
+    }
     const float3 lo = make_float3(box_lo[0], box_lo[1], box_lo[2]);
     const float3 sc = make_float3(box_scale[0], box_scale[1], box_scale[2]);
     int mblocks = (N / 4 + MORTON_THREADS - 1) / MORTON_THREADS;
     if (mblocks > 148 * 2) mblocks = 148 * 2;
     if (mblocks < 1) mblocks = 1;
     switch (T) {
-        case 1: morton_hist_kernel<1><<<mblocks, MORTON_THREADS, 0, st>>>(pos, type, N, lo, sc, b.key_a, b.meta, b.status[0], status_words, b.entry, entry_words); break;
-        case 2: morton_hist_kernel<2><<<mblocks, MORTON_THREADS, 0, st>>>(pos, type, N, lo, sc, b.key_a, b.meta, b.status[0], status_words, b.entry, entry_words); break;
-        case 3: morton_hist_kernel<3><<<mblocks, MORTON_THREADS, 0, st>>>(pos, type, N, lo, sc, b.key_a, b.meta, b.status[0], status_words, b.entry, entry_words); break;
-        default: morton_hist_kernel<4><<<mblocks, MORTON_THREADS, 0, st>>>(pos, type, N, lo, sc, b.key_a, b.meta, b.status[0], status_words, b.entry, entry_words); break;
+        case 1: morton_hist_kernel<1><<<mblocks, MORTON_THREADS, 0, st>>>(pos, type, N, lo, sc, b.key_a, b.meta, b.status[0], status_words, b.entry, entry_words, warp_slots); break;
+        case 2: morton_hist_kernel<2><<<mblocks, MORTON_THREADS, 0, st>>>(pos, type, N, lo, sc, b.key_a, b.meta, b.status[0], status_words, b.entry, entry_words, warp_slots); break;
+        case 3: morton_hist_kernel<3><<<mblocks, MORTON_THREADS, 0, st>>>(pos, type, N, lo, sc, b.key_a, b.meta, b.status[0], status_words, b.entry, entry_words, warp_slots); break;
+        default: morton_hist_kernel<4><<<mblocks, MORTON_THREADS, 0, st>>>(pos, type, N, lo, sc, b.key_a, b.meta, b.status[0], status_words, b.entry, entry_words, warp_slots); break;
     }
     // four passes a -> b -> a -> b -> a
     onesweep_kernel<true><<<tiles, SORT_THREADS, 0, st>>>(b.key_a, nullptr, b.key_b, b.idx_b, N, 0, b.meta->hist[0],
