@@ -326,6 +326,13 @@ __device__ __forceinline__ void check_tile(const GwShared &sm, int base, u64 nmx
     }
 }
 
+// eight entries with one 256-bit store (sm_100: STG.256); p is 32-byte aligned
+__device__ __forceinline__ void st_global_256(int32_t *p, const int4 a, const int4 b) {
+    asm volatile("st.global.v8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"l"(p), "r"(a.x), "r"(a.y), "r"(a.z), "r"(a.w),
+                 "r"(b.x), "r"(b.y), "r"(b.z), "r"(b.w)
+                 : "memory");
+}
+
 // four staged entries -> row[off .. off+3], never past the row capacity
 __device__ __forceinline__ void store4(int32_t *__restrict__ row, int off, int cap, bool vec_ok, const int4 v) {
     if (vec_ok && off + 4 <= cap) {
@@ -393,6 +400,7 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
     const uint32_t rot = (uint32_t)(lane & 7) << 4;
     const int ngroups = meta->group_count;
     const bool vec_ok = ((P.max_neigh & 3) == 0) && ((reinterpret_cast<uintptr_t>(nlist) & 15) == 0);
+    const bool vec256_ok = ((P.max_neigh & 7) == 0) && ((reinterpret_cast<uintptr_t>(nlist) & 31) == 0);
     const int cap = P.max_neigh;
     constexpr int NL = 32 / WS;                 // leaves per gather batch
     constexpr int CHUNK = GW_RING >= 64 ? 32 : 16;   // candidates checked between two looks at the ring fill
@@ -441,7 +449,10 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
                     for (int j = 0; j < 4; ++j)
                         v[j] = *static_cast<const int4 *>(
                             __cvta_shared_to_generic((size_t)(ring_s | ((off + 16u * j) & (GW_RING_BYTES - 16)))));
-                    if (vec_ok && flushed + 16 <= cap) {          // the common case: four aligned 128-bit stores
+                    if (vec256_ok && flushed + 16 <= cap) {       // the common case: two aligned 256-bit stores (sm_100)
+                        st_global_256(row + flushed, v[0], v[1]);
+                        st_global_256(row + flushed + 8, v[2], v[3]);
+                    } else if (vec_ok && flushed + 16 <= cap) {   // four aligned 128-bit stores
                         int4 *dst = reinterpret_cast<int4 *>(row + flushed);
 #pragma unroll
                         for (int j = 0; j < 4; ++j) dst[j] = v[j];
