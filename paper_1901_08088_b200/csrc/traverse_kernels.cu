@@ -268,6 +268,10 @@ __device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c) {
 #ifndef QBVH_GW_WARPS
 #define QBVH_GW_WARPS 4
 #endif
+#ifndef QBVH_GW_NB
+#define QBVH_GW_NB 3         // leaf batches gathered per step: a tile ring of 128 takes 31 + 3 x 32 candidates
+#endif
+constexpr int GW_NB = QBVH_GW_NB;
 #ifndef QBVH_GW_RING
 #define QBVH_GW_RING 32
 #endif
@@ -584,7 +588,7 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
                         tcount -= 32;
                         continue;
                     }
-                    if (wsz > 0 && lqn <= GW_LQ - 64) {
+                    if (wsz > 0 && lqn <= GW_LQ - 64) {   // (room for the 64 leaves a step can emit)
                         // ---- lines 10-19, up to 64 nodes per step: every lane pops one entry and tests that node
                         //      and, for a left child, its rope (= right sibling) as well ----
                         const int npop = (wsz > GW_WL - 96) ? 1 : min(wsz, 32);
@@ -632,37 +636,39 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
                         continue;
                     }
                     if (lqn > 0) {
-                        // ---- gather up to 2 x 32/WS leaves: lane j takes particle j % WS of leaf j / WS of each batch (a
-                        //      collapsed leaf has at most K <= WS particles); keep those within reach of the group box ----
-                        const int take = min(lqn, 2 * NL);
-                        uint2 lfA = make_uint2(0u, 0u), lfB = make_uint2(0u, 0u);
-                        if (li < take) lfA = sm.lq[lqn - 1 - li];
-                        if (NL + li < take) lfB = sm.lq[lqn - 1 - NL - li];
+                        // ---- gather up to GW_NB x 32/WS leaves: lane j takes particle j % WS of leaf j / WS of each batch (a
+                        //      collapsed leaf has at most K <= WS particles); keep those within reach of the group box.
+                        //      All position loads of the step are issued before the first is used ----
+                        const int take = min(lqn, GW_NB * NL);
+                        uint2 lf[GW_NB];
+                        float4 pc[GW_NB];
+                        bool keep[GW_NB];
+#pragma unroll
+                        for (int u = 0; u < GW_NB; ++u) {
+                            lf[u] = make_uint2(0u, 0u);
+                            if (u * NL + li < take) lf[u] = sm.lq[lqn - 1 - u * NL - li];
+                        }
                         lqn -= take;
                         // lanes past the end of their leaf load its first particle instead (no branch) and drop it
-                        const bool vA = sub < (int)lfA.y, vB = sub < (int)lfB.y;
-                        const float4 pA = __ldg(sorted_pos + (lfA.x + (vA ? (uint32_t)sub : 0u)));
-                        const float4 pB = __ldg(sorted_pos + (lfB.x + (vB ? (uint32_t)sub : 0u)));
-                        const bool keepA = vA && point_in_reach(pA, blo, bhi, R2);
-                        const bool keepB = vB && point_in_reach(pB, blo, bhi, R2);
-                        const uint32_t ka = __ballot_sync(FULL, keepA), kb = __ballot_sync(FULL, keepB);
-                        const int t0 = thead + tcount;
-                        if (keepA) {
-                            const int slot = (t0 + __popc(ka & lt_mask)) & (GW_TILE - 1);
-                            sm.tx[slot] = pA.x;
-                            sm.ty[slot] = pA.y;
-                            sm.tz[slot] = pA.z;
-                            sm.ti[slot] = __float_as_int(pA.w);
+#pragma unroll
+                        for (int u = 0; u < GW_NB; ++u)
+                            pc[u] = __ldg(sorted_pos + (lf[u].x + (sub < (int)lf[u].y ? (uint32_t)sub : 0u)));
+                        int nkept = 0;
+#pragma unroll
+                        for (int u = 0; u < GW_NB; ++u) {
+                            keep[u] = sub < (int)lf[u].y && point_in_reach(pc[u], blo, bhi, R2);
+                            const uint32_t kb = __ballot_sync(FULL, keep[u]);
+                            if (keep[u]) {
+                                const int slot = (thead + tcount + nkept + __popc(kb & lt_mask)) & (GW_TILE - 1);
+                                sm.tx[slot] = pc[u].x;
+                                sm.ty[slot] = pc[u].y;
+                                sm.tz[slot] = pc[u].z;
+                                sm.ti[slot] = __float_as_int(pc[u].w);
+                            }
+                            nkept += __popc(kb);
                         }
-                        if (keepB) {
-                            const int slot = (t0 + __popc(ka) + __popc(kb & lt_mask)) & (GW_TILE - 1);
-                            sm.tx[slot] = pB.x;
-                            sm.ty[slot] = pB.y;
-                            sm.tz[slot] = pB.z;
-                            sm.ti[slot] = __float_as_int(pB.w);
-                        }
-                        tcount += __popc(ka) + __popc(kb);
-                        if (STATS) st_cand += __popc(ka) + __popc(kb);
+                        tcount += nkept;
+                        if (STATS) st_cand += nkept;
                         __syncwarp();
                         continue;
                     }
