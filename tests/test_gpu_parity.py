@@ -270,3 +270,19 @@ def test_count_overlaps_is_the_papers_kernel(cid):
     # and it brackets the exact list: every true neighbor's leaf box overlaps
     nl.neighbors(w.r_list)
     assert np.all(got >= nl.n_neigh.cpu().numpy()[: w.N])
+
+
+@pytest.mark.parametrize("K", [1, 8])
+@pytest.mark.parametrize("cid", [1, 3, 4])
+def test_algorithm1_kernel_list_parity(cid, K):
+    """QBVH_OPT_VARIANT = 0: Algorithm 1 as written (one thread per particle) with the exact leaf
+    filter must emit the same lists as the oracle (and hence as the production kernel)."""
+    from paper_1901_08088_b200 import qbvh
+    w = W.make_config(cid, small=True)
+    qbvh.qbvh_set_option(qbvh.OPT_VARIANT, 0)
+    try:
+        out = gpu_run(w, K=K)
+    finally:
+        qbvh.qbvh_set_option(qbvh.OPT_VARIANT, 1)
+    rep = compare_with_oracle(w, out, ON.neighbor_list(w.pos, w.type, w.box, w.r_list))
+    assert rep["rows_checked"] == w.N
