@@ -286,3 +286,36 @@ def test_algorithm1_kernel_list_parity(cid, K):
         qbvh.qbvh_set_option(qbvh.OPT_VARIANT, 1)
     rep = compare_with_oracle(w, out, ON.neighbor_list(w.pos, w.type, w.box, w.r_list))
     assert rep["rows_checked"] == w.N
+
+
+def test_randomized_inputs_stress():
+    """Seeded random systems: sizes around warp/tile edges, 1-4 types with empty and rare ones, clustered, flat and
+    duplicated coordinates, skipped type pairs, odd row capacities (vector and scalar store paths, overflow), every
+    collapse threshold.  Each list must equal the oracle's."""
+    rng = np.random.default_rng(20240607)
+    for it in range(60):
+        N = int(rng.choice([1, 2, 5, 33, 100, 777, 3000, 9000]))
+        T = int(rng.choice([1, 1, 2, 3, 4]))
+        L = rng.uniform(6.0, 30.0, 3) * np.array([1, 1, rng.choice([1, 3])])
+        pos = rng.random((N, 3)) * L
+        if rng.random() < 0.5 and N > 10:
+            c = rng.random((max(1, N // 50), 3)) * L
+            pos[: N // 2] = (c[rng.integers(0, len(c), N // 2)] + rng.normal(0, 0.4, (N // 2, 3))) % L
+        if rng.random() < 0.2:
+            pos[:, 2] = L[2] * 0.25
+        if rng.random() < 0.2 and N > 3:
+            pos[1] = pos[0]
+        typ = None
+        if T > 1:
+            typ = rng.choice(T, N, p=rng.dirichlet(np.ones(T) * 0.5)).astype(np.int32)
+        p32, box = W._finish(pos, L)
+        r = rng.uniform(0.5, min(0.45 * float(L.min()), 4.0), (T, T)).astype(np.float32)
+        r = np.maximum(r, r.T)
+        if T > 1 and rng.random() < 0.3:
+            r[0, 1] = r[1, 0] = 0.0
+        cap = int(rng.choice([0, 3, 4, 12, 16, 50, 64, 200]))
+        K = int(rng.choice([1, 2, 4, 8, 16, 32]))
+        w = W.Workload(f"stress{it}", p32, typ, box, r, cap)
+        out = gpu_run(w, K=K, max_neigh=cap)
+        csr = ON.neighbor_list(w.pos, w.type, w.box, w.r_list, method="brute" if N <= 3000 else "cell")
+        compare_with_oracle(w, out, csr, allow_overflow=True)
