@@ -39,6 +39,8 @@ extern "C" {
 #define QBVH_ERR_CUTOFF_TOO_LARGE (-4) /* some padded r_ij >= L_d/2: a pair could be seen through two images       */
 #define QBVH_ERR_TYPE_RANGE (-5)       /* a type id outside [0, T) was seen by the build (reported by qbvh_neighbors) */
 #define QBVH_ERR_CUDA (-6)             /* a CUDA runtime call failed; text via qbvh_error_string(QBVH_ERR_CUDA)    */
+#define QBVH_ERR_INTERNAL (-7)         /* an internal bound was violated (the traversal's work list); the
+                                          lists of that call are invalid.  Never seen; reported instead of corrupting. */
 
 #define QBVH_MAX_TYPES 4 /* type id lives in bits 30-31 of the 32-bit sort key above the 30-bit Morton code */
 
@@ -54,8 +56,12 @@ int qbvh_set_num_types(int32_t T);
 /* Bytes of DEVICE workspace needed for N particles and T types (tree + scratch), a multiple of 256. */
 int64_t qbvh_workspace_bytes(int64_t N, int32_t T);
 
-/* Caller-owned DEVICE workspace, 256-byte aligned; must stay valid until the next qbvh_set_workspace.
- * Invalidates the current tree. */
+/* Caller-owned DEVICE workspace, 256-byte aligned; must stay valid until the next qbvh_set_workspace and its
+ * CONTENTS must not be modified by the caller between qbvh_build calls: rebuilding on the same workspace with the
+ * same N does not clear the tree builder's meeting slots, it tells stale ones apart by a per-build tag (DESIGN.md
+ * §3.6), so foreign data written there could be mistaken for a sibling.  Call qbvh_set_workspace again (same
+ * pointer is fine) after using the memory for anything else: that clears the slots at the next build.
+ * Invalidates the current tree.  qbvh_set_workspace(NULL, 0) detaches the library from the memory. */
 int qbvh_set_workspace(void *dev_ptr, int64_t bytes);
 
 /* Options (all take effect at the next qbvh_build unless noted). */
@@ -67,6 +73,8 @@ int qbvh_set_workspace(void *dev_ptr, int64_t bytes);
 #define QBVH_OPT_VARIANT 3       /* which traversal kernel qbvh_neighbors launches: 0 = Algorithm 1 as written, one
                                     thread per particle; 1 (default) = one warp per query group.
                                     Both produce identical lists.                                                 */
+#define QBVH_OPT_DEBUG_BUILD_TAG 4 /* testing only: v in [1, 2^24): the next qbvh_build on this workspace uses meeting-
+                                    slot tag v (forward jumps only) — lets a test reach the 24-bit wrap.           */
 int qbvh_set_option(int32_t key, int32_t value);
 int qbvh_get_option(int32_t key);
 
@@ -119,6 +127,13 @@ int qbvh_build_host(const float *pos, const int32_t *type, int64_t N, const floa
 int qbvh_neighbors_host(const float *r_list_ij, int32_t *nlist, int32_t *n_neigh, int32_t max_neigh);
 
 /* ---- inspection ----------------------------------------------------------------------------- */
+
+/* The padded pruning radius the traversal uses in every sphere/box overlap test (never in the pair predicate):
+ *   r_pad = up( up(r (1 + 2^-20)) + 8 ulp32(M) ),  M = max_d(|lo_d| + 2 L_d)      (reading R11)
+ * "the sphere radius is padded to account for uncertainty from loss of precision" — here for the
+ * fp32 roundings of x_i + v_j, y - x' and the squared sum, so that no true pair is pruned.
+ * Pure host arithmetic, needs no device.  box: HOST 6 floats as for qbvh_build.  Returns < 0 on bad arguments. */
+float qbvh_padded_radius(float r, const float *box);
 
 typedef struct qbvh_stats {
     uint64_t node_tests;    /* sphere-AABB tests of Algorithm 1 line 12 (root tests of line 4 excluded)           */

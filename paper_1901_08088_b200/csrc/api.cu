@@ -1,5 +1,4 @@
 // api.cu — the C-ABI of libqbvh.so (include/qbvh.h): argument checks, workspace carving, launches.
-#include <cfenv>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -70,26 +69,29 @@ int cuda_fail(cudaError_t e, const char *where) {
     return QBVH_ERR_CUDA;
 }
 
-float mul_ru(float a, float b) {
-    std::fesetround(FE_UPWARD);
-    volatile float r = a * b;
-    std::fesetround(FE_TONEAREST);
-    return r;
+// smallest fp32 value >= x (x finite, inside the fp32 range)
+float up_to_f32(double x) {
+    float f = (float)x;                       // round to nearest
+    if ((double)f < x) f = std::nextafterf(f, INFINITY);
+    return f;
 }
 
-// padded pruning radius: r_pad = add_ru(mul_ru(r, 1 + 2^-20), 8 ulp32(M)), M = max_d(|lo_d| + 2 L_d)
+// Padded pruning radius (reading R11; PAPER.md:140 pads the sphere for fp64 data only):
+//   r_pad = up(up(r (1 + 2^-20)) + 8 ulp32(M)),  M = max_d(|lo_d| + 2 L_d),  ulp32(M) = 2^(floor(log2 M) - 23).
+// Both sums below are exact in fp64 (a 24-bit times a 21-bit significand; two fp32 values less than 2^22 ulp apart),
+// so the only roundings are the two explicit ones upward.
 float padded_radius(float r, const float *box) {
     double M = 0.0;
     for (int d = 0; d < 3; ++d) M = std::fmax(M, std::fabs((double)box[d]) + 2.0 * (double)box[3 + d]);
-    int e;
-    std::frexp(M, &e);
-    const float pad_abs = (float)std::ldexp(8.0, (e - 1) - 23);
-    std::fesetround(FE_UPWARD);
-    volatile float a = r * (1.0f + 0x1p-20f);
-    volatile float b = a + pad_abs;
-    std::fesetround(FE_TONEAREST);
-    return b;
+    const double pad = std::scalbn(1.0, std::ilogb(M) - 20);      // 8 ulp32(M) = 2^3 2^(floor(log2 M) - 23)
+    const float a = up_to_f32((double)r * (1.0 + 0x1p-20));
+    double sum = (double)a + pad;
+    if (sum - pad != (double)a) sum = std::nextafter(sum, INFINITY);   // r below 2^-29 pad: stay on the safe side
+    return up_to_f32(sum);
 }
+
+// a * b rounded up (the product of two fp32 values is exact in fp64)
+float mul_ru(float a, float b) { return up_to_f32((double)a * (double)b); }
 
 // r_list -> the traversal's parameter block (exact r^2, padded pruning radius, Morton binning of the build)
 int make_params(const float *r_list, TraverseParams &P) {
@@ -150,6 +152,7 @@ int finish_neighbors() {
     cudaError_t e = cudaStreamSynchronize(g.stream);
     if (e != cudaSuccess) return cuda_fail(e, "stream synchronize");
     if (g.pinned[1] & 1) return QBVH_ERR_TYPE_RANGE;
+    if (g.pinned[1] & 2) return QBVH_ERR_INTERNAL;
     return g.pinned[0];
 }
 
@@ -196,6 +199,11 @@ int qbvh_set_option(int32_t key, int32_t value) {
             if (value < 0 || value > 1) return QBVH_ERR_INVALID_ARG;
             g.variant = value;
             return QBVH_OK;
+        case QBVH_OPT_DEBUG_BUILD_TAG:
+            // only forward: slots of earlier builds carry smaller tags and must never match a later build
+            if (value < 1 || value > 0xFFFFFF || (uint32_t)value <= g.build_tag) return QBVH_ERR_INVALID_ARG;
+            if (g.build_tag != 0) g.build_tag = (uint32_t)value - 1;   // a slot area still to be cleared stays at tag 0
+            return QBVH_OK;
         default:
             return QBVH_ERR_INVALID_ARG;
     }
@@ -206,6 +214,7 @@ int qbvh_get_option(int32_t key) {
         case QBVH_OPT_LEAF_COLLAPSE: return g.K;
         case QBVH_OPT_STATS: return g.stats ? 1 : 0;
         case QBVH_OPT_VARIANT: return g.variant;
+        case QBVH_OPT_DEBUG_BUILD_TAG: return (int)g.build_tag;
         default: return QBVH_ERR_INVALID_ARG;
     }
 }
@@ -323,10 +332,10 @@ int qbvh_neighbors_host(const float *r_list_ij, int32_t *nlist, int32_t *n_neigh
     int32_t *dlist = reinterpret_cast<int32_t *>(s + align256(12 * n1) + align256(4 * n1));
     int32_t *dcnt = reinterpret_cast<int32_t *>(s + align256(12 * n1) + align256(4 * n1) +
                                                 align256(4 * n1 * (int64_t)(max_neigh > 0 ? max_neigh : 1)));
+    if (N > 0 && (!n_neigh || (!nlist && max_neigh > 0))) return QBVH_ERR_INVALID_ARG;
     int rc = neighbors_impl(r_list_ij, dlist, dcnt, max_neigh);
     if (rc != QBVH_OK) return rc;
     if (N > 0) {
-        if (!n_neigh || (!nlist && max_neigh > 0)) return QBVH_ERR_INVALID_ARG;
         cudaError_t e = cudaMemcpyAsync(n_neigh, dcnt, 4 * N, cudaMemcpyDeviceToHost, g.stream);
         if (e != cudaSuccess) return cuda_fail(e, "D2H n_neigh");
         if (max_neigh > 0) {
@@ -335,6 +344,13 @@ int qbvh_neighbors_host(const float *r_list_ij, int32_t *nlist, int32_t *n_neigh
         }
     }
     return finish_neighbors();
+}
+
+float qbvh_padded_radius(float r, const float *box) {
+    if (!box || !(r > 0.0f) || !std::isfinite(r)) return -1.0f;
+    for (int d = 0; d < 3; ++d)
+        if (!std::isfinite(box[d]) || !std::isfinite(box[3 + d]) || !(box[3 + d] > 0.0f)) return -1.0f;
+    return padded_radius(r, box);
 }
 
 int qbvh_get_stats(qbvh_stats *out) {
@@ -386,6 +402,7 @@ const char *qbvh_error_string(int code) {
         case QBVH_ERR_WORKSPACE: return "workspace/staging missing, misaligned or too small";
         case QBVH_ERR_CUTOFF_TOO_LARGE: return "padded cutoff is not below half the shortest box length";
         case QBVH_ERR_TYPE_RANGE: return "a particle type id is outside [0, T)";
+        case QBVH_ERR_INTERNAL: return "internal bound violated (traversal work list); please report";
         case QBVH_ERR_CUDA: return g.cuda_msg;
         default: return code > 0 ? "ok (positive return value)" : "unknown error code";
     }

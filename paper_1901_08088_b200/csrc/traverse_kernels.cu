@@ -284,7 +284,7 @@ constexpr int GW_RING = QBVH_GW_RING;     // staged neighbors per lane: blocks o
 constexpr int GW_RING_BYTES = 4 * GW_RING;
 
 struct __align__(256) GwShared {
-    int32_t ring[32][GW_RING];                     // per-lane staged neighbors (256 bytes per lane)
+    int32_t ring[32][GW_RING];                     // per-lane staged neighbors (GW_RING_BYTES per lane)
     float tx[GW_TILE], ty[GW_TILE], tz[GW_TILE];   // candidate tile ring, structure of arrays
     int32_t ti[GW_TILE];                           // original particle index of each candidate
     uint32_t wl[GW_WL];                            // work list: node id | (also test its rope sibling) << 31
@@ -398,8 +398,8 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
     const uint32_t FULL = 0xFFFFFFFFu;
     const uint32_t lt_mask = (1u << lane) - 1u;
     GwShared &sm = s_all[warp];
-    int32_t *const myring = static_cast<int32_t *>(__builtin_assume_aligned(sm.ring[lane], 256));
-    const uint32_t ring_s = (uint32_t)__cvta_generic_to_shared(myring);   // 256-byte aligned
+    int32_t *const myring = static_cast<int32_t *>(__builtin_assume_aligned(sm.ring[lane], GW_RING_BYTES));
+    const uint32_t ring_s = (uint32_t)__cvta_generic_to_shared(myring);   // aligned to the ring size
     // every lane's ring starts at another quad, so that lanes filling at the same pace hit different banks
     const uint32_t rot = (uint32_t)(lane & 7) << 4;
     const int ngroups = meta->group_count;
@@ -411,6 +411,7 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
     const int li = lane / WS, sub = lane % WS;
     unsigned long long st_tests = 0, st_leaf = 0, st_cand = 0, st_checks = 0, st_steps = 0, st_groups = 0;
     int wmax = 0;
+    bool bound_violated = false;
 
     while (true) {
         int g = 0;
@@ -620,9 +621,17 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
                         const uint32_t pa = __ballot_sync(FULL, pushA), pb = __ballot_sync(FULL, pushB);
                         const uint32_t ea = __ballot_sync(FULL, emitA), eb = __ballot_sync(FULL, emitB);
                         const int base = wsz - npop;
-                        if (pushA) sm.wl[base + __popc(pa & lt_mask)] = (uint32_t)A.z | 0x80000000u;
-                        if (pushB) sm.wl[base + __popc(pa) + __popc(pb & lt_mask)] = (uint32_t)B.z | 0x80000000u;
-                        wsz = base + __popc(pa) + __popc(pb);
+                        // Bound of the work list: up to 160 entries a step pops <= 32 and pushes <= 64
+                        // (wsz <= 192); above 160 it pops ONE entry and pushes <= 2, a depth-first descent that can
+                        // grow the list by at most the depth of the tree below that entry (<= 60 levels: 30 code bits
+                        // + 30 index bits) => wsz <= 252 < GW_WL.  The guard makes a violated bound an error, never
+                        // an out-of-bounds write.
+                        const int nw = base + __popc(pa) + __popc(pb);
+                        const bool fits = nw <= GW_WL;
+                        if (pushA && fits) sm.wl[base + __popc(pa & lt_mask)] = (uint32_t)A.z | 0x80000000u;
+                        if (pushB && fits) sm.wl[base + __popc(pa) + __popc(pb & lt_mask)] = (uint32_t)B.z | 0x80000000u;
+                        wsz = fits ? nw : base;
+                        bound_violated |= !fits;
                         if (emitA) sm.lq[lqn + __popc(ea & lt_mask)] = make_uint2((uint32_t)(~A.z), (uint32_t)leaf_count(A, P.N, seg_end));
                         if (emitB)
                             sm.lq[lqn + __popc(ea) + __popc(eb & lt_mask)] = make_uint2((uint32_t)(~B.z), (uint32_t)leaf_count(B, P.N, seg_end));
@@ -712,6 +721,7 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
     }
     wmax = __reduce_max_sync(FULL, wmax);
     if (lane == 0 && wmax > 0) atomicMax(&meta->max_count, wmax);
+    if (lane == 0 && bound_violated) atomicOr(&meta->err_flags, 2);
     if (STATS && lane == 0) {
         atomicAdd(&meta->stats[5], st_groups);
         atomicAdd(&meta->stats[6], st_tests);

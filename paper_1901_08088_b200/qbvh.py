@@ -15,16 +15,16 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libqbvh.so")
 
 OK = 0
-ERR_INVALID_ARG, ERR_NOT_BUILT, ERR_WORKSPACE, ERR_CUTOFF_TOO_LARGE, ERR_TYPE_RANGE, ERR_CUDA = -1, -2, -3, -4, -5, -6
+ERR_INVALID_ARG, ERR_NOT_BUILT, ERR_WORKSPACE, ERR_CUTOFF_TOO_LARGE, ERR_TYPE_RANGE, ERR_CUDA, ERR_INTERNAL = -1, -2, -3, -4, -5, -6, -7
 MAX_TYPES = 4
-OPT_LEAF_COLLAPSE, OPT_STATS, OPT_VARIANT = 1, 2, 3
+OPT_LEAF_COLLAPSE, OPT_STATS, OPT_VARIANT, OPT_DEBUG_BUILD_TAG = 1, 2, 3, 4
 EXPORT_KEYS_SORTED, EXPORT_PERM, EXPORT_NODES, EXPORT_PARENT, EXPORT_FRAMES, EXPORT_SEGMENTS, EXPORT_SORTED_POS = range(1, 8)
 
 # every symbol include/qbvh.h declares
 SYMBOLS = ("qbvh_set_stream", "qbvh_set_num_types", "qbvh_workspace_bytes", "qbvh_set_workspace",
            "qbvh_set_option", "qbvh_get_option", "qbvh_build", "qbvh_neighbors", "qbvh_count_overlaps", "qbvh_staging_bytes",
            "qbvh_set_staging", "qbvh_build_host", "qbvh_neighbors_host", "qbvh_get_stats", "qbvh_debug_export",
-           "qbvh_error_string")
+           "qbvh_error_string", "qbvh_padded_radius")
 
 
 class QbvhStats(C.Structure):
@@ -63,6 +63,8 @@ _lib.qbvh_neighbors_host.argtypes = [_vp, _vp, _vp, _i32]
 _lib.qbvh_get_stats.argtypes = [C.POINTER(QbvhStats)]
 _lib.qbvh_debug_export.argtypes = [_i32, _vp, _i64]
 _lib.qbvh_debug_export.restype = _i64
+_lib.qbvh_padded_radius.argtypes = [C.c_float, _vp]
+_lib.qbvh_padded_radius.restype = C.c_float
 _lib.qbvh_error_string.argtypes = [C.c_int]
 _lib.qbvh_error_string.restype = C.c_char_p
 
@@ -78,6 +80,18 @@ def _ptr(x):
         return x.ctypes.data
     assert x.is_contiguous()
     return x.data_ptr()
+
+
+_bound_workspace = None   # (id of the NeighborList, device pointer) the C context currently points at
+_num_types = 1   # T of the last qbvh_set_num_types: the C side reads T x T floats from r_list_ij
+
+
+def _r_list(r_list_ij):
+    """HOST T x T fp32 cutoff table; the size is checked here because the C-ABI takes a bare pointer."""
+    r = np.ascontiguousarray(r_list_ij, dtype=np.float32)
+    if r.size != _num_types * _num_types:
+        raise ValueError(f"r_list_ij holds {r.size} values; qbvh_set_num_types({_num_types}) needs {_num_types}x{_num_types}")
+    return r
 
 
 def _host_f32(a, n):
@@ -101,7 +115,10 @@ def qbvh_set_stream(cuda_stream: int) -> int:
 
 
 def qbvh_set_num_types(T: int) -> int:
-    return _check(_lib.qbvh_set_num_types(T), "qbvh_set_num_types")
+    global _num_types
+    rc = _check(_lib.qbvh_set_num_types(T), "qbvh_set_num_types")
+    _num_types = int(T)
+    return rc
 
 
 def qbvh_workspace_bytes(N: int, T: int = 1) -> int:
@@ -109,6 +126,8 @@ def qbvh_workspace_bytes(N: int, T: int = 1) -> int:
 
 
 def qbvh_set_workspace(buf, nbytes: int | None = None) -> int:
+    global _bound_workspace
+    _bound_workspace = None
     if nbytes is None:
         nbytes = 0 if buf is None else buf.numel() * buf.element_size()
     return _check(_lib.qbvh_set_workspace(_ptr(buf), nbytes), "qbvh_set_workspace")
@@ -128,15 +147,15 @@ def qbvh_build(pos, type, N: int, box) -> int:
     return _check(_lib.qbvh_build(_ptr(pos), _ptr(type), N, box.ctypes.data), "qbvh_build")
 
 
-def qbvh_neighbors(r_list_ij, nlist, n_neigh, max_neigh: int, T: int | None = None) -> int:
+def qbvh_neighbors(r_list_ij, nlist, n_neigh, max_neigh: int) -> int:
     """r_list_ij: host T x T; nlist, n_neigh: DEVICE int32 tensors.  Returns M = max n_neigh (overflow iff M > max_neigh)."""
-    r = np.ascontiguousarray(r_list_ij, dtype=np.float32)
+    r = _r_list(r_list_ij)
     return _check(_lib.qbvh_neighbors(r.ctypes.data, _ptr(nlist), _ptr(n_neigh), max_neigh), "qbvh_neighbors")
 
 
 def qbvh_count_overlaps(r_list_ij, n_overlap) -> int:
     """The paper's accept-on-leaf-overlap count.  n_overlap: DEVICE int32 tensor of N."""
-    r = np.ascontiguousarray(r_list_ij, dtype=np.float32)
+    r = _r_list(r_list_ij)
     return _check(_lib.qbvh_count_overlaps(r.ctypes.data, _ptr(n_overlap)), "qbvh_count_overlaps")
 
 
@@ -157,8 +176,17 @@ def qbvh_build_host(pos, type, N: int, box) -> int:
 
 
 def qbvh_neighbors_host(r_list_ij, nlist, n_neigh, max_neigh: int) -> int:
-    r = np.ascontiguousarray(r_list_ij, dtype=np.float32)
+    r = _r_list(r_list_ij)
     return _check(_lib.qbvh_neighbors_host(r.ctypes.data, _ptr(nlist), _ptr(n_neigh), max_neigh), "qbvh_neighbors_host")
+
+
+def qbvh_padded_radius(r: float, box) -> float:
+    """Host arithmetic only (no device): the padded pruning radius of include/qbvh.h."""
+    box = _host_f32(box, 6)
+    v = float(_lib.qbvh_padded_radius(C.c_float(float(r)), box.ctypes.data))
+    if v < 0:
+        raise QbvhError(ERR_INVALID_ARG, "qbvh_padded_radius")
+    return v
 
 
 def qbvh_get_stats() -> dict:
@@ -203,14 +231,32 @@ class NeighborList:
         self.retries = 0
 
     def _activate(self):
+        """Point the process-global context at this object: stream, T and (only when it changed) the workspace —
+        qbvh_set_workspace restarts the build tags, i.e. costs a clear of the meeting slots at the next build."""
+        global _bound_workspace
         qbvh_set_stream(self.torch.cuda.current_stream(self.device).cuda_stream)
         qbvh_set_num_types(self.T)
+        if _bound_workspace != (id(self), self.workspace.data_ptr()):
+            qbvh_set_workspace(self.workspace)
+            _bound_workspace = (id(self), self.workspace.data_ptr())
+
+    def release(self):
+        """Detach the library from this object's workspace (the tree is gone afterwards)."""
+        global _bound_workspace
+        if _bound_workspace is not None and _bound_workspace[0] == id(self):
+            _bound_workspace = None
+            qbvh_set_workspace(None)
+
+    def __del__(self):
+        try:
+            self.release()
+        except Exception:
+            pass
 
     def build(self, pos, type, box):
         assert pos.is_cuda and pos.dtype == self.torch.float32 and tuple(pos.shape) == (self.N, 3)
         assert type is None or (type.is_cuda and type.dtype == self.torch.int32)
         self._activate()
-        qbvh_set_workspace(self.workspace)
         return qbvh_build(pos, type, self.N, box)
 
     def neighbors(self, r_list, retry: bool = True) -> int:

@@ -64,6 +64,37 @@ def _finish(pos64: np.ndarray, L) -> tuple[np.ndarray, np.ndarray]:
     return np.ascontiguousarray(p, dtype=np.float32), box
 
 
+def place(pos64: np.ndarray, L, lo) -> tuple[np.ndarray, np.ndarray]:
+    """[0,L) fp64 coordinates -> fp32 coordinates in a box whose origin is `lo` (any place, not centred), wrapped
+    *in fp32* into [lo, lo + L): every coordinate p satisfies lo <= p and p - lo < L exactly."""
+    L = np.broadcast_to(np.asarray(L, dtype=np.float64), (3,))
+    L32 = L.astype(np.float32)
+    lo32 = np.broadcast_to(np.asarray(lo, dtype=np.float64), (3,)).astype(np.float32)
+    p = (pos64 + lo32.astype(np.float64)).astype(np.float32)
+    for d in range(3):
+        c = p[:, d]
+        hi = lo32[d].astype(np.float64) + L32[d].astype(np.float64)      # exact upper face
+        c = np.where(c.astype(np.float64) >= hi, (c - L32[d]).astype(np.float32), c)
+        c = np.where(c < lo32[d], (c + L32[d]).astype(np.float32), c)
+        c = np.maximum(c, lo32[d])
+        top = np.float32(hi)
+        if np.float64(top) >= hi:
+            top = np.nextafter(top, np.float32(-np.inf))                # largest fp32 strictly below the face
+        c = np.minimum(c, top)
+        p[:, d] = c
+    box = np.concatenate([lo32, L32]).astype(np.float32)
+    return np.ascontiguousarray(p, dtype=np.float32), box
+
+
+def shifted(w: "Workload", lo) -> "Workload":
+    """The same configuration in a box with origin `lo` instead of -L/2 (positions re-rounded to fp32 there)."""
+    L = w.box[3:6].astype(np.float64)
+    p64 = w.pos.astype(np.float64) - w.box[:3].astype(np.float64)       # back to [0, L)
+    pos, box = place(p64, L, lo)
+    return Workload(f"{w.name}_lo{tuple(float(x) for x in np.atleast_1d(lo))}", pos, w.type, box, w.r_list,
+                    w.max_neigh, dict(w.meta))
+
+
 def _rng(config_id: int, seed: int) -> np.random.Generator:
     return np.random.default_rng([config_id, seed])
 
@@ -169,9 +200,21 @@ def polymer_melt(n_chains: int = 10_000, chain_len: int = 100, rho: float = 0.85
     uses a hash grid of cell width >= r_reject holding at most CAP beads per
     cell (beads beyond CAP in one cell are not seen by the test; deterministic).
     """
-    rng = _rng(config_id, seed)
     N = n_chains * chain_len
     L = (N / rho) ** (1.0 / 3.0)
+    # the full-size generator takes about a minute: keep its output in the temp directory (pure function of the args)
+    import os
+    import tempfile
+    tag = f"{n_chains}_{chain_len}_{rho}_{bond}_{r_reject}_{max_rounds}_{seed}_{config_id}"
+    cache = os.path.join(tempfile.gettempdir(), f"qbvh_polymer_melt_{tag}.npz")
+    if N >= 200_000 and os.path.exists(cache):
+        try:
+            z = np.load(cache)
+            return Workload(f"polymer_melt_N{N}", z["pos"], None, z["box"], np.array([[r_list]], dtype=np.float32),
+                            max_neigh, {"rho": rho, "L": L, "forced_accepts": int(z["forced"]), "config": config_id})
+        except Exception:
+            pass
+    rng = _rng(config_id, seed)
     nc = int(np.floor(L / r_reject))
     assert nc >= 3, "box too small for the rejection grid"
     w = L / nc
@@ -234,6 +277,12 @@ def polymer_melt(n_chains: int = 10_000, chain_len: int = 100, rho: float = 0.85
         insert(new)
         prev = new
     pos, box = _finish(beads.reshape(N, 3), L)
+    if N >= 200_000:
+        try:
+            np.savez(cache + f".{os.getpid()}.tmp.npz", pos=pos, box=box, forced=forced)
+            os.replace(cache + f".{os.getpid()}.tmp.npz", cache)
+        except Exception:
+            pass
     return Workload(f"polymer_melt_N{N}", pos, None, box,
                     np.array([[r_list]], dtype=np.float32), max_neigh,
                     {"rho": rho, "L": L, "forced_accepts": int(forced), "config": config_id})

@@ -319,3 +319,132 @@ def test_randomized_inputs_stress():
         out = gpu_run(w, K=K, max_neigh=cap)
         csr = ON.neighbor_list(w.pos, w.type, w.box, w.r_list, method="brute" if N <= 3000 else "cell")
         compare_with_oracle(w, out, csr, allow_overflow=True)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# Round-2 additions: boxes whose origin is not -L/2, the boundary pairs of the pad pin, Algorithm 1 as printed at
+# BASELINE sizes, the work-list bound, rebuilding in place on one workspace.
+# ---------------------------------------------------------------------------------------------------------------
+ORIGINS = [(0.0, 0.0, 0.0), (1000.0, -3000.0, 17.0), (65536.0, -65536.0, 32768.0)]
+
+
+@pytest.mark.parametrize("lo", ORIGINS)
+@pytest.mark.parametrize("cid", [1, 3, 5])
+def test_noncentred_box(cid, lo):
+    """box_lo enters the Morton binning (a1), the entry-cell selection and the pad: keys, nodes and lists must match
+    the oracle in boxes that do not start at -L/2 (far from the origin the fp32 grid is coarse: 2^-7 at 65536)."""
+    w = W.shifted(W.make_config(cid, small=True), lo)
+    for K in (1, 32):
+        out, t = check_build(w, K)
+        rep = compare_with_oracle(w, out, ON.neighbor_list(w.pos, w.type, w.box, w.r_list))
+        assert rep["rows_checked"] == w.N
+
+
+@pytest.mark.parametrize("lo", ORIGINS + [(-12.0, -12.0, -12.0)])
+def test_boundary_pairs_across_faces_and_corners(lo):
+    """The inputs of tests/test_oracle_tree.py::test_boundary_pairs_...: pairs at exactly r, one grid step inside and
+    outside, through face and corner images.  Production kernel and Algorithm 1 as printed, K = 1 and collapsed."""
+    from adversarial_inputs import boundary_pairs
+    from paper_1901_08088_b200 import qbvh
+    L, r, grid = 24.0, 3.0, 2.0 ** -6
+    p, lo64 = boundary_pairs(lo, L, r, grid)
+    pos, box = W.place(p, L, lo64)
+    w = W.Workload("boundary", pos, None, box, np.array([[r]], np.float32), 128)
+    csr = ON.neighbor_list(w.pos, None, w.box, w.r_list, method="brute")
+    for variant in (1, 0):
+        qbvh.qbvh_set_option(qbvh.OPT_VARIANT, variant)
+        try:
+            for K in (1, 8, 32):
+                compare_with_oracle(w, gpu_run(w, K=K), csr)
+        finally:
+            qbvh.qbvh_set_option(qbvh.OPT_VARIANT, 1)
+
+
+@pytest.mark.parametrize("cid", [2, 5])
+def test_algorithm1_as_printed_full_size(cid):
+    """BASELINE sizes through the paper's own kernels: variant 0 (Algorithm 1, one thread per particle, exact leaf
+    filter) must emit the oracle's lists, and qbvh_count_overlaps on the one-particle-per-leaf tree must equal the
+    CPU replay of Algorithm 1 per particle."""
+    import torch
+    from paper_1901_08088_b200 import qbvh
+    w = W.make_config(cid)
+    qbvh.qbvh_set_option(qbvh.OPT_VARIANT, 0)
+    try:
+        out = gpu_run(w, K=1)
+    finally:
+        qbvh.qbvh_set_option(qbvh.OPT_VARIANT, 1)
+    rep = compare_with_oracle(w, out, ON.neighbor_list(w.pos, w.type, w.box, w.r_list, method="cell"))
+    assert rep["rows_checked"] == w.N
+    dev = torch.device("cuda:0")
+    qbvh.qbvh_set_option(qbvh.OPT_LEAF_COLLAPSE, 1)
+    nl = qbvh.NeighborList(w.N, T=w.T, max_neigh=1, device=dev)
+    nl.build(torch.from_numpy(w.pos).to(dev), None, w.box)
+    cnt = torch.full((w.N,), -7, dtype=torch.int32, device=dev)
+    M = qbvh.qbvh_count_overlaps(w.r_list, cnt)
+    t = OT.build(w.pos, w.type, w.box, T=w.T)
+    tr = OT.traverse(t, w.box, w.r_list)
+    expect = tr["n_overlap"].astype(np.int64) - 1                       # minus the particle's own leaf (PAPER.md:65)
+    assert np.array_equal(cnt.cpu().numpy()[t.perm], expect) and M == int(expect.max())
+    assert np.all(expect[np.argsort(t.perm)] >= out["n_neigh"])        # brackets the exact list (PAPER.md:85, 196)
+
+
+def test_work_list_bound():
+    """The warp work list of the production traversal: a cutoff that reaches everything in a dense,
+    duplicate-ridden cloud drives the list to its 192-entry breadth-first fill and then into the one-entry depth-first
+    mode over deep subtrees (duplicates extend the tree by the index bits).  Lists must still equal the oracle's and
+    no bound may be reported violated (QBVH_ERR_INTERNAL would raise)."""
+    rng = np.random.default_rng(77)
+    L = 64.0
+    base = rng.random((600, 3)) * 6.0 + 29.0                  # a blob in the middle of the box
+    comb = 32.0 + 24.0 * 2.0 ** -np.arange(1, 25)[:, None] * np.ones((1, 3))   # a comb: keys with ever longer common prefixes
+    p = np.concatenate([np.repeat(base, 8, axis=0), np.repeat(comb, 16, axis=0), rng.random((300, 3)) * L])
+    p = p[rng.permutation(len(p))]
+    pos, box = W._finish(p, L)
+    for r, cap in ((30.0, 5600), (5.0, 5600)):
+        w = W.Workload("worklist", pos, None, box, np.array([[r]], np.float32), cap)
+        csr = ON.neighbor_list(w.pos, None, w.box, w.r_list, method="brute")
+        for K in (1, 2, 32):
+            compare_with_oracle(w, gpu_run(w, K=K), csr)
+
+
+def test_rebuild_in_place_on_one_workspace():
+    """What an MD code does: qbvh_build again and again on ONE workspace.  The meeting slots of the tree builder are
+    not cleared between builds, stale ones are told apart by a per-build tag.  Same N, different
+    positions / types / K each time, nodes, parents and lists compared with the oracle after every build, and the
+    24-bit tag driven through its wrap."""
+    import torch
+    from paper_1901_08088_b200 import qbvh
+    dev = torch.device("cuda:0")
+    N, T = 30_000, 2
+    rng = np.random.default_rng(11)
+    nl = qbvh.NeighborList(N, T=T, max_neigh=256, device=dev)
+    box_L = 40.0
+    tags = []
+    for it in range(7):
+        p = rng.random((N, 3)) * box_L
+        if it % 2:
+            p[: N // 3] = (p[: N // 3] * 0.2 + 10.0)            # a dense clump: another tree shape on the same slots
+        pos, box = W._finish(p, box_L)
+        typ = (rng.random(N) < (0.1 + 0.1 * it)).astype(np.int32)
+        r = np.array([[1.3, 1.1], [1.1, 0.9 + 0.05 * it]], np.float32)
+        K = [1, 32, 4, 1, 16, 32, 2][it]
+        qbvh.qbvh_set_option(qbvh.OPT_LEAF_COLLAPSE, K)
+        if it == 3:
+            nl._activate()
+            qbvh.qbvh_set_option(qbvh.OPT_DEBUG_BUILD_TAG, 0xFFFFFE)   # this build: 0xFFFFFE, next: 0xFFFFFF, then the wrap
+        nl.build(torch.from_numpy(pos).to(dev), torch.from_numpy(typ).to(dev), box)
+        tags.append(qbvh.qbvh_get_option(qbvh.OPT_DEBUG_BUILD_TAG))
+        w = W.Workload(f"rebuild{it}", pos, typ, box, r, 256)
+        t = OT.build(pos, typ, box, T=T)
+        nodes = qbvh.qbvh_debug_export(qbvh.EXPORT_NODES, N)
+        parent = qbvh.qbvh_debug_export(qbvh.EXPORT_PARENT, N)
+        real = np.ones(2 * N - 1, bool)
+        real[: N - 1] = t.first[: N - 1] >= 0
+        assert np.array_equal(nodes[real], expected_nodes(t, K)[real]), it
+        assert np.array_equal(parent[real], t.parent[real]), it
+        nl.n_neigh.fill_(-7)
+        M = nl.neighbors(r, retry=False)
+        out = {"M": M, "max_neigh": nl.max_neigh, "nlist": nl.nlist.cpu().numpy()[:N], "n_neigh": nl.n_neigh.cpu().numpy()[:N]}
+        compare_with_oracle(w, out, ON.neighbor_list(pos, typ, box, r))
+    assert tags == [1, 2, 3, 0xFFFFFE, 0xFFFFFF, 1, 2], tags      # no clearing between builds except at the wrap
+    qbvh.qbvh_set_option(qbvh.OPT_LEAF_COLLAPSE, 32)

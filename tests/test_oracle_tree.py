@@ -15,6 +15,7 @@ import pytest
 
 from oracle import neighbors as ON
 from oracle import tree as OT
+from adversarial_inputs import boundary_pairs
 from paper_1901_08088_b200 import workloads as W
 
 from conftest import read_golden
@@ -395,3 +396,78 @@ def test_false_positive_census_matches_paper(rho, key):
     # a7: mean number of images = prod_d (1 + 2 r_pad / extent_d) for uniform positions (closed form)
     L = float(w.box[3])
     assert abs(tr["n_images"].mean() - (1 + 2 * 3.0 / L) ** 3) < 0.02
+
+
+# --------------------------------------------------------------------------- R11: the padded pruning radius
+PAD_CASES = [  # (r, lo, L): centred boxes, boxes far from the origin, a box whose origin dwarfs its size, tiny and huge scales
+    (2.9, (-53.62, -53.62, -53.62), (107.25, 107.25, 107.25)),
+    (2.9, (0.0, 0.0, 0.0), (16.890675, 16.890675, 16.890675)),
+    (3.3, (-69.2, -69.2, -207.7), (138.46, 138.46, 415.39)),
+    (1.52246, (1000.0, -3000.0, 17.0), (105.5667, 105.5667, 105.5667)),
+    (11.62462, (65536.0, -65536.0, 32768.0), (163.3641, 163.3641, 163.3641)),
+    (0.75, (-1.0e6, 2.0e6, 3.0), (4.0, 5.0, 6.0)),
+    (3.0, (0.0, 0.0, 0.0), (8.0, 8.0, 8.0)),                     # M = 16 exactly: a power of two
+    (3.0, (0.0, 0.0, 0.0), (np.nextafter(np.float32(8), np.float32(0)),) * 3),   # M just below a power of two
+    (1.0e-3, (-0.01, -0.01, -0.01), (0.02, 0.02, 0.02)),
+    (4.0e4, (-1.0e5, -1.0e5, -1.0e5), (2.0e5, 2.0e5, 2.0e5)),
+]
+
+
+def pad_exact(r, box):
+    """r_pad from exact rationals: up32( up32(r (1 + 2^-20)) + 8 ulp32(M) ), M = max_d(|lo_d| + 2 L_d),
+    ulp32(M) = 2^(floor(log2 M) - 23) — the spacing of fp32 numbers at the largest coordinate magnitude the
+    traversal can form (x_i + v_j with |v_j| <= L)."""
+    M = max(abs(f32_to_frac(box[d])) + 2 * f32_to_frac(box[3 + d]) for d in range(3))
+    e = 0
+    while Fraction(2) ** (e + 1) <= M:
+        e += 1
+    while Fraction(2) ** e > M:
+        e -= 1
+    ulp = Fraction(2) ** (e - 23)
+    a = round_up_f32(f32_to_frac(r) * (1 + Fraction(1, 2 ** 20)))
+    return round_up_f32(f32_to_frac(a) + 8 * ulp), ulp
+
+
+@pytest.mark.parametrize("r,lo,L", PAD_CASES)
+def test_padded_radius_exact_rational(r, lo, L):
+    """Reading R11 ("the sphere radius is padded"): the oracle's r_pad AND the CUDA
+    library's host-side qbvh_padded_radius are each compared with the value from exact rational arithmetic — not with
+    one another.  A changed constant (8 -> 1, the exponent off by one, a rounding the wrong way) fails here."""
+    from paper_1901_08088_b200 import qbvh
+    box = np.array(list(lo) + list(L), np.float32)
+    r32 = np.float32(r)
+    want, ulp = pad_exact(r32, box)
+    # lower bound stated in the verdict of round 1: r_pad >= r (1 + 2^-20) + 8 ulp32(M), and it is the least such fp32 pair of roundings
+    assert f32_to_frac(want) >= f32_to_frac(r32) * (1 + Fraction(1, 2 ** 20)) + 8 * ulp
+    assert OT.r_pad(r32, box) == want
+    assert np.float32(qbvh.qbvh_padded_radius(float(r32), box)) == want
+    # the pad is what it is for: ulp32(M) really is the fp32 spacing at magnitude M
+    M = max(abs(float(box[d])) + 2 * float(box[3 + d]) for d in range(3))
+    assert float(ulp) == float(np.spacing(np.float32(M))) or float(ulp) * 2 == float(np.spacing(np.float32(M)))
+
+
+@pytest.mark.parametrize("lo", [(0.0, 0.0, 0.0), (1000.0, -3000.0, 17.0), (65536.0, -65536.0, 32768.0), (-12.0, -12.0, -12.0)])
+def test_boundary_pairs_across_faces_and_corners_are_never_missed(lo):
+    """Conservativeness where the pad matters: pairs at exactly r_c and one grid step inside,
+    reached through face and corner images, in boxes whose origin is not -L/2.  Algorithm 1's replay on the quantized
+    tree must accept the leaf of every O1 neighbor; pairs one step outside must not be O1 neighbors."""
+    L, r, grid = 24.0, 3.0, 2.0 ** -6
+    p, lo64 = boundary_pairs(lo, L, r, grid)
+    pos, box = W.place(p, L, lo64)
+    assert np.array_equal(pos.astype(np.float64) - box[:3].astype(np.float64), np.mod(p, L))   # placement was exact
+    rl = np.array([[r]], np.float32)
+    rp, nb, band = ON.neighbor_list(pos, None, box, rl, method="brute")
+    n = len(pos)
+    # the construction: every particle placed at exactly r or inside is a neighbor of its base point, those outside are not
+    d64 = np.array([[ON.pair(pos[i], pos[j], box, r)[2] for j in range(n)] for i in (0,)])[0]
+    assert np.sum(np.abs(d64 - r) < 1e-9) >= 10 and np.sum(np.abs(d64 - (r - grid)) < 1e-2) >= 10
+    for j in range(1, n):
+        assert (j in nb[rp[0]:rp[1]]) == (d64[j] <= r), (j, d64[j])
+    t = OT.build(pos, None, box)
+    tr = OT.traverse(t, box, rl, fill=True)
+    missed = 0
+    for k in range(n):
+        i = t.perm[k]
+        cand = t.perm[tr["cand"][tr["row_ptr"][k]:tr["row_ptr"][k + 1]]]
+        missed += len(np.setdiff1d(nb[rp[i]:rp[i + 1]], cand))
+    assert missed == 0
