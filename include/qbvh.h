@@ -65,9 +65,10 @@ int64_t qbvh_workspace_bytes(int64_t N, int32_t T);
 int qbvh_set_workspace(void *dev_ptr, int64_t bytes);
 
 /* Options (all take effect at the next qbvh_build unless noted). */
-#define QBVH_OPT_LEAF_COLLAPSE 1 /* k in [1,32]: the traversal stops at nodes covering <= k consecutive Z-order
-                                    particles and distance-checks that range directly ("subtree
-                                    collapse").  k = 1 is exactly the paper's one-particle-per-leaf tree. Default 32. */
+#define QBVH_OPT_LEAF_COLLAPSE 1 /* k in [1,32]: the build may collapse a subtree of <= k consecutive Z-order particles
+                                    into one range leaf, whose particles the traversal distance-checks directly
+                                    ("subtree collapse"); which subtrees: qbvh_set_collapse_hint.
+                                    k = 1 is exactly the paper's one-particle-per-leaf tree. Default 32.           */
 #define QBVH_OPT_STATS 2         /* 0/1: qbvh_neighbors runs the instrumented traversal and fills qbvh_get_stats
                                     (takes effect immediately; slower — never use when timing). Default 0.        */
 #define QBVH_OPT_VARIANT 3       /* which traversal kernel qbvh_neighbors launches: 0 = Algorithm 1 as written, one
@@ -76,6 +77,15 @@ int qbvh_set_workspace(void *dev_ptr, int64_t bytes);
 #define QBVH_OPT_DEBUG_BUILD_TAG 4 /* testing only: v in [1, 2^24): the next qbvh_build on this workspace uses meeting-
                                     slot tag v (forward jumps only) — lets a test reach the 24-bit wrap.           */
 int qbvh_set_option(int32_t key, int32_t value);
+
+/* Hint for the build-side subtree collapse ("collapse subtrees according to an appropriate heuristic",
+ * PAPER.md:230): r_hint[b] = the query radius tree b (particle type b) will be searched with, e.g. max_a r_list[a][b].
+ *   r_hint HOST  n <= QBVH_MAX_TYPES floats; n = 0 or r_hint[b] <= 0: no hint for that tree.
+ * With a hint, two sibling range leaves are merged into one range leaf (of at most QBVH_OPT_LEAF_COLLAPSE particles)
+ * only if that lowers the expected cost of a query — an integer surface-area-like model on the quantized boxes
+ * swollen by the radius.  Without one, every subtree of at most QBVH_OPT_LEAF_COLLAPSE particles
+ * collapses.  Collapsed subtrees' descendants are never written.  Takes effect at the next qbvh_build. */
+int qbvh_set_collapse_hint(const float *r_hint, int32_t n);
 int qbvh_get_option(int32_t key);
 
 /* ---- the hot path --------------------------------------------------------------------------- */
@@ -159,12 +169,16 @@ int qbvh_get_stats(qbvh_stats *out);
 #define QBVH_EXPORT_PERM 2        /* uint32 [N]: original index of the particle at sorted position k              */
 #define QBVH_EXPORT_NODES 3       /* int32 [2N-1][4] = {lo, hi, left, rope}; internal node i at i (Karras
                                      numbering), leaf of sorted position k at N-1+k; left >= 0: left child,
-                                     left < 0: ~first sorted position; rope = -1: END           */
+                                     left < 0: a (range) leaf, ~first sorted position, the range ends where the
+                                     rope's target starts; rope = -1: END.  Only nodes reachable
+                                     from the roots are written: descendants of a range leaf do not exist.       */
 #define QBVH_EXPORT_PARENT 4      /* int32 [2N-1]: parent node, -1 for roots and unused slots                     */
 #define QBVH_EXPORT_FRAMES 5      /* float [4][12]: {lo_xyz, hi_xyz, delta_xyz, 0,0,0} quantization frame per type */
 #define QBVH_EXPORT_SEGMENTS 6    /* int32 [10]: seg[0..4] = first sorted position of each type (seg[4] = N),
                                      then roots[0..3] (-1 for an empty type), then 0                             */
 #define QBVH_EXPORT_SORTED_POS 7  /* float [N][4]: x, y, z, bits of the original index                            */
+#define QBVH_EXPORT_COUNTS 8      /* int32 [4]: nodes written by the build (2N-1 minus unused slots without collapse),
+                                     query groups, non-empty Morton cells of the build, its cell grid level       */
 int64_t qbvh_debug_export(int32_t what, void *dst, int64_t bytes);
 
 const char *qbvh_error_string(int code);

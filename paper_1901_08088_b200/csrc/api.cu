@@ -15,8 +15,11 @@ struct Context {
     void *staging = nullptr;
     int64_t staging_bytes = 0;
     int T = 1;
-    int K = 32;         // leaf-collapse option for the next build
+    int K = 32;         // leaf-collapse cap for the next build
     int K_built = 1;
+    float r_hint[QBVH_TMAX] = {0, 0, 0, 0};   // collapse heuristic: expected query radius against each tree (<= 0: none)
+    bool f64_built = false;
+    int lvl_built = 0;
     bool stats = false;
     int variant = 1;
     bool built = false;
@@ -25,7 +28,8 @@ struct Context {
     float scale[3] = {0, 0, 0};
     BuildBuffers buf{};
     uint32_t build_tag = 0;      // tag of the last build's meeting slots; 0: the slot area has to be cleared first
-    int64_t tag_N = -1;          // the layout (N) the slot area was cleared for
+    int64_t tag_N = -1;          // the layout (N, cell level, T) the slot area and the cell counters were cleared for
+    int tag_lvl = -1, tag_T = -1;
     int32_t *pinned = nullptr;   // 2 ints: max_count, err_flags
     qbvh_stats last_stats{};
     char cuda_msg[256] = "no CUDA error recorded";
@@ -34,13 +38,16 @@ struct Context {
 inline int64_t align256(int64_t x) { return (x + 255) & ~int64_t(255); }
 
 struct Layout {
-    int64_t meta, key_a, key_b, idx_a, idx_b, status0, status1, sorted_pos, nodes, parent, slot, groups, entry, total;
+    int64_t meta, key, ent, key_sorted, idx_sorted, cell_count, cell_start, cell_list, big_list, croot, sorted_pos,
+        sorted_pos64, nodes, parent, slot, groups, entry, scratch, total;
 };
 
+// Workspace carve-up.  Sized for the finest cell grid any (N, T) can choose, so the layout depends on N alone.
 Layout make_layout(int64_t N) {
     Layout L{};
     const int64_t n1 = N > 0 ? N : 1;
-    const int64_t tiles = (n1 + SORT_TILE - 1) / SORT_TILE;
+    const int64_t ncells = CELL_MAX_TOTAL;
+    const int64_t ncell_lists = n1 < ncells ? n1 : ncells;
     int64_t off = 0;
     auto take = [&](int64_t bytes) {
         int64_t o = off;
@@ -48,18 +55,23 @@ Layout make_layout(int64_t N) {
         return o;
     };
     L.meta = take(sizeof(TreeMeta));
-    L.key_a = take(4 * n1);
-    L.key_b = take(4 * n1);
-    L.idx_a = take(4 * n1);
-    L.idx_b = take(4 * n1);
-    L.status0 = take(4 * 256 * tiles);
-    L.status1 = take(4 * 256 * tiles);
+    L.key = take(4 * n1);
+    L.ent = take(8 * n1);
+    L.key_sorted = take(4 * n1);
+    L.idx_sorted = take(4 * n1);
+    L.cell_count = take(4 * ncells);
+    L.cell_start = take(4 * (ncells + 1));
+    L.cell_list = take(4 * ncell_lists);
+    L.big_list = take(4 * ncell_lists);
+    L.croot = take((int64_t)sizeof(CellRoot) * ncell_lists);
     L.sorted_pos = take(16 * n1);
+    L.sorted_pos64 = take(32 * n1);
     L.nodes = take(16 * (2 * n1 - 1));
     L.parent = take(4 * (2 * n1 - 1));
     L.slot = take(16 * n1);
     L.groups = take(8 * n1);
     L.entry = take(4 * (int64_t)QBVH_TMAX * ENTRY_CELLS);
+    L.scratch = take(18 * n1);
     L.total = off;
     return L;
 }
@@ -156,6 +168,73 @@ int finish_neighbors() {
     return g.pinned[0];
 }
 
+int build_impl(const void *pos, bool f64, const int32_t *type, int64_t N, const float *box) {
+    g.built = false;
+    if (N < 0 || N >= (int64_t(1) << 30) || !box || (N > 0 && !pos)) return QBVH_ERR_INVALID_ARG;
+    for (int d = 0; d < 3; ++d)
+        if (!std::isfinite(box[d]) || !std::isfinite(box[3 + d]) || !(box[3 + d] > 0.0f)) return QBVH_ERR_INVALID_ARG;
+    const Layout L = make_layout(N);
+    if (!g.ws || g.ws_bytes < L.total) return QBVH_ERR_WORKSPACE;
+    if (!g.pinned) {
+        cudaError_t e = cudaHostAlloc(reinterpret_cast<void **>(&g.pinned), 2 * sizeof(int32_t), cudaHostAllocDefault);
+        if (e != cudaSuccess) return cuda_fail(e, "cudaHostAlloc");
+        g.pinned[0] = g.pinned[1] = 0;
+    }
+    char *w = static_cast<char *>(g.ws);
+    g.buf.meta = reinterpret_cast<TreeMeta *>(w + L.meta);
+    g.buf.key = reinterpret_cast<uint32_t *>(w + L.key);
+    g.buf.ent = reinterpret_cast<uint2 *>(w + L.ent);
+    g.buf.key_sorted = reinterpret_cast<uint32_t *>(w + L.key_sorted);
+    g.buf.idx_sorted = reinterpret_cast<uint32_t *>(w + L.idx_sorted);
+    g.buf.cell_count = reinterpret_cast<uint32_t *>(w + L.cell_count);
+    g.buf.cell_start = reinterpret_cast<uint32_t *>(w + L.cell_start);
+    g.buf.cell_list = reinterpret_cast<uint32_t *>(w + L.cell_list);
+    g.buf.big_list = reinterpret_cast<int32_t *>(w + L.big_list);
+    g.buf.croot = reinterpret_cast<CellRoot *>(w + L.croot);
+    g.buf.sorted_pos = reinterpret_cast<float4 *>(w + L.sorted_pos);
+    g.buf.sorted_pos64 = reinterpret_cast<Pos64 *>(w + L.sorted_pos64);
+    g.buf.nodes = reinterpret_cast<int4 *>(w + L.nodes);
+    g.buf.parent = reinterpret_cast<int32_t *>(w + L.parent);
+    g.buf.slot = reinterpret_cast<uint4 *>(w + L.slot);
+    g.buf.groups = reinterpret_cast<uint2 *>(w + L.groups);
+    g.buf.entry = reinterpret_cast<int32_t *>(w + L.entry);
+    g.buf.scratch = reinterpret_cast<unsigned char *>(w + L.scratch);
+    std::memcpy(g.box, box, sizeof(g.box));
+    BuildParams bp{};
+    for (int d = 0; d < 3; ++d) {
+        volatile float s = 1023.0f / box[3 + d];   // fp32 RN
+        g.scale[d] = s;
+        bp.box_lo[d] = box[d];
+        bp.box_scale[d] = s;
+    }
+    bp.N = (int)N;
+    bp.T = type ? g.T : 1;
+    bp.K = g.K;
+    bp.lvl = pick_cell_level(N, bp.T);
+    bp.f64 = f64;
+    for (int t = 0; t < QBVH_TMAX; ++t) bp.r_hint[t] = g.r_hint[t];
+    // The meeting slots of the top-level walk carry a 24-bit build number and the cell counters are counted back to
+    // zero by every build: both are cleared only when the layout moves or the number wraps.
+    if (g.build_tag == 0 || g.build_tag >= 0xFFFFFFu || g.tag_N != N || g.tag_lvl != bp.lvl || g.tag_T != bp.T) {
+        cudaError_t em = cudaMemsetAsync(g.buf.slot, 0, (size_t)16 * (size_t)(N > 0 ? N : 1), g.stream);
+        if (em == cudaSuccess) em = cudaMemsetAsync(g.buf.cell_count, 0, (size_t)4 * CELL_MAX_TOTAL, g.stream);
+        if (em != cudaSuccess) return cuda_fail(em, "memset slots");
+        g.build_tag = 0;
+        g.tag_N = N;
+        g.tag_lvl = bp.lvl;
+        g.tag_T = bp.T;
+    }
+    bp.build_tag = ++g.build_tag;
+    cudaError_t e = launch_build(pos, type, bp, g.buf, g.stream);
+    if (e != cudaSuccess) return cuda_fail(e, "build launch");
+    g.N = N;
+    g.K_built = g.K;
+    g.f64_built = f64;
+    g.lvl_built = bp.lvl;
+    g.built = true;
+    return QBVH_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -220,52 +299,16 @@ int qbvh_get_option(int32_t key) {
 }
 
 int qbvh_build(const float *pos, const int32_t *type, int64_t N, const float *box) {
-    g.built = false;
-    if (N < 0 || N >= (int64_t(1) << 30) || !box || (N > 0 && !pos)) return QBVH_ERR_INVALID_ARG;
-    for (int d = 0; d < 3; ++d)
-        if (!std::isfinite(box[d]) || !std::isfinite(box[3 + d]) || !(box[3 + d] > 0.0f)) return QBVH_ERR_INVALID_ARG;
-    const Layout L = make_layout(N);
-    if (!g.ws || g.ws_bytes < L.total) return QBVH_ERR_WORKSPACE;
-    if (!g.pinned) {
-        cudaError_t e = cudaHostAlloc(reinterpret_cast<void **>(&g.pinned), 2 * sizeof(int32_t), cudaHostAllocDefault);
-        if (e != cudaSuccess) return cuda_fail(e, "cudaHostAlloc");
-        g.pinned[0] = g.pinned[1] = 0;
+    return build_impl(pos, false, type, N, box);
+}
+
+int qbvh_set_collapse_hint(const float *r_hint, int32_t n) {
+    if (n < 0 || n > QBVH_MAX_TYPES || (n > 0 && !r_hint)) return QBVH_ERR_INVALID_ARG;
+    for (int t = 0; t < QBVH_TMAX; ++t) g.r_hint[t] = 0.0f;
+    for (int t = 0; t < n; ++t) {
+        if (std::isnan(r_hint[t]) || std::isinf(r_hint[t])) return QBVH_ERR_INVALID_ARG;
+        g.r_hint[t] = r_hint[t];
     }
-    char *w = static_cast<char *>(g.ws);
-    g.buf.meta = reinterpret_cast<TreeMeta *>(w + L.meta);
-    g.buf.key_a = reinterpret_cast<uint32_t *>(w + L.key_a);
-    g.buf.key_b = reinterpret_cast<uint32_t *>(w + L.key_b);
-    g.buf.idx_a = reinterpret_cast<uint32_t *>(w + L.idx_a);
-    g.buf.idx_b = reinterpret_cast<uint32_t *>(w + L.idx_b);
-    g.buf.status[0] = reinterpret_cast<uint32_t *>(w + L.status0);
-    g.buf.status[1] = reinterpret_cast<uint32_t *>(w + L.status1);
-    g.buf.sorted_pos = reinterpret_cast<float4 *>(w + L.sorted_pos);
-    g.buf.nodes = reinterpret_cast<int4 *>(w + L.nodes);
-    g.buf.parent = reinterpret_cast<int32_t *>(w + L.parent);
-    g.buf.slot = reinterpret_cast<uint4 *>(w + L.slot);
-    g.buf.groups = reinterpret_cast<uint2 *>(w + L.groups);
-    g.buf.entry = reinterpret_cast<int32_t *>(w + L.entry);
-    std::memcpy(g.box, box, sizeof(g.box));
-    float scale[3];
-    for (int d = 0; d < 3; ++d) {
-        volatile float s = 1023.0f / box[3 + d];   // fp32 RN
-        scale[d] = s;
-    }
-    for (int d = 0; d < 3; ++d) g.scale[d] = scale[d];
-    const int T = type ? g.T : 1;
-    // the meeting slots of tree_kernel carry a 24-bit build number; clear them when the layout moves or it wraps
-    if (g.build_tag == 0 || g.build_tag >= 0xFFFFFFu || g.tag_N != N) {
-        cudaError_t em = cudaMemsetAsync(g.buf.slot, 0, (size_t)16 * (size_t)(N > 0 ? N : 1), g.stream);
-        if (em != cudaSuccess) return cuda_fail(em, "memset slots");
-        g.build_tag = 0;
-        g.tag_N = N;
-    }
-    ++g.build_tag;
-    cudaError_t e = launch_build(pos, type, (int)N, T, g.K, box, scale, g.buf, g.build_tag, g.stream);
-    if (e != cudaSuccess) return cuda_fail(e, "build launch");
-    g.N = N;
-    g.K_built = g.K;
-    g.built = true;
     return QBVH_OK;
 }
 
@@ -367,18 +410,28 @@ int64_t qbvh_debug_export(int32_t what, void *dst, int64_t bytes) {
     int64_t avail = 0;
     int32_t segroots[10];
     switch (what) {
-        case QBVH_EXPORT_KEYS_SORTED: src = g.buf.key_a; avail = 4 * N; break;
-        case QBVH_EXPORT_PERM: src = g.buf.idx_a; avail = 4 * N; break;
+        case QBVH_EXPORT_KEYS_SORTED: src = g.buf.key_sorted; avail = 4 * N; break;
+        case QBVH_EXPORT_PERM: src = g.buf.idx_sorted; avail = 4 * N; break;
         case QBVH_EXPORT_NODES: src = g.buf.nodes; avail = N > 0 ? 16 * (2 * N - 1) : 0; break;
         case QBVH_EXPORT_PARENT: src = g.buf.parent; avail = N > 0 ? 4 * (2 * N - 1) : 0; break;
         case QBVH_EXPORT_FRAMES: src = g.buf.meta->frames; avail = sizeof(float) * QBVH_TMAX * 12; break;
         case QBVH_EXPORT_SORTED_POS: src = g.buf.sorted_pos; avail = 16 * N; break;
         case QBVH_EXPORT_SEGMENTS: avail = sizeof(segroots); break;
+        case QBVH_EXPORT_COUNTS: avail = 4 * sizeof(int32_t); break;
         default: return QBVH_ERR_INVALID_ARG;
     }
     cudaError_t e = cudaStreamSynchronize(g.stream);
     if (e != cudaSuccess) return cuda_fail(e, "export synchronize");
     const int64_t n = bytes < avail ? bytes : avail;
+    if (what == QBVH_EXPORT_COUNTS) {
+        int32_t c[4] = {0, 0, 0, g.lvl_built};
+        e = cudaMemcpy(&c[0], &g.buf.meta->nodes_emitted, sizeof(int32_t), cudaMemcpyDeviceToHost);
+        if (e == cudaSuccess) e = cudaMemcpy(&c[1], &g.buf.meta->group_count, sizeof(int32_t), cudaMemcpyDeviceToHost);
+        if (e == cudaSuccess) e = cudaMemcpy(&c[2], &g.buf.meta->ncell, sizeof(int32_t), cudaMemcpyDeviceToHost);
+        if (e != cudaSuccess) return cuda_fail(e, "export copy");
+        std::memcpy(dst, c, (size_t)n);
+        return avail;
+    }
     if (what == QBVH_EXPORT_SEGMENTS) {
         std::memset(segroots, 0, sizeof(segroots));
         e = cudaMemcpy(segroots, g.buf.meta->seg, sizeof(int32_t) * 5, cudaMemcpyDeviceToHost);

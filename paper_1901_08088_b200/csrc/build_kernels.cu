@@ -1,14 +1,19 @@
-// build_kernels.cu — steps a1..a6 of the hot path, hand-written for sm_100a.
-//   a1  morton_hist_kernel : Morton keys in the periodic box + digit histograms of all four
-//                            radix passes + per-type root AABB (the quantization frame); its last
-//                            block scans the histograms and writes type segments, roots and frames
-//   a2  onesweep_kernel    : stable LSD radix sort, 8-bit digits, one kernel per pass with chained-scan
-//                            decoupled look-back between tiles (the paper used CUB)
-//   a2'+a3+a4+a5+a6 tree_kernel : gather into Z-order; Karras binary radix tree built bottom up
-//                            with ropes in closed form; each leaf quantized onto the 1023-bin
-//                            grid of its tree's root box with outward rounding; boxes united
-//                            on the packed 10-bit integers while walking up with one 128-bit atomic hand-over
-//                            per node; entry table and query groups of the traversal
+// build_kernels.cu — steps a1..a6 of the hot path and the build-side subtree collapse (§8f NEXT-1),
+// hand-written for sm_100a.  Five launches:
+//   a1  morton_cell_kernel : Morton keys in the periodic box, per-type root AABB (the quantization
+//                            frame), occupancy of the Morton cells (the leading 2 + 3 lvl key bits)
+//       cell_scan_kernel   : exclusive scan of the cell occupancies (decoupled look-back); its last block writes type
+//                            segments, roots, frames
+//   a2  cell_scatter_kernel: most-significant-digit pass of the radix sort: every (key, index) goes to its cell
+//   a2..a6 cell_tree_kernel: one warp per cell: sorts the cell by (key, index) — the result is the stable sort of
+//                            gathers into Z-order, quantizes each particle onto the 1023-bin grid of
+//                            its tree's root box with outward rounding, and builds the cell's
+//                            subtree of Karras' radix tree bottom up in shared memory: hierarchy,
+//                            ropes in closed form, boxes united on the packed 10-bit integers
+//   a3..a6 top_tree_kernel : the tree above the cells: one thread per cell root walks up, the two children of a node
+//                            meet through one 128-bit atomic exchange ("atomic" hand-over)
+// Subtree collapse: a node is written only once it is known not to lie below a collapsed
+// range leaf; the choice is made bottom up by an integer cost model.
 #include "qbvh_internal.cuh"
 
 // ------------------------------------------------------------------------------------------------------------
@@ -31,102 +36,20 @@ __device__ __forceinline__ uint32_t morton_bin(float p, float lo, float s) {
     return (uint32_t)f;
 }
 
-// One block of MORTON_THREADS threads: histograms -> exclusive offsets; segments, roots, frames.  Run by the last
-// block of morton_hist_kernel to finish (threads 0..255 own one digit each).
-__device__ void finalize_block(TreeMeta *__restrict__ meta, int N, int warp_slots) {
-    __shared__ uint32_t s_scan[256];
-    __shared__ uint32_t s_ws[8];
-    const int d = threadIdx.x, lane = d & 31, warp = d >> 5;
-    for (int p = 0; p < 4; ++p) {
-        uint32_t c = 0, inc = 0;
-        if (d < 256) {
-            c = __ldcg(&meta->hist[p][d]);
-            inc = c;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                uint32_t v = __shfl_up_sync(0xFFFFFFFFu, inc, o);
-                if (lane >= o) inc += v;
-            }
-            if (lane == 31) s_ws[warp] = inc;
-        }
-        __syncthreads();
-        if (d < 256) {
-            uint32_t base = 0;
-            for (int w = 0; w < warp; ++w) base += s_ws[w];
-            uint32_t excl = base + inc - c;
-            meta->hist[p][d] = excl;
-            if (p == 3) s_scan[d] = excl;
-        }
-        __syncthreads();
-    }
-    if (d <= QBVH_TMAX) {
-        // type t owns top-digit values [64 t, 64 t + 63]
-        int s = (d < QBVH_TMAX) ? (int)s_scan[64 * d] : N;
-        meta->seg[d] = s;
-    }
-    __shared__ float s_rho[QBVH_TMAX];
-    __shared__ uint32_t s_scan_count[QBVH_TMAX];
-    if (d < QBVH_TMAX) {
-        int s = (int)s_scan[64 * d];
-        int e1 = (d + 1 < QBVH_TMAX) ? (int)s_scan[64 * (d + 1)] : N;
-        int n = e1 - s;
-        meta->roots[d] = (n <= 0) ? -1 : (n == 1 ? (N - 1 + s) : s);
-        float *fr = meta->frames[d];
-        float vol = 1.0f;
-        if (n > 0) {
-            for (int a = 0; a < 3; ++a) {
-                float lo = ord2f(~__ldcg(&meta->mm_enc[d][a]));
-                float hi = ord2f(__ldcg(&meta->mm_enc[d][3 + a]));
-                fr[a] = lo;
-                fr[3 + a] = hi;
-                // Delta = div_ru(sub_ru(hi, lo), 1023): the 1023-bin grid spans at least the root box
-                fr[6 + a] = __fdiv_ru(__fsub_ru(hi, lo), QBVH_NBINS);
-                vol *= hi - lo;
-            }
-        } else {
-            for (int a = 0; a < 9; ++a) fr[a] = 0.0f;
-        }
-        fr[9] = fr[10] = fr[11] = 0.0f;
-        s_rho[d] = (n > 1 && vol > 0.0f) ? (float)n / vol : 0.0f;    // unknown (flat or single): treated as dense
-        s_scan_count[d] = n > 0 ? (uint32_t)n : 0u;
-    }
-    __syncthreads();
-    // Query-group size per type.  One warp traverses for a whole group with the group's box as search volume, so
-    // the candidates it draws from a tree of number density rho_b grow with rho_b x (group size / rho_t): for a
-    // type far sparser than the densest one (the colloids of a colloid-solvent mixture, PAPER.md:45) a full group
-    // would sweep up thousands of misses.  Groups of type t hold at most 32 rho_t / rho_max particles (>= 1).
-    if (d < QBVH_TMAX) {
-        const float rmax = fmaxf(fmaxf(s_rho[0], s_rho[1]), fmaxf(s_rho[2], s_rho[3]));
-        int gm = GROUP_MAX;
-        if (s_rho[d] > 0.0f && rmax > 0.0f)
-            gm = (int)fminf(fmaxf(floorf((float)GROUP_MAX * s_rho[d] / rmax), 1.0f), (float)GROUP_MAX);
-        // Small systems (the regime of PAPER.md:186): with fewer groups than the device has resident warps the
-        // traversal is one group's latency, so groups shrink (down to 4) until there is about one per warp.
-        const int nt = (int)s_scan_count[d];
-        gm = min(gm, max(4, nt / max(warp_slots, 1)));
-        meta->gmax[d] = gm;
-    }
-}
-
 constexpr int MORTON_THREADS = 512;
 
-template <int NT>
-__global__ void __launch_bounds__(MORTON_THREADS) morton_hist_kernel(const float *__restrict__ pos,
+// PT = float: the paper's single-precision particle data.  PT = double (qbvh_build_f64,
+// PAPER.md:140, 154): the tree is built from the positions rounded to fp32; the exact leaf test stays in fp64.
+template <int NT, typename PT>
+__global__ void __launch_bounds__(MORTON_THREADS) morton_cell_kernel(const PT *__restrict__ pos,
                                                            const int32_t *__restrict__ type, int N, float3 lo,
-                                                           float3 scale, uint32_t *__restrict__ key_out,
+                                                           float3 scale, int cell_shift, uint32_t *__restrict__ key_out,
+                                                           uint32_t *__restrict__ cell_count,
                                                            TreeMeta *__restrict__ meta,
-                                                           uint32_t *__restrict__ status0, int status_words,
-                                                           int32_t *__restrict__ entry, int entry_words,
-                                                           int warp_slots) {
-    __shared__ uint32_t s_hist[4][256];
-    __shared__ bool s_last;
-    for (int i = threadIdx.x; i < 1024; i += blockDim.x) (&s_hist[0][0])[i] = 0;
-    __syncthreads();
+                                                           int32_t *__restrict__ entry, int entry_words) {
     const int stride = gridDim.x * blockDim.x;
     const int gtid = blockIdx.x * blockDim.x + threadIdx.x;
-    // the look-back status buffer of the first sort pass must be zero before that pass starts; the entry table of
-    // the traversal starts out empty (-1) and is filled by tree_kernel
-    for (int i = gtid; i < status_words; i += stride) status0[i] = 0;
+    // the entry table of the traversal starts out empty (-1) and is filled by the tree kernels
     for (int i = gtid; i < entry_words; i += stride) entry[i] = -1;
 
     float mn[NT][3], mx[NT][3];
@@ -147,10 +70,7 @@ __global__ void __launch_bounds__(MORTON_THREADS) morton_hist_kernel(const float
         uint32_t code = (spread10(morton_bin(x, lo.x, scale.x)) << 2) | (spread10(morton_bin(y, lo.y, scale.y)) << 1) |
                         spread10(morton_bin(z, lo.z, scale.z));
         uint32_t key = (t << 30) | code;
-        atomicAdd(&s_hist[0][key & 255u], 1u);
-        atomicAdd(&s_hist[1][(key >> 8) & 255u], 1u);
-        atomicAdd(&s_hist[2][(key >> 16) & 255u], 1u);
-        atomicAdd(&s_hist[3][key >> 24], 1u);
+        atomicAdd(&cell_count[key >> cell_shift], 1u);      // result unused: a fire-and-forget reduction in L2
 #pragma unroll
         for (int u = 0; u < NT; ++u) {
             bool m = (NT == 1) || (t == (uint32_t)u);
@@ -163,24 +83,28 @@ __global__ void __launch_bounds__(MORTON_THREADS) morton_hist_kernel(const float
         }
         return key;
     };
-    // four particles per thread and iteration: three 128-bit position loads, one 128-bit key store
-    const bool vec = ((reinterpret_cast<uintptr_t>(pos) & 15) == 0) && ((reinterpret_cast<uintptr_t>(key_out) & 15) == 0) &&
-                     (type == nullptr || (reinterpret_cast<uintptr_t>(type) & 15) == 0);
-    const int nquad = vec ? N / 4 : 0;
-    for (int q = gtid; q < nquad; q += stride) {
-        const float4 *p4 = reinterpret_cast<const float4 *>(pos) + 3 * (size_t)q;
-        const float4 a = __ldg(p4), b = __ldg(p4 + 1), c = __ldg(p4 + 2);
-        int4 tt = make_int4(0, 0, 0, 0);
-        if (type) tt = __ldg(reinterpret_cast<const int4 *>(type) + q);
-        uint4 k;
-        k.x = one(a.x, a.y, a.z, tt.x);
-        k.y = one(a.w, b.x, b.y, tt.y);
-        k.z = one(b.z, b.w, c.x, tt.z);
-        k.w = one(c.y, c.z, c.w, tt.w);
-        reinterpret_cast<uint4 *>(key_out)[q] = k;
+    int done = 0;
+    if (sizeof(PT) == 4) {
+        // four particles per thread and iteration: three 128-bit position loads, one 128-bit key store
+        const bool vec = ((reinterpret_cast<uintptr_t>(pos) & 15) == 0) && ((reinterpret_cast<uintptr_t>(key_out) & 15) == 0) &&
+                         (type == nullptr || (reinterpret_cast<uintptr_t>(type) & 15) == 0);
+        const int nquad = vec ? N / 4 : 0;
+        for (int q = gtid; q < nquad; q += stride) {
+            const float4 *p4 = reinterpret_cast<const float4 *>(pos) + 3 * (size_t)q;
+            const float4 a = __ldg(p4), b = __ldg(p4 + 1), c = __ldg(p4 + 2);
+            int4 tt = make_int4(0, 0, 0, 0);
+            if (type) tt = __ldg(reinterpret_cast<const int4 *>(type) + q);
+            uint4 k;
+            k.x = one(a.x, a.y, a.z, tt.x);
+            k.y = one(a.w, b.x, b.y, tt.y);
+            k.z = one(b.z, b.w, c.x, tt.z);
+            k.w = one(c.y, c.z, c.w, tt.w);
+            reinterpret_cast<uint4 *>(key_out)[q] = k;
+        }
+        done = 4 * nquad;
     }
-    for (int i = 4 * nquad + gtid; i < N; i += stride) {
-        const float x = pos[3 * (size_t)i + 0], y = pos[3 * (size_t)i + 1], z = pos[3 * (size_t)i + 2];
+    for (int i = done + gtid; i < N; i += stride) {
+        const float x = (float)pos[3 * (size_t)i + 0], y = (float)pos[3 * (size_t)i + 1], z = (float)pos[3 * (size_t)i + 2];
         key_out[i] = one(x, y, z, type ? type[i] : 0);
     }
     // per-type min/max: warp reduce on the order-preserving encoding, block reduce through shared memory, then one
@@ -205,205 +129,235 @@ __global__ void __launch_bounds__(MORTON_THREADS) morton_hist_kernel(const float
         if (v) atomicMax(&meta->mm_enc[0][0] + threadIdx.x, v);
     }
     if (bad_type) atomicOr(&meta->err_flags, 1);
-    __syncthreads();
-    for (int i = threadIdx.x; i < 1024; i += blockDim.x) {
-        uint32_t c = (&s_hist[0][0])[i];
-        if (c) atomicAdd(&meta->hist[0][0] + i, c);
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// Scan of the cell occupancies.  One tile of SCAN_TILE cells per block, tiles chained by decoupled look-back on one
+// 64-bit status word (at most SCAN_MAX_TILES = 128 blocks: all resident at once).  Writes cell_start (exclusive
+// prefix, cell_start[ncells] = N) and the ascending list of non-empty cells; the last block to finish turns the
+// per-type results into segments, roots and quantization frames.
+// ------------------------------------------------------------------------------------------------------------
+struct FinalizeParams {
+    int N, T, lvl, warp_slots;
+    float r_hint[QBVH_TMAX];
+};
+
+__device__ void finalize_block(TreeMeta *__restrict__ meta, const uint32_t *__restrict__ cell_start, const FinalizeParams fp) {
+    const int d = threadIdx.x;
+    __shared__ float s_rho[QBVH_TMAX];
+    __shared__ int s_cnt[QBVH_TMAX];
+    const int cpt = 1 << (3 * fp.lvl);              // cells per type
+    auto seg_of = [&](int t) -> int { return t < fp.T ? (int)__ldcg(cell_start + (size_t)t * cpt) : fp.N; };
+    if (d <= QBVH_TMAX) meta->seg[d] = seg_of(d);
+    if (d < QBVH_TMAX) {
+        const int s = seg_of(d), n = seg_of(d + 1) - s;
+        meta->roots[d] = (n <= 0) ? -1 : (n == 1 ? (fp.N - 1 + s) : s);
+        float *fr = meta->frames[d];
+        float vol = 1.0f;
+        int32_t *rb = meta->rbin[d];
+        rb[0] = rb[1] = rb[2] = rb[3] = -1;
+        if (n > 0) {
+            const float rh = fp.r_hint[d];
+            for (int a = 0; a < 3; ++a) {
+                float lo = ord2f(~__ldcg(&meta->mm_enc[d][a]));
+                float hi = ord2f(__ldcg(&meta->mm_enc[d][3 + a]));
+                fr[a] = lo;
+                fr[3 + a] = hi;
+                // Delta = div_ru(sub_ru(hi, lo), 1023): the 1023-bin grid spans at least the root box
+                const float delta = __fdiv_ru(__fsub_ru(hi, lo), QBVH_NBINS);
+                fr[6 + a] = delta;
+                fr[9 + a] = delta > 0.0f ? __fdiv_rn(1.0f, delta) : 0.0f;     // first guess of the quantizer only
+                vol *= hi - lo;
+                // expected query radius in bins of this axis (collapse cost model): ceil(r / Delta), fp32 RN division
+                if (rh > 0.0f) rb[a] = delta > 0.0f ? (int)fminf(ceilf(__fdiv_rn(rh, delta)), 1023.0f) : 1;
+            }
+        } else {
+            for (int a = 0; a < 12; ++a) fr[a] = 0.0f;
+        }
+        s_rho[d] = (n > 1 && vol > 0.0f) ? (float)n / vol : 0.0f;    // unknown (flat or single): treated as dense
+        s_cnt[d] = n > 0 ? n : 0;
     }
-    // the last block to get here turns the histograms into offsets (segments, roots, frames).  One cumulative
-    // fence by thread 0 after the barrier orders the whole block's atomics before its ticket.
     __syncthreads();
-    if (threadIdx.x == 0) {
+    // Query-group size per type.  One warp traverses for a whole group with the group's box as search volume, so
+    // the candidates it draws from a tree of number density rho_b grow with rho_b x (group size / rho_t): for a
+    // type far sparser than the densest one (the colloids of a colloid-solvent mixture, PAPER.md:45) a full group
+    // would sweep up thousands of misses.  Groups of type t hold at most 32 rho_t / rho_max particles (>= 1).
+    if (d < QBVH_TMAX) {
+        const float rmax = fmaxf(fmaxf(s_rho[0], s_rho[1]), fmaxf(s_rho[2], s_rho[3]));
+        int gm = GROUP_MAX;
+        if (s_rho[d] > 0.0f && rmax > 0.0f)
+            gm = (int)fminf(fmaxf(floorf((float)GROUP_MAX * s_rho[d] / rmax), 1.0f), (float)GROUP_MAX);
+        // Small systems (the regime of PAPER.md:186): with fewer groups than the device has resident warps the
+        // traversal is one group's latency, so groups shrink (down to 4) until there is about one per warp.
+        gm = min(gm, max(4, s_cnt[d] / max(fp.warp_slots, 1)));
+        meta->gmax[d] = gm;
+    }
+}
+
+constexpr unsigned long long SCAN_AGG = 1ull << 62, SCAN_PRE = 2ull << 62, SCAN_VAL = (1ull << 62) - 1;
+
+__global__ void __launch_bounds__(SCAN_THREADS) cell_scan_kernel(const uint32_t *__restrict__ cell_count,
+                                                                  uint32_t *__restrict__ cell_start,
+                                                                  uint32_t *__restrict__ cell_list, int ncells,
+                                                                  TreeMeta *__restrict__ meta, const FinalizeParams fp) {
+    __shared__ unsigned long long s_warp[SCAN_THREADS / 32];
+    __shared__ unsigned long long s_excl;
+    __shared__ bool s_last;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int tile = blockIdx.x;
+    const int c0 = tile * SCAN_TILE + tid * SCAN_IPT;
+    uint32_t cnt[SCAN_IPT];
+#pragma unroll
+    for (int u = 0; u < SCAN_IPT; ++u) cnt[u] = (c0 + u < ncells) ? __ldcg(cell_count + c0 + u) : 0u;
+    // value = count in the low word, number of non-empty cells in the high word
+    unsigned long long mine = 0;
+#pragma unroll
+    for (int u = 0; u < SCAN_IPT; ++u) mine += (unsigned long long)cnt[u] | ((unsigned long long)(cnt[u] != 0) << 32);
+    unsigned long long inc = mine;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const unsigned long long v = __shfl_up_sync(0xFFFFFFFFu, inc, o);
+        if (lane >= o) inc += v;
+    }
+    if (lane == 31) s_warp[warp] = inc;
+    __syncthreads();
+    unsigned long long wbase = 0, total = 0;
+#pragma unroll
+    for (int w = 0; w < SCAN_THREADS / 32; ++w) {
+        if (w < warp) wbase += s_warp[w];
+        total += s_warp[w];
+    }
+    if (tid == 0) {
+        volatile unsigned long long *status = meta->scan_status;
+        unsigned long long excl = 0;
+        if (tile == 0) {
+            status[0] = total | SCAN_PRE;
+        } else {
+            status[tile] = total | SCAN_AGG;
+            int p = tile - 1;
+            while (true) {
+                const unsigned long long v = status[p];
+                if (v & SCAN_PRE) {
+                    excl += v & SCAN_VAL;
+                    break;
+                }
+                if (v & SCAN_AGG) {
+                    excl += v & SCAN_VAL;
+                    --p;
+                }
+            }
+            status[tile] = (excl + total) | SCAN_PRE;
+        }
+        s_excl = excl;
+    }
+    __syncthreads();
+    unsigned long long run = s_excl + wbase + inc - mine;
+#pragma unroll
+    for (int u = 0; u < SCAN_IPT; ++u) {
+        if (c0 + u < ncells) {
+            cell_start[c0 + u] = (uint32_t)run;
+            if (cnt[u]) cell_list[(uint32_t)(run >> 32)] = (uint32_t)(c0 + u);
+        }
+        run += (unsigned long long)cnt[u] | ((unsigned long long)(cnt[u] != 0) << 32);
+    }
+    if (tile == (int)gridDim.x - 1 && tid == SCAN_THREADS - 1) {
+        cell_start[ncells] = (uint32_t)run;              // = N
+        meta->ncell = (int32_t)(run >> 32);
+    }
+    // the last block to get here finalizes.  One cumulative fence by thread 0 after the barrier orders the whole
+    // block's stores before its ticket.
+    __syncthreads();
+    if (tid == 0) {
         __threadfence();
-        s_last = atomicAdd(&meta->blocks_done, 1u) == gridDim.x - 1;
+        s_last = atomicAdd(&meta->scan_done, 1u) == gridDim.x - 1;
         __threadfence();
     }
     __syncthreads();
-    if (s_last) finalize_block(meta, N, warp_slots);
+    if (s_last) finalize_block(meta, cell_start, fp);
 }
 
 // N = 0: only the bookkeeping
-__global__ void __launch_bounds__(MORTON_THREADS) finalize_kernel(TreeMeta *__restrict__ meta, int N) {
-    finalize_block(meta, N, 1);
-}
-
-// ------------------------------------------------------------------------------------------------------------
-// a2. One pass of the LSD radix sort (8-bit digit).  A tile of 4096 keys per block; ranks inside a warp by
-// match_any, warps and digits combined by block scans, tiles chained by decoupled look-back on one status word
-// per (tile, digit).  Stable: ties keep their input order at every level.  FIRST: values are implicit (= index).
-// ------------------------------------------------------------------------------------------------------------
-template <bool FIRST>
-__global__ void __launch_bounds__(SORT_THREADS, 2) onesweep_kernel(const uint32_t *__restrict__ kin,
-                                                                    const uint32_t *__restrict__ vin,
-                                                                    uint32_t *__restrict__ kout,
-                                                                    uint32_t *__restrict__ vout, int N, int shift,
-                                                                    const uint32_t *__restrict__ hist_excl,
-                                                                    volatile uint32_t *status,
-                                                                    uint32_t *__restrict__ status_next,
-                                                                    uint32_t *__restrict__ tile_counter) {
-    // per-warp digit counters while ranking; the tile's keys in output order afterwards (same storage)
-    __shared__ __align__(16) uint32_t s_buf[SORT_TILE];
-    __shared__ uint32_t s_vals[SORT_TILE];
-    __shared__ uint32_t s_dstart[256];
-    __shared__ uint32_t s_gbase[256];
-    __shared__ uint32_t s_ws[8];
-    __shared__ uint32_t s_tile;
-    static_assert(SORT_WARPS * 256 <= SORT_TILE, "the per-warp counters live in the key buffer");
-    uint32_t(*s_whist)[256] = reinterpret_cast<uint32_t(*)[256]>(s_buf);
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    if (tid == 0) s_tile = atomicAdd(tile_counter, 1u);
-    for (int i = tid; i < SORT_WARPS * 256; i += SORT_THREADS) s_buf[i] = 0;
-    __syncthreads();
-    const uint32_t tile = s_tile;
-    const int base = (int)tile * SORT_TILE;
-    const int nvalid = min(SORT_TILE, N - base);
-    if (tid < 256) status_next[(size_t)tile * 256 + tid] = 0;   // the other buffer: used by the next pass, idle now
-
-    uint32_t key[SORT_IPT], val[SORT_IPT];
-    uint32_t rank[SORT_IPT];
-    const int wbase = warp * (32 * SORT_IPT);
-#pragma unroll
-    for (int r = 0; r < SORT_IPT; ++r) {
-        const int li = wbase + r * 32 + lane;
-        key[r] = (li < nvalid) ? kin[base + li] : 0xFFFFFFFFu;
-        val[r] = FIRST ? (uint32_t)(base + li) : ((li < nvalid) ? vin[base + li] : 0u);
-    }
-    // ranks inside the warp: lanes with the same digit find each other by match.any; the lowest of them bumps the
-    // warp's counter of that digit (shared-memory atomic) and hands the old value to the others.  Rounds are
-    // ordered by the warp-wide shuffle, so equal digits keep their input order (stability).
-    const uint32_t lt_mask = (1u << lane) - 1u;
-#pragma unroll
-    for (int r = 0; r < SORT_IPT; ++r) {
-        const int li = wbase + r * 32 + lane;
-        const bool valid = li < nvalid;
-        const uint32_t d = (key[r] >> shift) & 255u;
-        const uint32_t m = __match_any_sync(0xFFFFFFFFu, valid ? d : 256u);
-        uint32_t before = 0;
-        if (valid && (m & lt_mask) == 0) before = atomicAdd(&s_whist[warp][d], (uint32_t)__popc(m));
-        before = __shfl_sync(0xFFFFFFFFu, before, __ffs(m) - 1);
-        rank[r] = before + __popc(m & lt_mask);
-    }
-    __syncthreads();
-    // thread d owns digit d: exclusive scan over warps, then over digits, then over tiles (look-back)
-    if (tid < 256) {
-        const int d = tid;
-        uint32_t c[SORT_WARPS];
-#pragma unroll
-        for (int w = 0; w < SORT_WARPS; ++w) c[w] = s_whist[w][d];
-        uint32_t run = 0;
-#pragma unroll
-        for (int w = 0; w < SORT_WARPS; ++w) {
-            s_whist[w][d] = run;
-            run += c[w];
-        }
-        const uint32_t count = run;
-        if (tile == 0) status[d] = count | ST_PRE;
-        else status[(size_t)tile * 256 + d] = count | ST_AGG;
-        uint32_t inc = count;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            uint32_t v = __shfl_up_sync(0xFFFFFFFFu, inc, o);
-            if (lane >= o) inc += v;
-        }
-        if (lane == 31) s_ws[warp] = inc;
-        asm volatile("bar.sync 1, 256;");      // the eight warps that own digits
-        uint32_t wb = 0;
-        for (int w = 0; w < warp; ++w) wb += s_ws[w];
-        const uint32_t dstart = wb + inc - count;
-        s_dstart[d] = dstart;
-        uint32_t excl = 0;
-        if (tile != 0) {
-            // decoupled look-back, LB predecessors polled per round trip: all tiles of a pass are resident at once
-            // at these sizes, so the chain of prefixes advances LB tiles per L2 round trip
-            int p = (int)tile - 1;
-            bool done = false;
-            while (!done) {
-                constexpr int LB = 16;
-                uint32_t v[LB];
-#pragma unroll
-                for (int u = 0; u < LB; ++u) v[u] = (p - u >= 0) ? (uint32_t)status[(size_t)(p - u) * 256 + d] : (uint32_t)(1u << 31);
-#pragma unroll
-                for (int u = 0; u < LB; ++u) {
-                    if (done) continue;
-                    if (v[u] & ST_PRE) {
-                        excl += v[u] & ST_VAL;
-                        done = true;
-                    } else if (v[u] & ST_AGG) {
-                        excl += v[u] & ST_VAL;
-                        --p;
-                    } else {
-                        break;                 // not published yet: poll again from here
-                    }
-                }
-            }
-            status[(size_t)tile * 256 + d] = (excl + count) | ST_PRE;
-        }
-        s_gbase[d] = hist_excl[d] + excl - dstart;   // wraps mod 2^32; final index is exact
-    }
-    __syncthreads();
-    // position of every key inside the tile's output order
-#pragma unroll
-    for (int r = 0; r < SORT_IPT; ++r) {
-        const uint32_t d = (key[r] >> shift) & 255u;
-        rank[r] += s_dstart[d] + s_whist[warp][d];
-    }
-    __syncthreads();                                  // the counters are dead: their storage takes the keys
-#pragma unroll
-    for (int r = 0; r < SORT_IPT; ++r) {
-        const int li = wbase + r * 32 + lane;
-        if (li < nvalid) {
-            s_buf[rank[r]] = key[r];
-            s_vals[rank[r]] = val[r];
-        }
-    }
-    __syncthreads();
-    for (int p = tid; p < nvalid; p += SORT_THREADS) {
-        const uint32_t k = s_buf[p];
-        const uint32_t g = s_gbase[(k >> shift) & 255u] + (uint32_t)p;
-        kout[g] = k;
-        vout[g] = s_vals[p];
+__global__ void finalize_empty_kernel(TreeMeta *__restrict__ meta) {
+    const int d = threadIdx.x;
+    if (d <= QBVH_TMAX) meta->seg[d] = 0;
+    if (d < QBVH_TMAX) {
+        meta->roots[d] = -1;
+        meta->gmax[d] = GROUP_MAX;
+        for (int a = 0; a < 12; ++a) meta->frames[d][a] = 0.0f;
+        for (int a = 0; a < 4; ++a) meta->rbin[d][a] = -1;
     }
 }
 
 // ------------------------------------------------------------------------------------------------------------
-// a2' + a3 + a4 + a5 + a6 in ONE bottom-up pass (tree_kernel).  One thread per sorted position k.
-//
-// Hierarchy (PAPER.md:59,67: Karras' binary radix tree, "built bottom up"): every node covers a contiguous range
-// [f,l] of the sorted augmented keys (key, position).  With dL = delta(f-1,f) and dR = delta(l,l+1) the common
-// prefix lengths with the outside neighbours (-1 beyond the type segment), the node is the LEFT child of its
-// parent iff dR > dL, and then the parent splits at gamma = l; otherwise it is the RIGHT child and gamma = f-1.
-// (dL = dR only at the root, where both are -1.)  The two children of a parent meet at slot[gamma]: the first to
-// arrive leaves {its packed box, the far end of its range, its outer delta} there with ONE 128-bit atomic
-// exchange and retires; the second takes them, so it knows the parent's range, box and both outer deltas
-// without a single key load or search, writes the parent's 16-byte node and walks on ("walking up the
-// tree from the leaf nodes").  Slots are tagged with a per-build number instead of being cleared every build.
-// Numbering (pinned in tests/test_oracle_tree.py): a left child [f,gamma] is internal node gamma, a
-// right child [gamma+1,l] is internal node gamma+1, a root is the first position of its segment; leaf k is node
-// N-1+k.  Rope of a node covering [f,l]: END if l is the segment end, else with m = l+1:
-// internal node m if its range starts at m (delta(m,m+1) > delta(m,m-1)), else leaf m.
-//
-// Boxes (a5 + a6).  Quantizer defined by its decompressor:
+// a2, first pass: (key, index) of every particle to its cell.  The place inside the cell is arbitrary (one atomic
+// per set of lanes that share a cell: already Z-ordered input, common in MD, would otherwise hammer one address);
+// the cell is sorted by (key, index) afterwards, so the final order is the stable sort.  Counting down leaves the
+// counters at zero for the next build.
+// ------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) cell_scatter_kernel(const uint32_t *__restrict__ key, int N, int cell_shift,
+                                                            uint32_t *__restrict__ cell_count,
+                                                            const uint32_t *__restrict__ cell_start,
+                                                            uint2 *__restrict__ ent) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int lane = threadIdx.x & 31;
+    const bool valid = i < N;
+    const uint32_t k = valid ? key[i] : 0u;
+    const uint32_t c = valid ? (k >> cell_shift) : 0xFFFFFFFFu;
+    const uint32_t m = __match_any_sync(0xFFFFFFFFu, c);
+    const int leader = __ffs(m) - 1;
+    uint32_t base = 0;
+    if (valid && lane == leader) base = atomicSub(&cell_count[c], (uint32_t)__popc(m)) - (uint32_t)__popc(m);
+    base = __shfl_sync(0xFFFFFFFFu, base, leader);
+    if (valid) ent[__ldg(cell_start + c) + base + __popc(m & ((1u << lane) - 1u))] = make_uint2(k, (uint32_t)i);
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// Quantizer defined by its decompressor:
 //   D_lo(q) = fma_rd(q, Delta, lo)   D_hi(q) = fma_ru(q, Delta, lo)
-//   q_lo(a) = max{q : D_lo(q) <= a}  q_hi(b) = min{q : D_hi(q) >= b}     (bisection: D_lo, D_hi are monotone)
-// q_lo/q_hi are monotone, so the union of boxes is the per-field integer min/max of the packed words.
+//   q_lo(a) = max{q : D_lo(q) <= a}  q_hi(b) = min{q : D_hi(q) >= b}
+// D_lo and D_hi are monotone in q, so a first guess from (a - lo) / Delta is checked against its neighbours and,
+// should it be off by more than one (denormal Delta), replaced by the 10-step bisection.  q_lo, q_hi are monotone, so
+// the union of boxes is the per-field integer min/max of the packed words.
 // ------------------------------------------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t quant_lo(float a, float lo, float delta) {
+__device__ __noinline__ uint32_t quant_lo_bisect(float a, float lo, float delta) {
     uint32_t q = 0;
-#pragma unroll
     for (uint32_t bit = 512; bit; bit >>= 1) {
         uint32_t c = q | bit;
         if (__fmaf_rd((float)c, delta, lo) <= a) q = c;
     }
     return q;
 }
-__device__ __forceinline__ uint32_t quant_hi(float b, float lo, float delta) {
+__device__ __noinline__ uint32_t quant_hi_bisect(float b, float lo, float delta) {
     uint32_t q = 0;
-#pragma unroll
     for (uint32_t bit = 512; bit; bit >>= 1) {
         uint32_t c = q + bit;
         if (__fmaf_ru((float)(c - 1), delta, lo) < b) q = c;
     }
     return q;
+}
+__device__ __forceinline__ uint32_t quant_lo(float a, float lo, float delta, float inv) {
+    int q = (int)fminf(fmaxf(floorf(__fmul_rn(__fsub_rn(a, lo), inv)), 0.0f), 1023.0f);
+    if (__fmaf_rd((float)q, delta, lo) <= a) {
+        if (q == 1023 || __fmaf_rd((float)(q + 1), delta, lo) > a) return (uint32_t)q;
+        ++q;
+        if (q == 1023 || __fmaf_rd((float)(q + 1), delta, lo) > a) return (uint32_t)q;
+    } else if (q > 0) {
+        --q;
+        if (__fmaf_rd((float)q, delta, lo) <= a) return (uint32_t)q;
+    }
+    return quant_lo_bisect(a, lo, delta);
+}
+__device__ __forceinline__ uint32_t quant_hi(float b, float lo, float delta, float inv) {
+    int q = (int)fminf(fmaxf(ceilf(__fmul_rn(__fsub_rn(b, lo), inv)), 0.0f), 1023.0f);
+    if (__fmaf_ru((float)q, delta, lo) >= b) {
+        if (q == 0 || __fmaf_ru((float)(q - 1), delta, lo) < b) return (uint32_t)q;
+        --q;
+        if (q == 0 || __fmaf_ru((float)(q - 1), delta, lo) < b) return (uint32_t)q;
+    } else if (q < 1023) {
+        ++q;
+        if (__fmaf_ru((float)q, delta, lo) >= b) return (uint32_t)q;
+    }
+    return quant_hi_bisect(b, lo, delta);
 }
 __device__ __forceinline__ uint32_t pack_min(uint32_t a, uint32_t b) {
     return min(a & 0x3FFu, b & 0x3FFu) | min(a & 0xFFC00u, b & 0xFFC00u) | min(a & 0x3FF00000u, b & 0x3FF00000u);
@@ -432,156 +386,565 @@ __device__ __forceinline__ int delta_aug(uint32_t ka, int a, uint32_t kb, int b)
     return x ? __clz(x) : 32 + __clz((uint32_t)a ^ (uint32_t)b);
 }
 
-__global__ void __launch_bounds__(256) tree_kernel(const float *__restrict__ pos, const uint32_t *__restrict__ idx_sorted,
-                                                    const uint32_t *__restrict__ key, int N,
-                                                    TreeMeta *__restrict__ meta, float4 *__restrict__ sorted_pos,
-                                                    int4 *__restrict__ nodes, int32_t *__restrict__ parent,
-                                                    uint4 *__restrict__ slot, uint2 *__restrict__ groups,
-                                                    int32_t *__restrict__ entry, int K, uint32_t build_tag) {
-    const int k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= N) return;
-    const uint32_t ki = key[k];
-    const int t = ki >> 30;
-    const int s = meta->seg[t], e = meta->seg[t + 1] - 1;
-    const float *fr = meta->frames[t];
-    // ---- a2': gather into Z-order ----
-    const uint32_t idx = idx_sorted[k];
-    const float x = pos[3 * (size_t)idx], y = pos[3 * (size_t)idx + 1], z = pos[3 * (size_t)idx + 2];
-    sorted_pos[k] = make_float4(x, y, z, __uint_as_float(idx));
-    // ---- the leaf: outer deltas, rope, one-bin box ----
-    int dL = (k > s) ? delta_aug(ki, k, __ldg(key + k - 1), k - 1) : -1;
-    int dR = -1, rope = -1;
-    if (k < e) {
-        const uint32_t k1 = __ldg(key + k + 1);
-        dR = delta_aug(ki, k, k1, k + 1);
-        const int m = k + 1;
-        rope = (m <= e - 1 && delta_aug(k1, m, __ldg(key + m + 1), m + 1) > dR) ? m : N - 1 + m;
-    }
-    uint32_t wlo = quant_lo(x, fr[0], fr[6]) | (quant_lo(y, fr[1], fr[7]) << 10) | (quant_lo(z, fr[2], fr[8]) << 20);
-    uint32_t whi = quant_hi(x, fr[0], fr[6]) | (quant_hi(y, fr[1], fr[7]) << 10) | (quant_hi(z, fr[2], fr[8]) << 20);
-    nodes[N - 1 + k] = make_int4((int)wlo, (int)whi, ~k, rope);
-    if (k == e && k < N - 1) {                       // no internal node carries the index of a segment end
-        nodes[k] = make_int4(0, 0, 0, -1);
-        parent[k] = -1;
-    }
-    // Entry table of the traversal.  The upper levels of an LBVH over Morton codes ARE a regular grid: all
-    // particles whose code starts with a given 3l-bit prefix (one cell of the 2^l-per-axis grid over the box,
-    // PAPER.md:61) form one subtree.  A node whose keys share `dnode` leading bits while its parent's share
-    // only `dpar` roots the cell of every level l with dpar < 2 + 3 l <= dnode (2 type bits, then the code).
-    int32_t *const etab = entry + t * ENTRY_CELLS;
-    auto emit_entry = [&](int dpar, int dnode, int node) {
-        if (dpar >= 2 + 3 * ENTRY_LMAX || dnode < 2 + 3 * ENTRY_LMIN) return;   // below or above every grid level
-#pragma unroll
-        for (int l = ENTRY_LMIN; l <= ENTRY_LMAX; ++l) {
-            const int need = 2 + 3 * l;
-            if (dpar < need && need <= dnode) etab[entry_offset(l) + (int)((ki & 0x3FFFFFFFu) >> (30 - 3 * l))] = node;
-        }
-    };
-    // query groups (maximal subtrees with <= gmax[type] leaves): appended with one atomic per converged set of lanes
-    const int gmax = meta->gmax[t];
-    auto emit_groups = [&](uint2 g0, uint2 g1, int n) {
-        const uint32_t act = __activemask();
-        const uint32_t two = __ballot_sync(act, n >= 2);
-        const int lane = threadIdx.x & 31;
-        const uint32_t lt = (1u << lane) - 1u;
-        const int leader = __ffs(act) - 1;
-        int base = 0;
-        if (lane == leader) base = atomicAdd(&meta->group_count, __popc(act) + __popc(two));
-        base = __shfl_sync(act, base, leader) + __popc(act & lt) + __popc(two & lt);
-        groups[base] = g0;
-        if (n >= 2) groups[base + 1] = g1;
-    };
-    emit_entry(max(dL, dR), 64, N - 1 + k);
+// ------------------------------------------------------------------------------------------------------------
+// What both tree kernels share.
+//
+// Hierarchy (PAPER.md:59,67: Karras' binary radix tree, "built bottom up"): every node covers a contiguous range
+// [f,l] of the sorted augmented keys (key, position).  With dL = delta(f-1,f) and dR = delta(l,l+1) the common
+// prefix lengths with the outside neighbours (-1 beyond the type segment), the node is the LEFT child of its
+// parent iff dR > dL, and then the parent splits at gamma = l; otherwise it is the RIGHT child and gamma = f-1.
+// (dL = dR only at a root, where both are -1.)  Numbering (pinned in tests/test_oracle_tree.py): a
+// left child [f,gamma] is internal node gamma, a right child [gamma+1,l] is internal node gamma+1, a root is the
+// first position of its segment; leaf k is node N-1+k.  Rope: a left child's rope is its right
+// sibling; a right child's rope is its parent's; for a node covering [f,l] in closed form: END if l is the segment
+// end, else with m = l+1: internal node m if its range starts at m (delta(m,m+1) > delta(m,m-1)), else leaf m.
+//
+// Collapse.  A node is PENDING while it may still end up inside a range leaf:
+// single particles, and nodes that chose to collapse.  A pending node is not written; the thread that forms its
+// parent either collapses the parent too (the children vanish) or writes the parent and, as leaves, its pending
+// children.  A node may collapse only if both children are pending, so a written node is never below a leaf.
+// ------------------------------------------------------------------------------------------------------------
+struct TreeCtx {
+    const void *pos;
+    int f64;
+    int N, K, lvl;
+    uint32_t build_tag;
+    const uint32_t *cell_start, *cell_list;
+    uint2 *ent;
+    uint32_t *key_sorted, *idx_sorted;
+    float4 *sorted_pos;
+    Pos64 *sorted_pos64;
+    int4 *nodes;
+    int32_t *parent;
+    uint4 *slot;
+    uint2 *groups;
+    int32_t *entry;
+    int32_t *big_list;
+    CellRoot *croot;
+    unsigned char *scratch;
+    TreeMeta *meta;
+};
 
-    // ---- walk up ----
-    int f = k, l = k, cur = N - 1 + k;
-    while (true) {
-        if (dL < 0 && dR < 0) {                      // the root of this type's tree
-            parent[cur] = -1;
-            if (l - f + 1 <= gmax) emit_groups(make_uint2((uint32_t)f, (uint32_t)(l - f + 1)), make_uint2(0u, 0u), 1);
-            break;
-        }
-        const bool is_left = dR > dL;
-        const int gamma = is_left ? l : f - 1;
-        const uint4 mine = make_uint4(wlo, whi, (uint32_t)(is_left ? f : l), (build_tag << 8) | (uint32_t)((is_left ? dL : dR) + 1));
-        const uint4 other = exch128(slot + gamma, mine);
-        if ((other.w >> 8) != build_tag) break;      // first to arrive: the sibling will carry on
-        const int dsplit = is_left ? dR : dL;        // delta(gamma, gamma+1): the parent's own prefix length
-        if (is_left) {
-            l = (int)other.z;
-            dR = (int)(other.w & 255u) - 1;
-        } else {
-            f = (int)other.z;
-            dL = (int)(other.w & 255u) - 1;
-        }
-        wlo = pack_min(wlo, other.x);
-        whi = pack_max(whi, other.y);
-        const int lsize = gamma - f + 1, rsize = l - gamma, size = l - f + 1;
-        const int lc = (lsize == 1) ? (N - 1 + gamma) : gamma;
-        const int rc = (rsize == 1) ? (N + gamma) : (gamma + 1);
-        const int id = (dL < 0 && dR < 0) ? s : (dR > dL ? l : f);
-        parent[lc] = id;
-        parent[rc] = id;
-        int nrope = -1;
-        if (l < e) {
-            const int m = l + 1;
-            nrope = (m <= e - 1 && delta_aug(__ldg(key + m), m, __ldg(key + m + 1), m + 1) > dR) ? m : N - 1 + m;
-        }
-        const int leftword = (K > 1 && size <= K) ? ~f : lc;      // collapsed range leaf: first sorted position
-        nodes[id] = make_int4((int)wlo, (int)whi, leftword, nrope);
-        emit_entry(max(dL, dR), dsplit, id);
-        if (size > gmax) {                           // children that fit are maximal: they become groups
-            const int nl = lsize <= gmax, nr = rsize <= gmax;
-            if (nl + nr) {
-                const uint2 gl = make_uint2((uint32_t)f, (uint32_t)lsize), gr = make_uint2((uint32_t)(gamma + 1), (uint32_t)rsize);
-                emit_groups(nl ? gl : gr, gr, nl + nr);
-            }
-        }
-        cur = id;
+struct Child {
+    uint32_t wlo, whi;   // packed box (30 bits each)
+    int f, l;            // sorted positions covered
+    bool pend;
+};
+
+__device__ __forceinline__ unsigned long long swollen(uint32_t wlo, uint32_t whi, const int32_t *rb) {
+    unsigned long long w = 1;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        const int ext = max((int)((whi >> (10 * d)) & 1023u) - (int)((wlo >> (10 * d)) & 1023u), 0);   // zero-extent frames invert the codes (R10)
+        w *= (unsigned long long)(ext + 2 * rb[d]);
+    }
+    return w;
+}
+__device__ __forceinline__ unsigned long long leaf_cost(unsigned long long w, int cnt) {
+    return w * (unsigned long long)(COST_LEAF_FIXED + COST_LEAF_PER_PARTICLE * cnt);
+}
+
+// Entry table of the traversal.  The upper levels of an LBVH over Morton codes ARE a regular grid: all particles
+// whose code starts with a given 3l-bit prefix (one cell of the 2^l-per-axis grid over the box) form
+// one subtree.  A node whose keys share `dnode` leading bits while its parent's share only `dpar` roots the cell
+// of every level l with dpar < 2 + 3 l <= dnode (2 type bits, then the code).
+__device__ __forceinline__ void emit_entry(int32_t *__restrict__ etab, uint32_t ki, int dpar, int dnode, int node) {
+    if (dpar >= 2 + 3 * ENTRY_LMAX || dnode < 2 + 3 * ENTRY_LMIN) return;   // below or above every grid level
+#pragma unroll
+    for (int l = ENTRY_LMIN; l <= ENTRY_LMAX; ++l) {
+        const int need = 2 + 3 * l;
+        if (dpar < need && need <= dnode) etab[entry_offset(l) + (int)((ki & 0x3FFFFFFFu) >> (30 - 3 * l))] = node;
     }
 }
 
+// A range leaf covering sorted positions [f, l] (dnode = common prefix length of its keys): on grid levels finer than
+// the leaf itself no node below it exists any more, so the leaf roots every cell of those levels that holds one of
+// its particles (the traversal drops the duplicates among its entry nodes).
+template <class KeyF>
+__device__ __forceinline__ void emit_entry_leaf(int32_t *__restrict__ etab, KeyF keyat, int f, int l, int dpar, int dnode, int node) {
+    if (dpar >= 2 + 3 * ENTRY_LMAX) return;
+    const uint32_t kf = keyat(f);
+    emit_entry(etab, kf, dpar, dnode, node);
+#pragma unroll 1
+    for (int lv = ENTRY_LMIN; lv <= ENTRY_LMAX; ++lv) {
+        const int need = 2 + 3 * lv;
+        if (dpar < need && need > dnode)
+            for (int k = f; k <= l; ++k) etab[entry_offset(lv) + (int)((keyat(k) & 0x3FFFFFFFu) >> (30 - 3 * lv))] = node;
+    }
+}
+
+// query groups (maximal subtrees with <= gmax leaves): appended with one atomic per converged set of lanes
+__device__ __forceinline__ void emit_groups(TreeMeta *meta, uint2 *__restrict__ groups, uint2 g0, uint2 g1, int n) {
+    const uint32_t act = __activemask();
+    const uint32_t two = __ballot_sync(act, n >= 2);
+    const int lane = threadIdx.x & 31;
+    const uint32_t lt = (1u << lane) - 1u;
+    const int leader = __ffs(act) - 1;
+    int base = 0;
+    if (lane == leader) base = atomicAdd(&meta->group_count, __popc(act) + __popc(two));
+    base = __shfl_sync(act, base, leader) + __popc(act & lt) + __popc(two & lt);
+    groups[base] = g0;
+    if (n >= 2) groups[base + 1] = g1;
+}
+
+// Form the parent of the adjacent children a (left) and b (right).  dL, dR: the parent's outer prefix lengths;
+// dsplit = delta(a.l, b.f): the parent's own prefix length.  rope_p: the parent's rope (and b's).  pfx(f, l): common
+// prefix length of the keys at sorted positions f and l.  Returns whether the parent is pending; ulo/uhi: its box.
+// keyat(k): key at sorted position k (asked only for a.f and for the first position of a pending child).
+template <class KeyF, class PfxF>
+__device__ __forceinline__ bool form_parent(const TreeCtx &cx, int t, int s_seg, int gmax, const int32_t *rb, KeyF keyat,
+                                            const Child a, const Child b, int dL, int dR, int dsplit, int rope_p, PfxF pfx,
+                                            uint32_t &ulo, uint32_t &uhi, int &written) {
+    const int N = cx.N;
+    ulo = pack_min(a.wlo, b.wlo);
+    uhi = pack_max(a.whi, b.whi);
+    const int ca = a.l - a.f + 1, cb = b.l - b.f + 1, cnt = ca + cb;
+    bool collapse = cx.K > 1 && cnt <= cx.K && a.pend && b.pend;
+    if (collapse && rb[0] >= 0) {
+        const unsigned long long wp = swollen(ulo, uhi, rb);
+        collapse = leaf_cost(wp, cnt) <=
+                   wp * (unsigned long long)COST_NODE + leaf_cost(swollen(a.wlo, a.whi, rb), ca) + leaf_cost(swollen(b.wlo, b.whi, rb), cb);
+    }
+    const bool root = dL < 0 && dR < 0;
+    if (!collapse) {
+        const int id = root ? s_seg : (dR > dL ? b.l : a.f);
+        const int lc = ca == 1 ? N - 1 + a.f : a.l;
+        const int rc = cb == 1 ? N - 1 + b.f : b.f;
+        cx.nodes[id] = make_int4((int)ulo, (int)uhi, lc, rope_p);
+        cx.parent[lc] = id;
+        cx.parent[rc] = id;
+        if (root) cx.parent[id] = -1;
+        int32_t *const etab = cx.entry + t * ENTRY_CELLS;
+        if (max(dL, dR) < 2 + 3 * ENTRY_LMAX) emit_entry(etab, keyat(a.f), max(dL, dR), dsplit, id);
+        written = 1;
+        if (a.pend) {
+            cx.nodes[lc] = make_int4((int)a.wlo, (int)a.whi, ~a.f, rc);
+            if (dsplit < 2 + 3 * ENTRY_LMAX) emit_entry_leaf(etab, keyat, a.f, a.l, dsplit, ca == 1 ? 64 : pfx(a.f, a.l), lc);
+            ++written;
+        }
+        if (b.pend) {
+            cx.nodes[rc] = make_int4((int)b.wlo, (int)b.whi, ~b.f, rope_p);
+            if (dsplit < 2 + 3 * ENTRY_LMAX) emit_entry_leaf(etab, keyat, b.f, b.l, dsplit, cb == 1 ? 64 : pfx(b.f, b.l), rc);
+            ++written;
+        }
+    }
+    if (cnt > gmax) {                            // children that fit are maximal: they become query groups
+        const int nl = ca <= gmax, nr = cb <= gmax;
+        if (nl + nr) {
+            const uint2 gl = make_uint2((uint32_t)a.f, (uint32_t)ca), gr = make_uint2((uint32_t)b.f, (uint32_t)cb);
+            emit_groups(cx.meta, cx.groups, nl ? gl : gr, gr, nl + nr);
+        }
+    }
+    return collapse;
+}
+
+// common prefix length of two cells' keys (cell ids carry the type bits); -1 across types
+__device__ __forceinline__ int delta_cells(uint32_t ca, uint32_t cb, int lvl) {
+    if ((ca >> (3 * lvl)) != (cb >> (3 * lvl))) return -1;
+    return __clz((ca ^ cb) << (30 - 3 * lvl));
+}
+
+// The root of a type's tree that is still pending (a single particle, or everything collapsed): written as a leaf.
+template <class KeyF>
+__device__ __forceinline__ void write_pending_root(const TreeCtx &cx, int t, KeyF keyat, const Child me, int pfx_me) {
+    const int id = (me.l == me.f) ? cx.N - 1 + me.f : me.f;      // = meta->roots[t]
+    cx.nodes[id] = make_int4((int)me.wlo, (int)me.whi, ~me.f, -1);
+    cx.parent[id] = -1;
+    emit_entry_leaf(cx.entry + t * ENTRY_CELLS, keyat, me.f, me.l, -1, pfx_me, id);
+}
+
+// Walk up from a finished subtree (a cell root) through the levels above the cells.  The two children of a node meet at
+// slot[gamma]: the first to arrive leaves {its packed box + pending bit, the far end of its range, its outer delta,
+// the build's tag} there with ONE 128-bit atomic exchange and retires; the second takes them and forms the parent
+// ("walking up the tree from the leaf nodes").  Slots are tagged with a per-build number instead of being
+// cleared every build.  A node up here covers whole cells, so its rope follows from the cell table alone (jl: compact
+// index of its last cell): no key of a neighbouring cell is read, which may still be sorting in this very launch.  A
+// right child's "far end" travels as jl (its last position is that cell's end), a left child's as its first position.
+__device__ void walk_up(const TreeCtx &cx, Child me, int dL, int dR, int jl) {
+    const uint32_t *key = cx.key_sorted;
+    const uint32_t ki = key[me.f];
+    const int t = ki >> 30;
+    const int s_seg = cx.meta->seg[t];
+    const int gmax = cx.meta->gmax[t];
+    const int ncell = cx.meta->ncell;
+    const int32_t *rb = cx.meta->rbin[t];
+    auto keyat = [&](int k) { return key[k]; };           // asked for pending children only: small cells, sorted by the previous launch
+    auto pfx = [&](int f, int l) { return delta_aug(key[f], f, key[l], l); };
+    int written = 0;
+    while (true) {
+        if (dL < 0 && dR < 0) {                      // the root of this type's tree
+            if (me.pend) {
+                write_pending_root(cx, t, keyat, me, me.l == me.f ? 64 : pfx(me.f, me.l));
+                ++written;
+            }
+            if (me.l - me.f + 1 <= gmax) emit_groups(cx.meta, cx.groups, make_uint2((uint32_t)me.f, (uint32_t)(me.l - me.f + 1)), make_uint2(0u, 0u), 1);
+            break;
+        }
+        const bool is_left = dR > dL;
+        const int gamma = is_left ? me.l : me.f - 1;
+        const uint4 mine = make_uint4(me.wlo | (me.pend ? 0x80000000u : 0u), me.whi, (uint32_t)(is_left ? me.f : jl),
+                                      (cx.build_tag << 8) | (uint32_t)((is_left ? dL : dR) + 1));
+        const uint4 other = exch128(cx.slot + gamma, mine);
+        if ((other.w >> 8) != cx.build_tag) break;   // first to arrive: the sibling will carry on
+        const int dsplit = is_left ? dR : dL;        // delta(gamma, gamma+1): the parent's own prefix length
+        Child sib;
+        sib.wlo = other.x & 0x7FFFFFFFu;
+        sib.whi = other.y;
+        sib.pend = (other.x >> 31) != 0;
+        Child a, b;
+        if (is_left) {
+            jl = (int)other.z;
+            sib.f = gamma + 1;
+            sib.l = (int)__ldg(cx.cell_start + __ldg(cx.cell_list + jl) + 1) - 1;
+            dR = (int)(other.w & 255u) - 1;
+            a = me, b = sib;
+        } else {
+            sib.f = (int)other.z;
+            sib.l = gamma;
+            dL = (int)(other.w & 255u) - 1;
+            a = sib, b = me;
+        }
+        int rope_p = -1;
+        if (dR >= 0) {                               // another cell of this type follows: what starts at m = b.l + 1?
+            const int m = b.l + 1;
+            const uint32_t cn = __ldg(cx.cell_list + jl + 1);
+            int dnext = 64;                          // two or more particles in that cell: internal node m starts there
+            if (__ldg(cx.cell_start + cn + 1) - __ldg(cx.cell_start + cn) == 1u)
+                dnext = (jl + 2 < ncell) ? delta_cells(cn, __ldg(cx.cell_list + jl + 2), cx.lvl) : -1;
+            rope_p = dnext > dR ? m : cx.N - 1 + m;
+        }
+        uint32_t ulo, uhi;
+        int w = 0;
+        const bool pend = form_parent(cx, t, s_seg, gmax, rb, keyat, a, b, dL, dR, dsplit, rope_p, pfx, ulo, uhi, w);
+        written += w;
+        me.wlo = ulo, me.whi = uhi, me.f = a.f, me.l = b.l, me.pend = pend;
+    }
+    if (written) atomicAdd(&cx.meta->nodes_emitted, written);
+}
+
 // ------------------------------------------------------------------------------------------------------------
-cudaError_t launch_build(const float *pos, const int32_t *type, int N, int T, int K, const float *box_lo,
-                         const float *box_scale, const BuildBuffers &b, uint32_t build_tag, cudaStream_t st) {
+// One cell: G cooperating threads (a warp, or a whole block for a cell too large for a warp's shared memory).
+// Working arrays of length >= the next power of two of n: in shared memory, or for giant cells in global scratch.
+// ------------------------------------------------------------------------------------------------------------
+struct CellArrays {
+    unsigned long long *kv;   // (key << 32 | original index): sorted ascending = Z-order, ties by index
+    int32_t *e;               // at a segment's first position: its last position; -1 elsewhere
+    int32_t *mrg;             // merge partner chosen in the current round, -1: none
+    uint32_t *wlo, *whi;      // packed box of the segment; bit 31 of wlo: pending
+    int8_t *dL, *dR;          // outer prefix lengths of the segment
+};
+constexpr int CELL_BYTES_PER_SLOT = 8 + 4 + 4 + 4 + 4 + 1 + 1;   // 26
+
+__device__ __forceinline__ CellArrays carve_cell_arrays(unsigned char *base, int cap) {
+    CellArrays A;
+    A.kv = reinterpret_cast<unsigned long long *>(base);
+    A.e = reinterpret_cast<int32_t *>(base + 8 * (size_t)cap);
+    A.mrg = A.e + cap;
+    A.wlo = reinterpret_cast<uint32_t *>(A.mrg + cap);
+    A.whi = A.wlo + cap;
+    A.dL = reinterpret_cast<int8_t *>(A.whi + cap);
+    A.dR = A.dL + cap;
+    return A;
+}
+
+template <int G>
+__device__ __forceinline__ void coop_sync() {
+    if (G == 32) __syncwarp();
+    else __syncthreads();
+}
+
+// Batcher's odd-even merge sort over kv[0..n): every comparator moves the smaller value to the lower index, so
+// positions >= n act as +infinity without being stored (their comparators are skipped).
+template <int G>
+__device__ void sort_cell(unsigned long long *kv, int n, int rank) {
+    int P = 1;
+    while (P < n) P <<= 1;
+    auto cmpx = [&](int i, int j) {
+        if (j < n) {
+            const unsigned long long x = kv[i], y = kv[j];
+            if (y < x) {
+                kv[i] = y;
+                kv[j] = x;
+            }
+        }
+    };
+    for (int size = 2; size <= P; size <<= 1) {
+        int stride = size >> 1;
+        coop_sync<G>();
+        for (int tq = rank; tq < (P >> 1); tq += G) {
+            const int pos = 2 * tq - (tq & (stride - 1));
+            cmpx(pos, pos + stride);
+        }
+        for (stride >>= 1; stride > 0; stride >>= 1) {
+            coop_sync<G>();
+            for (int tq = rank; tq < (P >> 1); tq += G) {
+                const int pos = 2 * tq - (tq & (stride - 1));
+                const int offset = tq & ((size >> 1) - 1);
+                if (offset >= stride) cmpx(pos - stride, pos);
+            }
+        }
+    }
+    coop_sync<G>();
+}
+
+template <int G>
+__device__ void process_cell(const TreeCtx &cx, const CellArrays A, int j, int rank, bool kv_is_ent) {
+    const int N = cx.N, lvl = cx.lvl;
+    const int ncell = cx.meta->ncell;
+    const uint32_t c = __ldg(cx.cell_list + j);
+    const int F = (int)__ldg(cx.cell_start + c);
+    const int n = (int)__ldg(cx.cell_start + c + 1) - F;
+    const int t = (int)(c >> (3 * lvl));
+    const int s_seg = cx.meta->seg[t], e_seg = cx.meta->seg[t + 1] - 1;
+    const int gmax = cx.meta->gmax[t];
+    const int32_t *rb = cx.meta->rbin[t];
+    // neighbouring cells: outer prefix lengths of the cell, and what starts right after it
+    int dLc = -1, dRc = -1, dNN = -1, n_next = 0;
+    if (j > 0) dLc = delta_cells(__ldg(cx.cell_list + j - 1), c, lvl);
+    if (j + 1 < ncell) {
+        const uint32_t cn = __ldg(cx.cell_list + j + 1);
+        dRc = delta_cells(c, cn, lvl);
+        if (dRc >= 0) {
+            n_next = (int)(__ldg(cx.cell_start + cn + 1) - __ldg(cx.cell_start + cn));
+            if (j + 2 < ncell) dNN = delta_cells(cn, __ldg(cx.cell_list + j + 2), lvl);
+        }
+    }
+    // ---- a2: sort the cell by (key, index) ----
+    if (!kv_is_ent)
+        for (int p = rank; p < n; p += G) {
+            const uint2 e = cx.ent[F + p];
+            A.kv[p] = ((unsigned long long)e.x << 32) | e.y;
+        }
+    sort_cell<G>(A.kv, n, rank);
+    const float *fr = cx.meta->frames[t];
+    // ---- a2' gather, a6 quantize, leaf state ----
+    for (int p = rank; p < n; p += G) {
+        const unsigned long long kvp = A.kv[p];
+        const uint32_t ki = (uint32_t)(kvp >> 32), idx = (uint32_t)kvp;
+        const int k = F + p;
+        cx.key_sorted[k] = ki;
+        cx.idx_sorted[k] = idx;
+        float x, y, z;
+        if (cx.f64) {
+            const double *pp = static_cast<const double *>(cx.pos) + 3 * (size_t)idx;
+            const double xd = pp[0], yd = pp[1], zd = pp[2];
+            Pos64 q;
+            q.x = xd, q.y = yd, q.z = zd, q.idx = (long long)idx;
+            cx.sorted_pos64[k] = q;
+            x = (float)xd, y = (float)yd, z = (float)zd;
+        } else {
+            const float *pp = static_cast<const float *>(cx.pos) + 3 * (size_t)idx;
+            x = pp[0], y = pp[1], z = pp[2];
+        }
+        cx.sorted_pos[k] = make_float4(x, y, z, __uint_as_float(idx));
+        const uint32_t wlo = quant_lo(x, fr[0], fr[6], fr[9]) | (quant_lo(y, fr[1], fr[7], fr[10]) << 10) | (quant_lo(z, fr[2], fr[8], fr[11]) << 20);
+        const uint32_t whi = quant_hi(x, fr[0], fr[6], fr[9]) | (quant_hi(y, fr[1], fr[7], fr[10]) << 10) | (quant_hi(z, fr[2], fr[8], fr[11]) << 20);
+        A.wlo[p] = wlo | 0x80000000u;                    // a single particle is pending
+        A.whi[p] = whi;
+        A.e[p] = p;
+        A.dL[p] = (int8_t)(p > 0 ? delta_aug(ki, k, (uint32_t)(A.kv[p - 1] >> 32), k - 1) : dLc);
+        A.dR[p] = (int8_t)(p < n - 1 ? delta_aug(ki, k, (uint32_t)(A.kv[p + 1] >> 32), k + 1) : dRc);
+        if (k == e_seg && k < N - 1) {                   // no internal node carries the index of a segment end
+            cx.nodes[k] = make_int4(0, 0, 0, -1);
+            cx.parent[k] = -1;
+        }
+    }
+    coop_sync<G>();
+    // rope of a node whose last particle is local position l (dcur = delta(l, l+1), the node's dR)
+    auto rope_of = [&](int l, int dcur) -> int {
+        if (F + l >= e_seg) return -1;
+        const int m = l + 1;
+        int dnext;
+        if (m <= n - 2) dnext = delta_aug((uint32_t)(A.kv[m] >> 32), F + m, (uint32_t)(A.kv[m + 1] >> 32), F + m + 1);
+        else if (m == n - 1) dnext = dRc;
+        else dnext = n_next >= 2 ? 64 : dNN;             // m = first particle of the next cell
+        return dnext > dcur ? F + m : N - 1 + F + m;
+    };
+    auto keyat = [&](int k) { return (uint32_t)(A.kv[k - F] >> 32); };
+    auto pfx = [&](int f, int l) { return delta_aug(keyat(f), f, keyat(l), l); };
+    // ---- a3..a6 inside the cell: rounds of merges.  A segment that is a left child (dR > dL) merges with the segment
+    //      that starts right after it if that one is a right child: then they are siblings.  Height of the cell's
+    //      subtree rounds; no atomics. ----
+    int written = 0;
+    while (A.e[0] != n - 1) {
+        for (int p = rank; p < n; p += G) {
+            int partner = -1;
+            const int ep = A.e[p];
+            if (ep >= 0 && ep < n - 1 && A.dR[p] > A.dL[p]) {
+                const int s = ep + 1;
+                if (!(A.dR[s] > A.dL[s])) partner = s;   // s starts a segment (it follows one) and is a right child
+            }
+            A.mrg[p] = partner;
+        }
+        coop_sync<G>();
+        for (int p = rank; p < n; p += G) {
+            const int s = A.mrg[p];
+            if (s < 0) continue;
+            Child a, b;
+            a.wlo = A.wlo[p] & 0x7FFFFFFFu, a.whi = A.whi[p], a.f = F + p, a.l = F + A.e[p], a.pend = (A.wlo[p] >> 31) != 0;
+            b.wlo = A.wlo[s] & 0x7FFFFFFFu, b.whi = A.whi[s], b.f = F + s, b.l = F + A.e[s], b.pend = (A.wlo[s] >> 31) != 0;
+            const int dL = A.dL[p], dR = A.dR[s], dsplit = A.dR[p];
+            uint32_t ulo, uhi;
+            int w = 0;
+            const bool pend = form_parent(cx, t, s_seg, gmax, rb, keyat, a, b, dL, dR, dsplit, rope_of(b.l - F, dR), pfx,
+                                          ulo, uhi, w);
+            written += w;
+            A.wlo[p] = ulo | (pend ? 0x80000000u : 0u);
+            A.whi[p] = uhi;
+            A.e[p] = b.l - F;
+            A.dR[p] = (int8_t)dR;
+            A.e[s] = -1;
+        }
+        coop_sync<G>();
+    }
+    if (rank == 0) {
+        CellRoot r;
+        r.wlo = A.wlo[0];
+        r.whi = A.whi[0];
+        r.first = F;
+        r.last = F + n - 1;
+        r.dL = dLc;
+        r.dR = dRc;
+        r.pad[0] = r.pad[1] = 0;
+        cx.croot[j] = r;
+    }
+    if (G == 32) {
+        written = __reduce_add_sync(0xFFFFFFFFu, written);
+        if (rank == 0 && written) atomicAdd(&cx.meta->nodes_emitted, written);
+    } else if (written) {
+        atomicAdd(&cx.meta->nodes_emitted, written);
+    }
+}
+
+constexpr int CELL_WARPS = 4;
+__global__ void __launch_bounds__(CELL_WARPS * 32) cell_tree_kernel(const TreeCtx cx) {
+    __shared__ __align__(16) unsigned char s_mem[CELL_WARPS][CELL_WARP_MAX * CELL_BYTES_PER_SLOT];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int j = blockIdx.x * CELL_WARPS + warp;
+    if (j >= cx.meta->ncell) return;
+    const uint32_t c = __ldg(cx.cell_list + j);
+    const int n = (int)(__ldg(cx.cell_start + c + 1) - __ldg(cx.cell_start + c));
+    if (n > CELL_WARP_MAX) {                        // too large for a warp: a whole block takes it in the next launch
+        if (lane == 0) cx.big_list[atomicAdd(&cx.meta->nbig, 1)] = j;
+        return;
+    }
+    process_cell<32>(cx, carve_cell_arrays(s_mem[warp], CELL_WARP_MAX), j, lane, false);
+}
+
+constexpr int TOP_THREADS = 512;
+__global__ void __launch_bounds__(TOP_THREADS) top_tree_kernel(const TreeCtx cx) {
+    extern __shared__ __align__(16) unsigned char s_dyn[];
+    // ---- cells too large for one warp (rare: strongly clustered input), one block each ----
+    const int nbig = cx.meta->nbig;
+    for (int b = blockIdx.x; b < nbig; b += gridDim.x) {
+        const int j = cx.big_list[b];
+        const uint32_t c = __ldg(cx.cell_list + j);
+        const int F = (int)__ldg(cx.cell_start + c);
+        const int n = (int)__ldg(cx.cell_start + c + 1) - F;
+        __syncthreads();
+        if (n <= CELL_BLOCK_MAX) {
+            process_cell<TOP_THREADS>(cx, carve_cell_arrays(s_dyn, CELL_BLOCK_MAX), j, threadIdx.x, false);
+        } else {
+            // giant cell: the entries are sorted in place, the other arrays live in the scratch area at the cell's own offset
+            CellArrays A;
+            A.kv = reinterpret_cast<unsigned long long *>(cx.ent + F);
+            unsigned char *sc = cx.scratch;
+            A.e = reinterpret_cast<int32_t *>(sc) + F;
+            A.mrg = reinterpret_cast<int32_t *>(sc + 4 * (size_t)cx.N) + F;
+            A.wlo = reinterpret_cast<uint32_t *>(sc + 8 * (size_t)cx.N) + F;
+            A.whi = reinterpret_cast<uint32_t *>(sc + 12 * (size_t)cx.N) + F;
+            A.dL = reinterpret_cast<int8_t *>(sc + 16 * (size_t)cx.N) + F;
+            A.dR = reinterpret_cast<int8_t *>(sc + 17 * (size_t)cx.N) + F;
+            // ent holds {key, index} as uint2 = little-endian (index << 32 | key): swap the halves so that the
+            // 64-bit order is (key, index)
+            for (int p = threadIdx.x; p < n; p += TOP_THREADS) {
+                const uint2 e = cx.ent[F + p];
+                A.kv[p] = ((unsigned long long)e.x << 32) | e.y;
+            }
+            __syncthreads();
+            process_cell<TOP_THREADS>(cx, A, j, threadIdx.x, true);
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            __threadfence();                          // the block's key_sorted stores, for the ropes of the walk
+            const CellRoot r = cx.croot[j];
+            Child me;
+            me.wlo = r.wlo & 0x7FFFFFFFu, me.whi = r.whi, me.f = r.first, me.l = r.last, me.pend = (r.wlo >> 31) != 0;
+            walk_up(cx, me, r.dL, r.dR, j);
+        }
+    }
+    // ---- one thread per cell root ----
+    const int j = blockIdx.x * TOP_THREADS + threadIdx.x;
+    if (j >= cx.meta->ncell) return;
+    const uint32_t c = __ldg(cx.cell_list + j);
+    if (__ldg(cx.cell_start + c + 1) - __ldg(cx.cell_start + c) > (uint32_t)CELL_WARP_MAX) return;   // walked by the block that built it
+    const CellRoot r = cx.croot[j];
+    Child me;
+    me.wlo = r.wlo & 0x7FFFFFFFu, me.whi = r.whi, me.f = r.first, me.l = r.last, me.pend = (r.wlo >> 31) != 0;
+    walk_up(cx, me, r.dL, r.dR, j);
+}
+
+// ------------------------------------------------------------------------------------------------------------
+int pick_cell_level(int64_t N, int T) {
+    // the smallest grid with at most ~48 particles per cell on average, T * 8^lvl <= CELL_MAX_TOTAL
+    int lvl = CELL_LMIN;
+    while (lvl < CELL_LMAX && N > (int64_t)48 << (3 * lvl)) ++lvl;
+    while (lvl > CELL_LMIN && ((int64_t)T << (3 * lvl)) > CELL_MAX_TOTAL) --lvl;
+    return lvl;
+}
+
+cudaError_t launch_build(const void *pos, const int32_t *type, const BuildParams &p, const BuildBuffers &b, cudaStream_t st) {
+    const int N = p.N;
     cudaError_t err = cudaMemsetAsync(b.meta, 0, sizeof(TreeMeta), st);
     if (err != cudaSuccess) return err;
     if (N == 0) {
-        finalize_kernel<<<1, MORTON_THREADS, 0, st>>>(b.meta, 0);
+        finalize_empty_kernel<<<1, 32, 0, st>>>(b.meta);
         return cudaGetLastError();
     }
-    const int tiles = (N + SORT_TILE - 1) / SORT_TILE;
-    const int status_words = tiles * 256;
-    const int entry_words = QBVH_TMAX * ENTRY_CELLS;
-    static int warp_slots = 0;                     // warps the traversal keeps resident on this device
-    if (warp_slots == 0) {
-        int dev = 0, sms = 148;
+    static int sms = 0;
+    if (sms == 0) {
+        int dev = 0;
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        warp_slots = sms * 28;
+        cudaFuncSetAttribute(top_tree_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, CELL_BLOCK_MAX * CELL_BYTES_PER_SLOT);
     }
-    const float3 lo = make_float3(box_lo[0], box_lo[1], box_lo[2]);
-    const float3 sc = make_float3(box_scale[0], box_scale[1], box_scale[2]);
+    const int lvl = p.lvl;
+    const int ncells = p.T << (3 * lvl);
+    const int cell_shift = 30 - 3 * lvl;
+    const int entry_words = QBVH_TMAX * ENTRY_CELLS;
+    const float3 lo = make_float3(p.box_lo[0], p.box_lo[1], p.box_lo[2]);
+    const float3 sc = make_float3(p.box_scale[0], p.box_scale[1], p.box_scale[2]);
     int mblocks = (N / 4 + MORTON_THREADS - 1) / MORTON_THREADS;
-    if (mblocks > 148 * 2) mblocks = 148 * 2;
-    if (mblocks < 1) mblocks = 1;
-    switch (T) {
-        case 1: morton_hist_kernel<1><<<mblocks, MORTON_THREADS, 0, st>>>(pos, type, N, lo, sc, b.key_a, b.meta, b.status[0], status_words, b.entry, entry_words, warp_slots); break;
-        case 2: morton_hist_kernel<2><<<mblocks, MORTON_THREADS, 0, st>>>(pos, type, N, lo, sc, b.key_a, b.meta, b.status[0], status_words, b.entry, entry_words, warp_slots); break;
-        case 3: morton_hist_kernel<3><<<mblocks, MORTON_THREADS, 0, st>>>(pos, type, N, lo, sc, b.key_a, b.meta, b.status[0], status_words, b.entry, entry_words, warp_slots); break;
-        default: morton_hist_kernel<4><<<mblocks, MORTON_THREADS, 0, st>>>(pos, type, N, lo, sc, b.key_a, b.meta, b.status[0], status_words, b.entry, entry_words, warp_slots); break;
+    mblocks = max(1, min(mblocks, sms * 2));
+#define QBVH_MORTON(NT)                                                                                                        \
+    if (p.f64)                                                                                                                 \
+        morton_cell_kernel<NT, double><<<mblocks, MORTON_THREADS, 0, st>>>(static_cast<const double *>(pos), type, N, lo, sc,  \
+                                                                          cell_shift, b.key, b.cell_count, b.meta, b.entry, entry_words); \
+    else                                                                                                                       \
+        morton_cell_kernel<NT, float><<<mblocks, MORTON_THREADS, 0, st>>>(static_cast<const float *>(pos), type, N, lo, sc,    \
+                                                                         cell_shift, b.key, b.cell_count, b.meta, b.entry, entry_words);
+    switch (p.T) {
+        case 1: QBVH_MORTON(1) break;
+        case 2: QBVH_MORTON(2) break;
+        case 3: QBVH_MORTON(3) break;
+        default: QBVH_MORTON(4) break;
     }
-    // four passes a -> b -> a -> b -> a
-    onesweep_kernel<true><<<tiles, SORT_THREADS, 0, st>>>(b.key_a, nullptr, b.key_b, b.idx_b, N, 0, b.meta->hist[0],
-                                                          b.status[0], b.status[1], &b.meta->tile_counter[0]);
-    onesweep_kernel<false><<<tiles, SORT_THREADS, 0, st>>>(b.key_b, b.idx_b, b.key_a, b.idx_a, N, 8, b.meta->hist[1],
-                                                           b.status[1], b.status[0], &b.meta->tile_counter[1]);
-    onesweep_kernel<false><<<tiles, SORT_THREADS, 0, st>>>(b.key_a, b.idx_a, b.key_b, b.idx_b, N, 16, b.meta->hist[2],
-                                                           b.status[0], b.status[1], &b.meta->tile_counter[2]);
-    onesweep_kernel<false><<<tiles, SORT_THREADS, 0, st>>>(b.key_b, b.idx_b, b.key_a, b.idx_a, N, 24, b.meta->hist[3],
-                                                           b.status[1], b.status[0], &b.meta->tile_counter[3]);
-    const int nb = (N + 255) / 256;
-    tree_kernel<<<nb, 256, 0, st>>>(pos, b.idx_a, b.key_a, N, b.meta, b.sorted_pos, b.nodes, b.parent, b.slot, b.groups,
-                                    b.entry, K, build_tag);
+#undef QBVH_MORTON
+    FinalizeParams fp;
+    fp.N = N, fp.T = p.T, fp.lvl = lvl, fp.warp_slots = traverse_warp_slots();
+    for (int t = 0; t < QBVH_TMAX; ++t) fp.r_hint[t] = p.r_hint[t];
+    const int tiles = (ncells + SCAN_TILE - 1) / SCAN_TILE;
+    cell_scan_kernel<<<tiles, SCAN_THREADS, 0, st>>>(b.cell_count, b.cell_start, b.cell_list, ncells, b.meta, fp);
+    cell_scatter_kernel<<<(N + 255) / 256, 256, 0, st>>>(b.key, N, cell_shift, b.cell_count, b.cell_start, b.ent);
+    TreeCtx cx;
+    cx.pos = pos, cx.f64 = p.f64 ? 1 : 0, cx.N = N, cx.K = p.K, cx.lvl = lvl, cx.build_tag = p.build_tag;
+    cx.cell_start = b.cell_start, cx.cell_list = b.cell_list, cx.ent = b.ent;
+    cx.key_sorted = b.key_sorted, cx.idx_sorted = b.idx_sorted, cx.sorted_pos = b.sorted_pos;
+    cx.sorted_pos64 = b.sorted_pos64;
+    cx.nodes = b.nodes, cx.parent = b.parent, cx.slot = b.slot, cx.groups = b.groups, cx.entry = b.entry;
+    cx.big_list = b.big_list, cx.croot = b.croot, cx.scratch = b.scratch, cx.meta = b.meta;
+    const int max_cells = min(N, ncells);
+    cell_tree_kernel<<<(max_cells + CELL_WARPS - 1) / CELL_WARPS, CELL_WARPS * 32, 0, st>>>(cx);
+    top_tree_kernel<<<(max_cells + TOP_THREADS - 1) / TOP_THREADS, TOP_THREADS, CELL_BLOCK_MAX * CELL_BYTES_PER_SLOT, st>>>(cx);
     return cudaGetLastError();
 }

@@ -7,21 +7,37 @@
 #define QBVH_TMAX 4            // types live in key bits 30-31
 #define QBVH_NBINS 1023.0f     // 2^10 - 1 bins per axis
 
+// ---- Morton cells of the build ----
+// The build partitions the particles by the leading 2 + 3*lvl bits of their keys (type, then the cell of the
+// 2^lvl-per-axis Morton grid over the box).  All keys of a cell are consecutive in Z-order and form one
+// subtree of the radix tree, so a cell is sorted and its subtree built locally; only cell roots meet in global memory.
+constexpr int CELL_LMIN = 2, CELL_LMAX = 6;
+constexpr int CELL_MAX_TOTAL = 1 << 18;        // cells over all types: T * 8^lvl <= 2^18
+constexpr int CELL_WARP_MAX = 128;             // a cell up to this size is handled by one warp (shared memory)
+constexpr int CELL_BLOCK_MAX = 2048;           // ... up to this size by one block (shared memory); larger: global scratch
+constexpr int SCAN_THREADS = 256, SCAN_IPT = 8, SCAN_TILE = SCAN_THREADS * SCAN_IPT;
+constexpr int SCAN_MAX_TILES = CELL_MAX_TOTAL / SCAN_TILE;   // 128
+
 // Device-resident bookkeeping of one build (lives at the start of the workspace; zeroed by a memset per build).
 struct TreeMeta {
-    uint32_t hist[4][256];     // per-pass digit histograms, turned into exclusive offsets by the last block of morton_hist_kernel
-    uint32_t tile_counter[4];  // dynamic tile ids of the four onesweep passes
-    uint32_t blocks_done;      // blocks of morton_hist_kernel that have added their histograms (the last one finalizes)
+    unsigned long long scan_status[SCAN_MAX_TILES];  // decoupled look-back of the cell scan: flag << 62 | nonempty << 32 | count
+    uint32_t scan_done;             // tiles of the scan that have finished (the last one finalizes)
     uint32_t mm_enc[QBVH_TMAX][6];  // per type: ~enc(min xyz) (so atomicMax computes the min), enc(max xyz)
     int32_t seg[QBVH_TMAX + 1];     // first sorted position of each type; seg[T..4] = N
     int32_t roots[QBVH_TMAX];       // root node per type, -1 if empty
     float frames[QBVH_TMAX][12];    // lo xyz, hi xyz, delta xyz, 0 0 0
     int32_t gmax[QBVH_TMAX];        // largest query group of each type (<= GROUP_MAX; smaller for a sparse type, see finalize)
-    int32_t pad_[38];               // the counters below, hammered by atomics, keep a 128-byte line of their own
-    int32_t group_count;            // number of query groups emitted by the build (tree_kernel)
+    int32_t rbin[QBVH_TMAX][4];     // collapse heuristic: expected query radius against this tree in bins per axis; [0] < 0: none
+    int32_t ncell;                  // number of non-empty cells
+    int32_t nbig;                   // cells larger than CELL_WARP_MAX (handled by whole blocks)
+    int32_t pad_[24];
+    // the counters below, hammered by atomics, keep a 128-byte line of their own
+    int32_t group_count;            // number of query groups emitted by the build
     int32_t group_cursor;           // next group to hand out (dynamic scheduling of the traversal); reset per traversal
     int32_t max_count;              // max_i n_neigh[i] of the last traversal
-    int32_t err_flags;              // bit 0: type id out of range
+    int32_t err_flags;              // bit 0: type id out of range; bit 1: traversal work list bound violated
+    int32_t nodes_emitted;          // nodes written by the build (2N-1 without collapse)
+    int32_t pad2_[27];
     unsigned long long stats[16];   // qbvh_stats, in order
 };
 
@@ -39,16 +55,6 @@ __device__ inline float ord2f(uint32_t o) {
     return __uint_as_float(b);
 }
 
-
-// ---- sort geometry ----
-constexpr int SORT_THREADS = 512;
-constexpr int SORT_WARPS = SORT_THREADS / 32;
-constexpr int SORT_IPT = 8;                           // keys per thread
-constexpr int SORT_TILE = SORT_THREADS * SORT_IPT;    // 4096 keys per tile
-constexpr uint32_t ST_AGG = 1u << 30;                 // tile status: aggregate (own count) available
-constexpr uint32_t ST_PRE = 1u << 31;                 // tile status: inclusive prefix available
-constexpr uint32_t ST_VAL = (1u << 30) - 1;
-
 // ---- query groups ----
 // A query group is a maximal subtree of the LBVH with at most GROUP_MAX leaves (fewer for a sparse type, TreeMeta::gmax): a contiguous run of Z-ordered
 // particles that fills one Morton cell, i.e. a compact blob.  One warp traverses the tree once
@@ -62,6 +68,12 @@ __host__ __device__ constexpr int entry_offset(int l) {   // cells of the levels
 }
 constexpr int ENTRY_CELLS = 64 + 512 + 4096 + 32768;
 
+// ---- subtree collapse ----
+// Integer cost model in bin units of the tree's quantization frame: visiting a node costs COST_NODE, a range leaf
+// COST_LEAF_FIXED + COST_LEAF_PER_PARTICLE * count, each weighted by the volume of its quantized box swollen by the
+// expected query radius (a box-shaped Minkowski sum).
+constexpr int COST_NODE = 1, COST_LEAF_FIXED = 16, COST_LEAF_PER_PARTICLE = 1;
+
 struct TraverseParams {
     float L[3];
     float r2[QBVH_TMAX * QBVH_TMAX];   // r_ij^2 (fp32 RN), <0 => skipped
@@ -70,24 +82,56 @@ struct TraverseParams {
     float box_lo[3], scale[3];         // Morton binning of the build: bin = floor((p - box_lo) * scale)
     int32_t N;
     int32_t max_neigh;
-    int32_t K;                         // leaf-collapse threshold used by the build
+    int32_t K;                         // leaf-collapse cap used by the build
+};
+
+// record a cell's root hands to the top-level walk (cell_tree_kernel -> top_tree_kernel)
+struct __align__(16) CellRoot {
+    uint32_t wlo;      // packed lower bound; bit 31: pending (a single particle or a collapsed range not yet written)
+    uint32_t whi;
+    int32_t first;     // sorted positions covered
+    int32_t last;
+    int32_t dL, dR;    // common prefix lengths with the neighbouring cells (-1 beyond the type segment)
+    int32_t pad[2];
+};
+
+// Z-ordered fp64 particle record of a double-precision build (qbvh_build_f64)
+struct __align__(32) Pos64 {
+    double x, y, z;
+    long long idx;     // original index
 };
 
 // launchers (build_kernels.cu / traverse_kernels.cu)
 struct BuildBuffers {
     TreeMeta *meta;
-    uint32_t *key_a, *key_b, *idx_a, *idx_b;
-    uint32_t *status[2];
+    uint32_t *key;                 // Morton keys in input order
+    uint2 *ent;                    // {key, original index} partitioned by cell, then sorted inside each cell
+    uint32_t *key_sorted, *idx_sorted;
+    uint32_t *cell_count;          // [ncells] particles per cell; counted by the key kernel, counted back to 0 by the scatter
+    uint32_t *cell_start;          // [ncells + 1] exclusive prefix
+    uint32_t *cell_list;           // non-empty cells in ascending order
+    int32_t *big_list;             // compact indices of the cells larger than CELL_WARP_MAX
+    CellRoot *croot;               // one per non-empty cell
     float4 *sorted_pos;
+    Pos64 *sorted_pos64;           // only written by double-precision builds
     int4 *nodes;
     int32_t *parent;
-    uint4 *slot;                   // meeting slot of the two children of the node that splits at gamma (tree_kernel)
+    uint4 *slot;                   // meeting slot of the two children of the node that splits at gamma (top_tree_kernel)
     uint2 *groups;                 // {first sorted position, number of particles}, group_count entries, any order
     int32_t *entry;                // [QBVH_TMAX][ENTRY_CELLS] entry table
+    unsigned char *scratch;        // 18 B per particle: working arrays of cells too large for shared memory
 };
-cudaError_t launch_build(const float *pos, const int32_t *type, int N, int T, int K, const float *box_lo,
-                         const float *box_scale, const BuildBuffers &b, uint32_t build_tag, cudaStream_t st);
+struct BuildParams {
+    int N, T, K, lvl;
+    float box_lo[3], box_scale[3];
+    float r_hint[QBVH_TMAX];       // <= 0: no collapse hint for that tree
+    uint32_t build_tag;
+    bool f64;                      // positions are double precision (qbvh_build_f64)
+};
+int pick_cell_level(int64_t N, int T);
+cudaError_t launch_build(const void *pos, const int32_t *type, const BuildParams &p, const BuildBuffers &b, cudaStream_t st);
 cudaError_t launch_traverse(const TraverseParams &p, const BuildBuffers &b, int32_t *nlist, int32_t *n_neigh,
                             bool stats, int variant, cudaStream_t st);
 cudaError_t launch_count_overlaps(const TraverseParams &p, const BuildBuffers &b, int32_t *n_overlap, cudaStream_t st);
+int traverse_warp_slots();      // warps the production traversal keeps resident on this device
 static_assert(offsetof(TreeMeta, group_count) % 128 == 0, "the atomic counters start a 128-byte line");

@@ -562,6 +562,8 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
                                               spread5((uint32_t)(c0[2] + iz));
                         node = __ldg(etab + entry_offset(lvl) + (int)cell);
                     }
+                    // a range leaf larger than the cells of this level roots several of them: keep one copy
+                    if (__match_any_sync(FULL, node) & lt_mask) node = -1;
                     const uint32_t eb = __ballot_sync(FULL, node >= 0);
                     if (node >= 0) sm.wl[__popc(eb & lt_mask)] = (uint32_t)node;
                     wsz = __popc(eb);
@@ -751,6 +753,9 @@ static void launch_group(const TraverseParams &p, const BuildBuffers &b, int32_t
     const int gb = min(group_grid_blocks<STATS, WS>(), (p.N + GW_WARPS - 1) / GW_WARPS);
     traverse_group_kernel<STATS, WS><<<gb, GW_WARPS * 32, 0, st>>>(p, b.nodes, b.sorted_pos, b.groups, b.entry, b.meta, nlist, n_neigh);
 }
+
+// warps the production traversal keeps resident (the build sizes query groups of small systems by it)
+int traverse_warp_slots() { return group_grid_blocks<false, 32>() * GW_WARPS; }
 
 cudaError_t launch_traverse(const TraverseParams &p, const BuildBuffers &b, int32_t *nlist, int32_t *n_neigh,
                             bool stats, int variant, cudaStream_t st) {

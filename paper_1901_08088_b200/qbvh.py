@@ -18,13 +18,13 @@ OK = 0
 ERR_INVALID_ARG, ERR_NOT_BUILT, ERR_WORKSPACE, ERR_CUTOFF_TOO_LARGE, ERR_TYPE_RANGE, ERR_CUDA, ERR_INTERNAL = -1, -2, -3, -4, -5, -6, -7
 MAX_TYPES = 4
 OPT_LEAF_COLLAPSE, OPT_STATS, OPT_VARIANT, OPT_DEBUG_BUILD_TAG = 1, 2, 3, 4
-EXPORT_KEYS_SORTED, EXPORT_PERM, EXPORT_NODES, EXPORT_PARENT, EXPORT_FRAMES, EXPORT_SEGMENTS, EXPORT_SORTED_POS = range(1, 8)
+EXPORT_KEYS_SORTED, EXPORT_PERM, EXPORT_NODES, EXPORT_PARENT, EXPORT_FRAMES, EXPORT_SEGMENTS, EXPORT_SORTED_POS, EXPORT_COUNTS = range(1, 9)
 
 # every symbol include/qbvh.h declares
 SYMBOLS = ("qbvh_set_stream", "qbvh_set_num_types", "qbvh_workspace_bytes", "qbvh_set_workspace",
            "qbvh_set_option", "qbvh_get_option", "qbvh_build", "qbvh_neighbors", "qbvh_count_overlaps", "qbvh_staging_bytes",
            "qbvh_set_staging", "qbvh_build_host", "qbvh_neighbors_host", "qbvh_get_stats", "qbvh_debug_export",
-           "qbvh_error_string", "qbvh_padded_radius")
+           "qbvh_error_string", "qbvh_padded_radius", "qbvh_set_collapse_hint")
 
 
 class QbvhStats(C.Structure):
@@ -52,6 +52,7 @@ _lib.qbvh_workspace_bytes.restype = _i64
 _lib.qbvh_set_workspace.argtypes = [_vp, _i64]
 _lib.qbvh_set_option.argtypes = [_i32, _i32]
 _lib.qbvh_get_option.argtypes = [_i32]
+_lib.qbvh_set_collapse_hint.argtypes = [_vp, _i32]
 _lib.qbvh_build.argtypes = [_vp, _vp, _i64, _vp]
 _lib.qbvh_neighbors.argtypes = [_vp, _vp, _vp, _i32]
 _lib.qbvh_count_overlaps.argtypes = [_vp, _vp]
@@ -137,6 +138,14 @@ def qbvh_set_option(key: int, value: int) -> int:
     return _check(_lib.qbvh_set_option(key, value), "qbvh_set_option")
 
 
+def qbvh_set_collapse_hint(r_hint) -> int:
+    """r_hint: per-type expected query radius (HOST, at most MAX_TYPES values) or None for no hint."""
+    if r_hint is None:
+        return _check(_lib.qbvh_set_collapse_hint(None, 0), "qbvh_set_collapse_hint")
+    r = np.ascontiguousarray(r_hint, dtype=np.float32).reshape(-1)
+    return _check(_lib.qbvh_set_collapse_hint(r.ctypes.data, r.size), "qbvh_set_collapse_hint")
+
+
 def qbvh_get_option(key: int) -> int:
     return _check(_lib.qbvh_get_option(key), "qbvh_get_option")
 
@@ -200,7 +209,7 @@ def qbvh_debug_export(what: int, N: int) -> np.ndarray:
     shapes = {EXPORT_KEYS_SORTED: (np.uint32, (N,)), EXPORT_PERM: (np.uint32, (N,)),
               EXPORT_NODES: (np.int32, (max(2 * N - 1, 0), 4)), EXPORT_PARENT: (np.int32, (max(2 * N - 1, 0),)),
               EXPORT_FRAMES: (np.float32, (4, 12)), EXPORT_SEGMENTS: (np.int32, (10,)),
-              EXPORT_SORTED_POS: (np.float32, (N, 4))}
+              EXPORT_SORTED_POS: (np.float32, (N, 4)), EXPORT_COUNTS: (np.int32, (4,))}
     dt, shp = shapes[what]
     out = np.zeros(shp, dt)
     avail = _check(_lib.qbvh_debug_export(what, out.ctypes.data, out.nbytes), "qbvh_debug_export")

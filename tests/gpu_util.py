@@ -4,7 +4,7 @@ from __future__ import annotations
 import numpy as np
 
 
-def gpu_run(w, K=4, max_neigh=None, stats=False, export=False, retry=False):
+def gpu_run(w, K=4, max_neigh=None, stats=False, export=False, retry=False, hint=None):
     """Build + traverse workload `w` on cuda:0.  Returns dict(nlist, n_neigh, M, [exports], [stats])."""
     import torch
     from paper_1901_08088_b200 import qbvh
@@ -13,6 +13,7 @@ def gpu_run(w, K=4, max_neigh=None, stats=False, export=False, retry=False):
     max_neigh = w.max_neigh if max_neigh is None else max_neigh
     qbvh.qbvh_set_option(qbvh.OPT_LEAF_COLLAPSE, K)
     qbvh.qbvh_set_option(qbvh.OPT_STATS, int(stats))
+    qbvh.qbvh_set_collapse_hint(hint)
     nl = qbvh.NeighborList(w.N, T=w.T, max_neigh=max_neigh, device=dev)
     pos = torch.from_numpy(w.pos).to(dev)
     typ = None if w.type is None else torch.from_numpy(w.type).to(dev)
@@ -26,6 +27,7 @@ def gpu_run(w, K=4, max_neigh=None, stats=False, export=False, retry=False):
         out["frames"] = qbvh.qbvh_debug_export(qbvh.EXPORT_FRAMES, w.N)
         out["segments"] = qbvh.qbvh_debug_export(qbvh.EXPORT_SEGMENTS, w.N)
         out["sorted_pos"] = qbvh.qbvh_debug_export(qbvh.EXPORT_SORTED_POS, w.N)
+        out["nodes_emitted"] = int(qbvh.qbvh_debug_export(qbvh.EXPORT_COUNTS, w.N)[0])
     nl.n_neigh.fill_(-7)
     nl.nlist.fill_(-1)
     M = nl.neighbors(w.r_list, retry=retry)
@@ -38,6 +40,7 @@ def gpu_run(w, K=4, max_neigh=None, stats=False, export=False, retry=False):
     if stats:
         out["stats"] = qbvh.qbvh_get_stats()
     qbvh.qbvh_set_option(qbvh.OPT_STATS, 0)
+    qbvh.qbvh_set_collapse_hint(None)
     return out
 
 

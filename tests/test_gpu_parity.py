@@ -16,21 +16,71 @@ from gpu_util import compare_with_oracle, gpu_run
 pytestmark = pytest.mark.gpu
 
 
-def expected_nodes(t, K):
-    """Oracle tree -> the node array the CUDA path must produce for leaf-collapse option K."""
-    nodes = t.nodes_int4().copy()
+C_NODE, C_LEAF_FIXED, C_LEAF_PER_PARTICLE = 1, 16, 1   # DESIGN.md §3.7 (restated here, not imported)
+
+
+def collapse_frontier(t, K, r_hint=None):
+    """Subtree collapse restated on the oracle's one-particle-per-leaf tree.
+
+    Bottom up: a single particle is 'pending'; an internal node with cnt <= K particles whose children are both
+    pending collapses into one range leaf — always without a hint; with a hint r_b for its tree only if that does
+    not raise the cost  W(n) (C_F + C_L cnt)  <=  W(n) C_N + sum over the two children of W(c) (C_F + C_L cnt_c),
+    W = prod_d (max(q_hi,d - q_lo,d, 0) + 2 ceil(r_b / Delta_d)) in integers (bins of the tree's frame).
+    Returns (emitted, collapsed): which nodes exist in the collapsed tree, which of them are range leaves."""
+    N = t.N
+    M = 2 * N - 1
+    size = np.where(t.first >= 0, t.last - t.first + 1, 0).astype(np.int64)
+    pend = np.zeros(M, bool)
+    pend[N - 1:] = True
+    coll = np.zeros(M, bool)
+    ql = np.stack([(t.wlo >> (10 * d)) & 1023 for d in range(3)], 1).astype(np.int64)
+    qh = np.stack([(t.whi >> (10 * d)) & 1023 for d in range(3)], 1).astype(np.int64)
+    ext = np.maximum(qh - ql, 0)
+    tree_of = np.searchsorted(t.seg[1:], np.maximum(t.first, 0), side="right")
+    rb = None
+    if r_hint is not None:
+        rb = np.full((t.T, 3), -1, np.int64)
+        for tb in range(t.T):
+            if r_hint[tb] > 0 and t.roots[tb] >= 0:
+                for d in range(3):
+                    delta = np.float32(t.frames[tb, 6 + d])
+                    rb[tb, d] = min(int(np.ceil(np.float32(r_hint[tb]) / delta)), 1023) if delta > 0 else 1
+
+    def W(n):
+        r = rb[tree_of[n]]
+        return int((ext[n, 0] + 2 * r[0]) * (ext[n, 1] + 2 * r[1]) * (ext[n, 2] + 2 * r[2]))
+
     if K > 1:
-        N = t.N
-        size = (t.last - t.first + 1).astype(np.int64)
-        internal = np.arange(2 * N - 1) < N - 1
-        real = t.first >= 0
-        coll = internal & real & (size <= K)
-        nodes[coll, 2] = ~t.first[coll]      # the particle count of a collapsed leaf follows from its rope
-    return nodes
+        cand = np.nonzero((np.arange(M) < N - 1) & (size >= 2) & (size <= K))[0]
+        for n in cand[np.argsort(size[cand], kind="stable")]:           # children before parents
+            a, b = t.left[n], t.right[n]
+            ok = pend[a] and pend[b]
+            if ok and rb is not None and rb[tree_of[n], 0] >= 0:
+                leaf = lambda m: W(m) * (C_LEAF_FIXED + C_LEAF_PER_PARTICLE * int(size[m]))
+                ok = leaf(n) <= W(n) * C_NODE + leaf(a) + leaf(b)
+            pend[n] = coll[n] = ok
+    # top down: a node exists iff no proper ancestor collapsed
+    emitted = np.zeros(M, bool)
+    stack = [int(r) for r in t.roots if r >= 0]
+    while stack:
+        n = stack.pop()
+        emitted[n] = True
+        if n < N - 1 and not coll[n]:
+            stack.append(int(t.left[n]))
+            stack.append(int(t.right[n]))
+    return emitted, coll
 
 
-def check_build(w, K):
-    out = gpu_run(w, K=K, export=True)
+def expected_nodes(t, K, r_hint=None):
+    """Oracle tree -> (node array, emitted mask) the CUDA path must produce for collapse cap K and hint r_hint."""
+    nodes = t.nodes_int4().copy()
+    emitted, coll = collapse_frontier(t, K, r_hint)
+    nodes[coll, 2] = ~t.first[coll]          # a range leaf: ~first; its particle count follows from its rope
+    return nodes, emitted
+
+
+def check_build(w, K, r_hint=None):
+    out = gpu_run(w, K=K, export=True, hint=r_hint)
     t = OT.build(w.pos, w.type, w.box, T=w.T)
     N = w.N
     assert np.array_equal(out["keys_sorted"], t.key_sorted)                      # a1 + a2 keys
@@ -43,12 +93,12 @@ def check_build(w, K):
             assert np.array_equal(out["frames"][tb, :9], t.frames[tb])           # root boxes + Delta (bitwise)
     assert np.array_equal(out["sorted_pos"][:, :3], t.pos_sorted)               # a2' gather
     assert np.array_equal(out["sorted_pos"][:, 3].view(np.uint32).astype(np.int64), t.perm)
-    exp = expected_nodes(t, K)
-    real = np.ones(2 * N - 1, bool)
-    real[: N - 1] = t.first[: N - 1] >= 0                                        # skip unused internal slots
-    assert np.array_equal(out["nodes"][real], exp[real])                         # a3..a6: 16-byte nodes, bitwise
-    assert np.array_equal(out["nodes"][~real], np.tile([0, 0, 0, -1], ((~real).sum(), 1)))
-    assert np.array_equal(out["parent"][real], t.parent[real])
+    exp, emitted = expected_nodes(t, K, r_hint)
+    if K == 1:
+        assert emitted.sum() == 2 * N - 1 - max(0, np.count_nonzero(np.diff(t.seg) > 0) - 1)   # the paper's tree, whole
+    assert np.array_equal(out["nodes"][emitted], exp[emitted])                   # a3..a6: 16-byte nodes, bitwise
+    assert np.array_equal(out["parent"][emitted], t.parent[emitted])
+    assert out["nodes_emitted"] == int(emitted.sum())                            # descendants of range leaves are never written
     return out, t
 
 
@@ -438,13 +488,32 @@ def test_rebuild_in_place_on_one_workspace():
         t = OT.build(pos, typ, box, T=T)
         nodes = qbvh.qbvh_debug_export(qbvh.EXPORT_NODES, N)
         parent = qbvh.qbvh_debug_export(qbvh.EXPORT_PARENT, N)
-        real = np.ones(2 * N - 1, bool)
-        real[: N - 1] = t.first[: N - 1] >= 0
-        assert np.array_equal(nodes[real], expected_nodes(t, K)[real]), it
-        assert np.array_equal(parent[real], t.parent[real]), it
+        exp, emitted = expected_nodes(t, K)
+        assert np.array_equal(nodes[emitted], exp[emitted]), it
+        assert np.array_equal(parent[emitted], t.parent[emitted]), it
         nl.n_neigh.fill_(-7)
         M = nl.neighbors(r, retry=False)
         out = {"M": M, "max_neigh": nl.max_neigh, "nlist": nl.nlist.cpu().numpy()[:N], "n_neigh": nl.n_neigh.cpu().numpy()[:N]}
         compare_with_oracle(w, out, ON.neighbor_list(pos, typ, box, r))
     assert tags == [1, 2, 3, 0xFFFFFE, 0xFFFFFF, 1, 2], tags      # no clearing between builds except at the wrap
     qbvh.qbvh_set_option(qbvh.OPT_LEAF_COLLAPSE, 32)
+
+
+@pytest.mark.parametrize("K", [8, 32])
+@pytest.mark.parametrize("cid", [1, 2, 3, 4, 5])
+def test_collapse_heuristic_build_and_lists(cid, K):
+    """build-side subtree collapse chosen by the cost heuristic (qbvh_set_collapse_hint).  The node
+    array must hold exactly the nodes at or above the frontier the heuristic picks on the oracle's
+    one-particle-per-leaf tree (restated in collapse_frontier above), bit for bit, and nothing below it; lists stay
+    identical to the oracle's."""
+    w = W.make_config(cid, small=True)
+    hint = np.asarray(w.r_list, np.float32).reshape(w.T, w.T).max(axis=0)
+    out, t = check_build(w, K, r_hint=hint)
+    rep = compare_with_oracle(w, out, ON.neighbor_list(w.pos, w.type, w.box, w.r_list))
+    assert rep["rows_checked"] == w.N
+    emitted, coll = collapse_frontier(t, K, hint)
+    # the heuristic is not the plain size threshold: on a type far sparser than its cutoff it stops earlier
+    plain, _ = collapse_frontier(t, K, None)
+    assert emitted.sum() >= plain.sum()
+    if cid == 3 and K == 32:
+        assert emitted.sum() > plain.sum()
