@@ -38,7 +38,7 @@ struct Context {
 inline int64_t align256(int64_t x) { return (x + 255) & ~int64_t(255); }
 
 struct Layout {
-    int64_t meta, key, ent, key_sorted, idx_sorted, cell_count, cell_start, cell_list, big_list, croot, sorted_pos,
+    int64_t meta, key, rank, ent, key_sorted, idx_sorted, cell_count, cell_start, cell_list, big_list, croot, sorted_pos,
         sorted_pos64, nodes, parent, slot, groups, entry, scratch, total;
 };
 
@@ -56,6 +56,7 @@ Layout make_layout(int64_t N) {
     };
     L.meta = take(sizeof(TreeMeta));
     L.key = take(4 * n1);
+    L.rank = take(4 * n1);
     L.ent = take(8 * n1);
     L.key_sorted = take(4 * n1);
     L.idx_sorted = take(4 * n1);
@@ -183,6 +184,7 @@ int build_impl(const void *pos, bool f64, const int32_t *type, int64_t N, const 
     char *w = static_cast<char *>(g.ws);
     g.buf.meta = reinterpret_cast<TreeMeta *>(w + L.meta);
     g.buf.key = reinterpret_cast<uint32_t *>(w + L.key);
+    g.buf.rank = reinterpret_cast<uint32_t *>(w + L.rank);
     g.buf.ent = reinterpret_cast<uint2 *>(w + L.ent);
     g.buf.key_sorted = reinterpret_cast<uint32_t *>(w + L.key_sorted);
     g.buf.idx_sorted = reinterpret_cast<uint32_t *>(w + L.idx_sorted);

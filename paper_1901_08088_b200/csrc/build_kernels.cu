@@ -36,19 +36,25 @@ __device__ __forceinline__ uint32_t morton_bin(float p, float lo, float s) {
     return (uint32_t)f;
 }
 
-constexpr int MORTON_THREADS = 512;
+constexpr int MORTON_THREADS = 256;
 
 // PT = float: the paper's single-precision particle data.  PT = double (qbvh_build_f64,
 // PAPER.md:140, 154): the tree is built from the positions rounded to fp32; the exact leaf test stays in fp64.
+// Four consecutive particles per thread, every particle of the system in flight at once (one wave of threads).
+// rank_out[i] = place of particle i inside its Morton cell, in order of arrival (one atomic per set of lanes that
+// share a cell: already Z-ordered input, common in MD, would otherwise hammer one address); the cell is sorted by
+// (key, index) afterwards, so the final order is the stable sort whatever the arrival order was.
 template <int NT, typename PT>
 __global__ void __launch_bounds__(MORTON_THREADS) morton_cell_kernel(const PT *__restrict__ pos,
                                                            const int32_t *__restrict__ type, int N, float3 lo,
                                                            float3 scale, int cell_shift, uint32_t *__restrict__ key_out,
+                                                           uint32_t *__restrict__ rank_out,
                                                            uint32_t *__restrict__ cell_count,
                                                            TreeMeta *__restrict__ meta,
                                                            int32_t *__restrict__ entry, int entry_words) {
     const int stride = gridDim.x * blockDim.x;
     const int gtid = blockIdx.x * blockDim.x + threadIdx.x;
+    const int lane = threadIdx.x & 31;
     // the entry table of the traversal starts out empty (-1) and is filled by the tree kernels
     for (int i = gtid; i < entry_words; i += stride) entry[i] = -1;
 
@@ -61,54 +67,77 @@ __global__ void __launch_bounds__(MORTON_THREADS) morton_cell_kernel(const PT *_
             mx[t][d] = -INFINITY;
         }
     bool bad_type = false;
-    auto one = [&](float x, float y, float z, int tt) -> uint32_t {
-        if (tt < 0 || tt >= NT) {
-            bad_type = true;
-            tt = 0;
-        }
-        const uint32_t t = (uint32_t)tt;
-        uint32_t code = (spread10(morton_bin(x, lo.x, scale.x)) << 2) | (spread10(morton_bin(y, lo.y, scale.y)) << 1) |
-                        spread10(morton_bin(z, lo.z, scale.z));
-        uint32_t key = (t << 30) | code;
-        atomicAdd(&cell_count[key >> cell_shift], 1u);      // result unused: a fire-and-forget reduction in L2
+    const int i0 = 4 * gtid;
+    float px[4], py[4], pz[4];
+    int tt[4] = {0, 0, 0, 0};
+    const bool full = i0 + 3 < N;
+    if (sizeof(PT) == 4 && full && ((reinterpret_cast<uintptr_t>(pos) & 15) == 0)) {
+        const float4 *p4 = reinterpret_cast<const float4 *>(pos) + 3 * (size_t)gtid;   // three 128-bit loads
+        const float4 a = __ldg(p4), b = __ldg(p4 + 1), c = __ldg(p4 + 2);
+        px[0] = a.x, py[0] = a.y, pz[0] = a.z, px[1] = a.w, py[1] = b.x, pz[1] = b.y;
+        px[2] = b.z, py[2] = b.w, pz[2] = c.x, px[3] = c.y, py[3] = c.z, pz[3] = c.w;
+    } else {
 #pragma unroll
-        for (int u = 0; u < NT; ++u) {
-            bool m = (NT == 1) || (t == (uint32_t)u);
-            mn[u][0] = m ? fminf(mn[u][0], x) : mn[u][0];
-            mn[u][1] = m ? fminf(mn[u][1], y) : mn[u][1];
-            mn[u][2] = m ? fminf(mn[u][2], z) : mn[u][2];
-            mx[u][0] = m ? fmaxf(mx[u][0], x) : mx[u][0];
-            mx[u][1] = m ? fmaxf(mx[u][1], y) : mx[u][1];
-            mx[u][2] = m ? fmaxf(mx[u][2], z) : mx[u][2];
+        for (int u = 0; u < 4; ++u) {
+            const int i = min(i0 + u, N - 1);
+            px[u] = (float)pos[3 * (size_t)i + 0], py[u] = (float)pos[3 * (size_t)i + 1], pz[u] = (float)pos[3 * (size_t)i + 2];
         }
-        return key;
-    };
-    int done = 0;
-    if (sizeof(PT) == 4) {
-        // four particles per thread and iteration: three 128-bit position loads, one 128-bit key store
-        const bool vec = ((reinterpret_cast<uintptr_t>(pos) & 15) == 0) && ((reinterpret_cast<uintptr_t>(key_out) & 15) == 0) &&
-                         (type == nullptr || (reinterpret_cast<uintptr_t>(type) & 15) == 0);
-        const int nquad = vec ? N / 4 : 0;
-        for (int q = gtid; q < nquad; q += stride) {
-            const float4 *p4 = reinterpret_cast<const float4 *>(pos) + 3 * (size_t)q;
-            const float4 a = __ldg(p4), b = __ldg(p4 + 1), c = __ldg(p4 + 2);
-            int4 tt = make_int4(0, 0, 0, 0);
-            if (type) tt = __ldg(reinterpret_cast<const int4 *>(type) + q);
-            uint4 k;
-            k.x = one(a.x, a.y, a.z, tt.x);
-            k.y = one(a.w, b.x, b.y, tt.y);
-            k.z = one(b.z, b.w, c.x, tt.z);
-            k.w = one(c.y, c.z, c.w, tt.w);
-            reinterpret_cast<uint4 *>(key_out)[q] = k;
-        }
-        done = 4 * nquad;
     }
-    for (int i = done + gtid; i < N; i += stride) {
-        const float x = (float)pos[3 * (size_t)i + 0], y = (float)pos[3 * (size_t)i + 1], z = (float)pos[3 * (size_t)i + 2];
-        key_out[i] = one(x, y, z, type ? type[i] : 0);
+    if (type) {
+        if (full && ((reinterpret_cast<uintptr_t>(type) & 15) == 0)) {
+            const int4 t4 = __ldg(reinterpret_cast<const int4 *>(type) + gtid);
+            tt[0] = t4.x, tt[1] = t4.y, tt[2] = t4.z, tt[3] = t4.w;
+        } else {
+#pragma unroll
+            for (int u = 0; u < 4; ++u) tt[u] = type[min(i0 + u, N - 1)];
+        }
+    }
+    uint32_t key[4], rank[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+        const bool valid = i0 + u < N;
+        int ty = tt[u];
+        if (valid && (ty < 0 || ty >= NT)) {
+            bad_type = true;
+            ty = 0;
+        }
+        const uint32_t t = (uint32_t)ty;
+        const float x = px[u], y = py[u], z = pz[u];
+        const uint32_t code = (spread10(morton_bin(x, lo.x, scale.x)) << 2) | (spread10(morton_bin(y, lo.y, scale.y)) << 1) |
+                              spread10(morton_bin(z, lo.z, scale.z));
+        key[u] = (t << 30) | code;
+        if (valid) {
+#pragma unroll
+            for (int v = 0; v < NT; ++v) {
+                const bool m = (NT == 1) || (t == (uint32_t)v);
+                mn[v][0] = m ? fminf(mn[v][0], x) : mn[v][0];
+                mn[v][1] = m ? fminf(mn[v][1], y) : mn[v][1];
+                mn[v][2] = m ? fminf(mn[v][2], z) : mn[v][2];
+                mx[v][0] = m ? fmaxf(mx[v][0], x) : mx[v][0];
+                mx[v][1] = m ? fmaxf(mx[v][1], y) : mx[v][1];
+                mx[v][2] = m ? fmaxf(mx[v][2], z) : mx[v][2];
+            }
+        }
+        const uint32_t c = valid ? (key[u] >> cell_shift) : 0xFFFFFFFFu;
+        const uint32_t m = __match_any_sync(0xFFFFFFFFu, c);
+        const int leader = __ffs(m) - 1;
+        uint32_t base = 0;
+        if (valid && lane == leader) base = atomicAdd(&cell_count[c], (uint32_t)__popc(m));
+        rank[u] = __shfl_sync(0xFFFFFFFFu, base, leader) + __popc(m & ((1u << lane) - 1u));
+    }
+    if (full && ((reinterpret_cast<uintptr_t>(key_out) & 15) == 0) && ((reinterpret_cast<uintptr_t>(rank_out) & 15) == 0)) {
+        reinterpret_cast<uint4 *>(key_out)[gtid] = make_uint4(key[0], key[1], key[2], key[3]);
+        reinterpret_cast<uint4 *>(rank_out)[gtid] = make_uint4(rank[0], rank[1], rank[2], rank[3]);
+    } else {
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+            if (i0 + u < N) {
+                key_out[i0 + u] = key[u];
+                rank_out[i0 + u] = rank[u];
+            }
     }
     // per-type min/max: warp reduce on the order-preserving encoding, block reduce through shared memory, then one
-    // global atomic per block and value (same-address atomics serialise in L2)
+    // global atomic per block and value
     __shared__ uint32_t s_mm[QBVH_TMAX][6];
     if (threadIdx.x < QBVH_TMAX * 6) (&s_mm[0][0])[threadIdx.x] = 0u;
     __syncthreads();
@@ -118,7 +147,7 @@ __global__ void __launch_bounds__(MORTON_THREADS) morton_cell_kernel(const PT *_
         for (int d = 0; d < 3; ++d) {
             uint32_t a = __reduce_max_sync(0xFFFFFFFFu, ~f2ord(mn[t][d]));
             uint32_t b = __reduce_max_sync(0xFFFFFFFFu, f2ord(mx[t][d]));
-            if ((threadIdx.x & 31) == 0) {
+            if (lane == 0) {
                 if (a != ~f2ord(INFINITY)) atomicMax(&s_mm[t][d], a);
                 if (b != f2ord(-INFINITY)) atomicMax(&s_mm[t][3 + d], b);
             }
@@ -194,9 +223,10 @@ __device__ void finalize_block(TreeMeta *__restrict__ meta, const uint32_t *__re
     }
 }
 
-constexpr unsigned long long SCAN_AGG = 1ull << 62, SCAN_PRE = 2ull << 62, SCAN_VAL = (1ull << 62) - 1;
-
-__global__ void __launch_bounds__(SCAN_THREADS) cell_scan_kernel(const uint32_t *__restrict__ cell_count,
+// One tile of SCAN_TILE cells per block.  No chain between the tiles: every block publishes its tile's total, all
+// blocks meet at a grid-wide barrier (at most SCAN_MAX_TILES = 128 blocks: all resident at once), then every block
+// sums the totals before it.  Reading a counter also clears it for the next build.
+__global__ void __launch_bounds__(SCAN_THREADS) cell_scan_kernel(uint32_t *__restrict__ cell_count,
                                                                   uint32_t *__restrict__ cell_start,
                                                                   uint32_t *__restrict__ cell_list, int ncells,
                                                                   TreeMeta *__restrict__ meta, const FinalizeParams fp) {
@@ -204,11 +234,21 @@ __global__ void __launch_bounds__(SCAN_THREADS) cell_scan_kernel(const uint32_t 
     __shared__ unsigned long long s_excl;
     __shared__ bool s_last;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int tile = blockIdx.x;
+    const int tile = blockIdx.x, ntiles = gridDim.x;
     const int c0 = tile * SCAN_TILE + tid * SCAN_IPT;
     uint32_t cnt[SCAN_IPT];
+    if (c0 + SCAN_IPT <= ncells) {
+        const uint4 a = __ldcg(reinterpret_cast<const uint4 *>(cell_count + c0)), b = __ldcg(reinterpret_cast<const uint4 *>(cell_count + c0) + 1);
+        cnt[0] = a.x, cnt[1] = a.y, cnt[2] = a.z, cnt[3] = a.w, cnt[4] = b.x, cnt[5] = b.y, cnt[6] = b.z, cnt[7] = b.w;
+        reinterpret_cast<uint4 *>(cell_count + c0)[0] = make_uint4(0u, 0u, 0u, 0u);
+        reinterpret_cast<uint4 *>(cell_count + c0)[1] = make_uint4(0u, 0u, 0u, 0u);
+    } else {
 #pragma unroll
-    for (int u = 0; u < SCAN_IPT; ++u) cnt[u] = (c0 + u < ncells) ? __ldcg(cell_count + c0 + u) : 0u;
+        for (int u = 0; u < SCAN_IPT; ++u) {
+            cnt[u] = (c0 + u < ncells) ? __ldcg(cell_count + c0 + u) : 0u;
+            if (c0 + u < ncells) cell_count[c0 + u] = 0u;
+        }
+    }
     // value = count in the low word, number of non-empty cells in the high word
     unsigned long long mine = 0;
 #pragma unroll
@@ -227,28 +267,30 @@ __global__ void __launch_bounds__(SCAN_THREADS) cell_scan_kernel(const uint32_t 
         if (w < warp) wbase += s_warp[w];
         total += s_warp[w];
     }
-    if (tid == 0) {
-        volatile unsigned long long *status = meta->scan_status;
-        unsigned long long excl = 0;
-        if (tile == 0) {
-            status[0] = total | SCAN_PRE;
-        } else {
-            status[tile] = total | SCAN_AGG;
-            int p = tile - 1;
-            while (true) {
-                const unsigned long long v = status[p];
-                if (v & SCAN_PRE) {
-                    excl += v & SCAN_VAL;
-                    break;
-                }
-                if (v & SCAN_AGG) {
-                    excl += v & SCAN_VAL;
-                    --p;
-                }
-            }
-            status[tile] = (excl + total) | SCAN_PRE;
+    volatile unsigned long long *tot = meta->scan_status;
+    if (ntiles > 1) {
+        if (tid == 0) {
+            tot[tile] = total;
+            __threadfence();
+            atomicAdd(&meta->scan_arrived, 1u);
+            while (*(volatile uint32_t *)&meta->scan_arrived < (uint32_t)ntiles) {}
+            __threadfence();
         }
-        s_excl = excl;
+        __syncthreads();
+        // exclusive prefix of the tile: the totals of the tiles before it (ntiles <= 128 <= SCAN_THREADS)
+        unsigned long long v = (tid < tile) ? tot[tid] : 0ull;
+#pragma unroll
+        for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, o);
+        __syncthreads();
+        if (lane == 0) s_warp[warp] = v;
+        __syncthreads();
+        if (tid == 0) {
+            unsigned long long e = 0;
+            for (int w = 0; w < SCAN_THREADS / 32; ++w) e += s_warp[w];
+            s_excl = e;
+        }
+    } else if (tid == 0) {
+        s_excl = 0;
     }
     __syncthreads();
     unsigned long long run = s_excl + wbase + inc - mine;
@@ -260,7 +302,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) cell_scan_kernel(const uint32_t 
         }
         run += (unsigned long long)cnt[u] | ((unsigned long long)(cnt[u] != 0) << 32);
     }
-    if (tile == (int)gridDim.x - 1 && tid == SCAN_THREADS - 1) {
+    if (tile == ntiles - 1 && tid == SCAN_THREADS - 1) {
         cell_start[ncells] = (uint32_t)run;              // = N
         meta->ncell = (int32_t)(run >> 32);
     }
@@ -289,26 +331,16 @@ __global__ void finalize_empty_kernel(TreeMeta *__restrict__ meta) {
 }
 
 // ------------------------------------------------------------------------------------------------------------
-// a2, first pass: (key, index) of every particle to its cell.  The place inside the cell is arbitrary (one atomic
-// per set of lanes that share a cell: already Z-ordered input, common in MD, would otherwise hammer one address);
-// the cell is sorted by (key, index) afterwards, so the final order is the stable sort.  Counting down leaves the
-// counters at zero for the next build.
+// a2, first pass (the most significant digit of the radix sort): (key, index) of every particle to its cell, at the
+// place the key kernel drew for it.
 // ------------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) cell_scatter_kernel(const uint32_t *__restrict__ key, int N, int cell_shift,
-                                                            uint32_t *__restrict__ cell_count,
-                                                            const uint32_t *__restrict__ cell_start,
+__global__ void __launch_bounds__(256) cell_scatter_kernel(const uint32_t *__restrict__ key, const uint32_t *__restrict__ rank,
+                                                            int N, int cell_shift, const uint32_t *__restrict__ cell_start,
                                                             uint2 *__restrict__ ent) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    const int lane = threadIdx.x & 31;
-    const bool valid = i < N;
-    const uint32_t k = valid ? key[i] : 0u;
-    const uint32_t c = valid ? (k >> cell_shift) : 0xFFFFFFFFu;
-    const uint32_t m = __match_any_sync(0xFFFFFFFFu, c);
-    const int leader = __ffs(m) - 1;
-    uint32_t base = 0;
-    if (valid && lane == leader) base = atomicSub(&cell_count[c], (uint32_t)__popc(m)) - (uint32_t)__popc(m);
-    base = __shfl_sync(0xFFFFFFFFu, base, leader);
-    if (valid) ent[__ldg(cell_start + c) + base + __popc(m & ((1u << lane) - 1u))] = make_uint2(k, (uint32_t)i);
+    if (i >= N) return;
+    const uint32_t k = __ldg(key + i);
+    ent[__ldg(cell_start + (k >> cell_shift)) + __ldg(rank + i)] = make_uint2(k, (uint32_t)i);
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -687,6 +719,53 @@ __device__ void sort_cell(unsigned long long *kv, int n, int rank) {
     coop_sync<G>();
 }
 
+// A warp's cell (n <= CELL_WARP_MAX): rank by counting.  Every lane keeps its own entries in registers, every entry
+// is broadcast once from shared memory and counted against them; all keys are distinct (the index is part of them).
+__device__ __forceinline__ void sort_cell_warp(unsigned long long *kv, int n, int lane) {
+    constexpr int Q = CELL_WARP_MAX / 32;
+    unsigned long long mine[Q];
+    int below[Q];
+#pragma unroll
+    for (int q = 0; q < Q; ++q) {
+        mine[q] = (lane + 32 * q < n) ? kv[lane + 32 * q] : ~0ull;
+        below[q] = 0;
+    }
+    __syncwarp();
+    if (n <= 32) {
+#pragma unroll 4
+        for (int jj = 0; jj < n; ++jj) below[0] += kv[jj] < mine[0];
+    } else {
+#pragma unroll 2
+        for (int jj = 0; jj < n; ++jj) {
+            const unsigned long long v = kv[jj];
+#pragma unroll
+            for (int q = 0; q < Q; ++q) below[q] += v < mine[q];
+        }
+    }
+    __syncwarp();
+#pragma unroll
+    for (int q = 0; q < Q; ++q)
+        if (lane + 32 * q < n) kv[below[q]] = mine[q];
+    __syncwarp();
+}
+
+// packed-box union of the particles at local positions [f, l] of a warp's cell
+__device__ __forceinline__ void range_box(const CellArrays &A, int f, int l, int lane, uint32_t &lo, uint32_t &hi) {
+    uint32_t x0 = 1023u, y0 = 1023u, z0 = 1023u, x1 = 0u, y1 = 0u, z1 = 0u;
+    for (int p = f + lane; p <= l; p += 32) {
+        const uint32_t a = A.wlo[p], b = A.whi[p];
+        x0 = min(x0, a & 1023u), y0 = min(y0, (a >> 10) & 1023u), z0 = min(z0, (a >> 20) & 1023u);
+        x1 = max(x1, b & 1023u), y1 = max(y1, (b >> 10) & 1023u), z1 = max(z1, (b >> 20) & 1023u);
+    }
+    const uint32_t FULL = 0xFFFFFFFFu;
+    // one reduction per bound: the three 10-bit fields travel in one word (min of the sum is not the sum of the
+    // mins, so the fields are reduced one by one)
+    x0 = __reduce_min_sync(FULL, x0), y0 = __reduce_min_sync(FULL, y0), z0 = __reduce_min_sync(FULL, z0);
+    x1 = __reduce_max_sync(FULL, x1), y1 = __reduce_max_sync(FULL, y1), z1 = __reduce_max_sync(FULL, z1);
+    lo = x0 | (y0 << 10) | (z0 << 20);
+    hi = x1 | (y1 << 10) | (z1 << 20);
+}
+
 template <int G>
 __device__ void process_cell(const TreeCtx &cx, const CellArrays A, int j, int rank, bool kv_is_ent) {
     const int N = cx.N, lvl = cx.lvl;
@@ -715,7 +794,12 @@ __device__ void process_cell(const TreeCtx &cx, const CellArrays A, int j, int r
             const uint2 e = cx.ent[F + p];
             A.kv[p] = ((unsigned long long)e.x << 32) | e.y;
         }
-    sort_cell<G>(A.kv, n, rank);
+    if (G == 32) {
+        __syncwarp();
+        sort_cell_warp(A.kv, n, rank);
+    } else {
+        sort_cell<G>(A.kv, n, rank);
+    }
     const float *fr = cx.meta->frames[t];
     // ---- a2' gather, a6 quantize, leaf state ----
     for (int p = rank; p < n; p += G) {
@@ -762,6 +846,68 @@ __device__ void process_cell(const TreeCtx &cx, const CellArrays A, int j, int r
     };
     auto keyat = [&](int k) { return (uint32_t)(A.kv[k - F] >> 32); };
     auto pfx = [&](int f, int l) { return delta_aug(keyat(f), f, keyat(l), l); };
+    if (G == 32 && cx.K > 1 && rb[0] < 0 && gmax >= cx.K) {
+        // (gmax >= K: query groups are unions of range leaves, so none has to be cut out of a leaf's inside)
+        // ---- Collapse by size alone (no cost hint): a node is a range leaf iff it holds <= K particles, so only the
+        //      nodes with more than K particles exist as internal nodes.  They are split top down — the split of a
+        //      range is where the highest differing bit of its first and last augmented key flips —
+        //      and nothing below the range leaves is ever touched.  Same tree as the rounds below would give. ----
+        const int lane = rank;
+        int written = 0;
+        CellRoot r;
+        r.first = F, r.last = F + n - 1, r.dL = dLc, r.dR = dRc, r.pad[0] = r.pad[1] = 0;
+        if (n <= cx.K) {
+            uint32_t lo, hi;
+            range_box(A, 0, n - 1, lane, lo, hi);
+            r.wlo = lo | 0x80000000u, r.whi = hi;      // pending: the top-level walk decides
+        } else {
+            auto aug = [&](int p) { return (A.kv[p] & 0xFFFFFFFF00000000ull) | (unsigned long long)(uint32_t)(F + p); };
+            int32_t *stack = A.mrg;                      // entries f | l << 8 | (dL+1) << 16 | (dR+1) << 24
+            int sp = 0;
+            if (lane == 0) stack[0] = 0 | ((n - 1) << 8) | ((dLc + 1) << 16) | ((dRc + 1) << 24);
+            sp = 1;
+            __syncwarp();
+            while (sp > 0) {
+                const uint32_t ent = (uint32_t)stack[--sp];
+                __syncwarp();
+                const int f = ent & 255u, l = (ent >> 8) & 255u, dL = (int)((ent >> 16) & 255u) - 1, dR = (int)(ent >> 24) - 1;
+                const int bit = 63 - __clzll((long long)(aug(f) ^ aug(l)));
+                int g = l;                               // first position whose key has the bit set
+                for (int base = f + 1; base <= l; base += 32) {
+                    const int p = base + lane;
+                    const uint32_t m = __ballot_sync(0xFFFFFFFFu, p <= l && ((aug(p) >> bit) & 1ull));
+                    if (m) {
+                        g = base + __ffs(m) - 1;
+                        break;
+                    }
+                }
+                const int gam = g - 1, dsplit = 63 - bit;
+                Child a, b;
+                a.f = F + f, a.l = F + gam, b.f = F + gam + 1, b.l = F + l;
+                range_box(A, f, gam, lane, a.wlo, a.whi);
+                range_box(A, gam + 1, l, lane, b.wlo, b.whi);
+                const int ca = gam - f + 1, cb = l - gam;
+                a.pend = ca <= cx.K, b.pend = cb <= cx.K;
+                if (lane == 0) {
+                    uint32_t ulo, uhi;
+                    int w = 0;
+                    // cnt > K: form_parent never collapses this node; it writes it and its pending children
+                    form_parent(cx, t, s_seg, gmax, rb, keyat, a, b, dL, dR, dsplit, rope_of(l, dR), pfx, ulo, uhi, w);
+                    written += w;
+                    if (f == 0 && l == n - 1) r.wlo = ulo, r.whi = uhi;
+                    if (!a.pend) stack[sp] = f | (gam << 8) | ((dL + 1) << 16) | ((dsplit + 1) << 24);
+                    if (!b.pend) stack[sp + (a.pend ? 0 : 1)] = (gam + 1) | (l << 8) | ((dsplit + 1) << 16) | ((dR + 1) << 24);
+                }
+                sp += (a.pend ? 0 : 1) + (b.pend ? 0 : 1);
+                __syncwarp();
+            }
+        }
+        if (lane == 0) {
+            cx.croot[j] = r;
+            if (written) atomicAdd(&cx.meta->nodes_emitted, written);
+        }
+        return;
+    }
     // ---- a3..a6 inside the cell: rounds of merges.  A segment that is a left child (dR > dL) merges with the segment
     //      that starts right after it if that one is a right child: then they are siblings.  Height of the cell's
     //      subtree rounds; no atomics. ----
@@ -914,15 +1060,14 @@ cudaError_t launch_build(const void *pos, const int32_t *type, const BuildParams
     const int entry_words = QBVH_TMAX * ENTRY_CELLS;
     const float3 lo = make_float3(p.box_lo[0], p.box_lo[1], p.box_lo[2]);
     const float3 sc = make_float3(p.box_scale[0], p.box_scale[1], p.box_scale[2]);
-    int mblocks = (N / 4 + MORTON_THREADS - 1) / MORTON_THREADS;
-    mblocks = max(1, min(mblocks, sms * 2));
+    const int mblocks = ((N + 3) / 4 + MORTON_THREADS - 1) / MORTON_THREADS;
 #define QBVH_MORTON(NT)                                                                                                        \
     if (p.f64)                                                                                                                 \
         morton_cell_kernel<NT, double><<<mblocks, MORTON_THREADS, 0, st>>>(static_cast<const double *>(pos), type, N, lo, sc,  \
-                                                                          cell_shift, b.key, b.cell_count, b.meta, b.entry, entry_words); \
+                                                                          cell_shift, b.key, b.rank, b.cell_count, b.meta, b.entry, entry_words); \
     else                                                                                                                       \
         morton_cell_kernel<NT, float><<<mblocks, MORTON_THREADS, 0, st>>>(static_cast<const float *>(pos), type, N, lo, sc,    \
-                                                                         cell_shift, b.key, b.cell_count, b.meta, b.entry, entry_words);
+                                                                         cell_shift, b.key, b.rank, b.cell_count, b.meta, b.entry, entry_words);
     switch (p.T) {
         case 1: QBVH_MORTON(1) break;
         case 2: QBVH_MORTON(2) break;
@@ -935,7 +1080,7 @@ cudaError_t launch_build(const void *pos, const int32_t *type, const BuildParams
     for (int t = 0; t < QBVH_TMAX; ++t) fp.r_hint[t] = p.r_hint[t];
     const int tiles = (ncells + SCAN_TILE - 1) / SCAN_TILE;
     cell_scan_kernel<<<tiles, SCAN_THREADS, 0, st>>>(b.cell_count, b.cell_start, b.cell_list, ncells, b.meta, fp);
-    cell_scatter_kernel<<<(N + 255) / 256, 256, 0, st>>>(b.key, N, cell_shift, b.cell_count, b.cell_start, b.ent);
+    cell_scatter_kernel<<<(N + 255) / 256, 256, 0, st>>>(b.key, b.rank, N, cell_shift, b.cell_start, b.ent);
     TreeCtx cx;
     cx.pos = pos, cx.f64 = p.f64 ? 1 : 0, cx.N = N, cx.K = p.K, cx.lvl = lvl, cx.build_tag = p.build_tag;
     cx.cell_start = b.cell_start, cx.cell_list = b.cell_list, cx.ent = b.ent;

@@ -20,7 +20,8 @@ constexpr int SCAN_MAX_TILES = CELL_MAX_TOTAL / SCAN_TILE;   // 128
 
 // Device-resident bookkeeping of one build (lives at the start of the workspace; zeroed by a memset per build).
 struct TreeMeta {
-    unsigned long long scan_status[SCAN_MAX_TILES];  // decoupled look-back of the cell scan: flag << 62 | nonempty << 32 | count
+    unsigned long long scan_status[SCAN_MAX_TILES];  // cell scan: total of every tile, non-empty cells << 32 | particles
+    uint32_t scan_arrived;          // tiles of the scan that have published their total (grid-wide barrier)
     uint32_t scan_done;             // tiles of the scan that have finished (the last one finalizes)
     uint32_t mm_enc[QBVH_TMAX][6];  // per type: ~enc(min xyz) (so atomicMax computes the min), enc(max xyz)
     int32_t seg[QBVH_TMAX + 1];     // first sorted position of each type; seg[T..4] = N
@@ -30,7 +31,7 @@ struct TreeMeta {
     int32_t rbin[QBVH_TMAX][4];     // collapse heuristic: expected query radius against this tree in bins per axis; [0] < 0: none
     int32_t ncell;                  // number of non-empty cells
     int32_t nbig;                   // cells larger than CELL_WARP_MAX (handled by whole blocks)
-    int32_t pad_[24];
+    int32_t pad_[23];
     // the counters below, hammered by atomics, keep a 128-byte line of their own
     int32_t group_count;            // number of query groups emitted by the build
     int32_t group_cursor;           // next group to hand out (dynamic scheduling of the traversal); reset per traversal
@@ -105,9 +106,10 @@ struct __align__(32) Pos64 {
 struct BuildBuffers {
     TreeMeta *meta;
     uint32_t *key;                 // Morton keys in input order
+    uint32_t *rank;                // place of every particle inside its cell (order of arrival)
     uint2 *ent;                    // {key, original index} partitioned by cell, then sorted inside each cell
     uint32_t *key_sorted, *idx_sorted;
-    uint32_t *cell_count;          // [ncells] particles per cell; counted by the key kernel, counted back to 0 by the scatter
+    uint32_t *cell_count;          // [ncells] particles per cell; counted by the key kernel, cleared again by the scan
     uint32_t *cell_start;          // [ncells + 1] exclusive prefix
     uint32_t *cell_list;           // non-empty cells in ascending order
     int32_t *big_list;             // compact indices of the cells larger than CELL_WARP_MAX
