@@ -74,8 +74,8 @@ int qbvh_set_workspace(void *dev_ptr, int64_t bytes);
 #define QBVH_OPT_VARIANT 3       /* which traversal kernel qbvh_neighbors launches: 0 = Algorithm 1 as written, one
                                     thread per particle; 1 (default) = one warp per query group.
                                     Both produce identical lists.                                                 */
-#define QBVH_OPT_DEBUG_BUILD_TAG 4 /* testing only: v in [1, 2^24): the next qbvh_build on this workspace uses meeting-
-                                    slot tag v (forward jumps only) — lets a test reach the 24-bit wrap.           */
+#define QBVH_OPT_DEBUG_BUILD_TAG 4 /* testing only: v in [1, 2^18): the next qbvh_build on this workspace uses meeting-
+                                    slot tag v (forward jumps only) — lets a test reach the 18-bit wrap.           */
 int qbvh_set_option(int32_t key, int32_t value);
 
 /* Hint for the build-side subtree collapse ("collapse subtrees according to an appropriate heuristic",

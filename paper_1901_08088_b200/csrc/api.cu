@@ -215,9 +215,9 @@ int build_impl(const void *pos, bool f64, const int32_t *type, int64_t N, const 
     bp.lvl = pick_cell_level(N, bp.T);
     bp.f64 = f64;
     for (int t = 0; t < QBVH_TMAX; ++t) bp.r_hint[t] = g.r_hint[t];
-    // The meeting slots of the top-level walk carry a 24-bit build number and the cell counters are counted back to
+    // The meeting slots of the top-level walk carry an 18-bit build number and the cell counters are counted back to
     // zero by every build: both are cleared only when the layout moves or the number wraps.
-    if (g.build_tag == 0 || g.build_tag >= 0xFFFFFFu || g.tag_N != N || g.tag_lvl != bp.lvl || g.tag_T != bp.T) {
+    if (g.build_tag == 0 || g.build_tag >= QBVH_TAG_MAX || g.tag_N != N || g.tag_lvl != bp.lvl || g.tag_T != bp.T) {
         cudaError_t em = cudaMemsetAsync(g.buf.slot, 0, (size_t)16 * (size_t)(N > 0 ? N : 1), g.stream);
         if (em == cudaSuccess) em = cudaMemsetAsync(g.buf.cell_count, 0, (size_t)4 * CELL_MAX_TOTAL, g.stream);
         if (em != cudaSuccess) return cuda_fail(em, "memset slots");
@@ -282,7 +282,7 @@ int qbvh_set_option(int32_t key, int32_t value) {
             return QBVH_OK;
         case QBVH_OPT_DEBUG_BUILD_TAG:
             // only forward: slots of earlier builds carry smaller tags and must never match a later build
-            if (value < 1 || value > 0xFFFFFF || (uint32_t)value <= g.build_tag) return QBVH_ERR_INVALID_ARG;
+            if (value < 1 || value > (int32_t)QBVH_TAG_MAX || (uint32_t)value <= g.build_tag) return QBVH_ERR_INVALID_ARG;
             if (g.build_tag != 0) g.build_tag = (uint32_t)value - 1;   // a slot area still to be cleared stays at tag 0
             return QBVH_OK;
         default:

@@ -118,13 +118,18 @@ __global__ void __launch_bounds__(MORTON_THREADS) morton_cell_kernel(const PT *_
                 mx[v][2] = m ? fmaxf(mx[v][2], z) : mx[v][2];
             }
         }
-        const uint32_t c = valid ? (key[u] >> cell_shift) : 0xFFFFFFFFu;
-        const uint32_t m = __match_any_sync(0xFFFFFFFFu, c);
-        const int leader = __ffs(m) - 1;
-        uint32_t base = 0;
-        if (valid && lane == leader) base = atomicAdd(&cell_count[c], (uint32_t)__popc(m));
-        rank[u] = __shfl_sync(0xFFFFFFFFu, base, leader) + __popc(m & ((1u << lane) - 1u));
     }
+    // the four draws of a thread are independent: all atomics are issued before the first result is used
+    uint32_t grp[4], base[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) grp[u] = __match_any_sync(0xFFFFFFFFu, (i0 + u < N) ? (key[u] >> cell_shift) : 0xFFFFFFFFu);
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+        base[u] = 0;
+        if (i0 + u < N && lane == __ffs(grp[u]) - 1) base[u] = atomicAdd(&cell_count[key[u] >> cell_shift], (uint32_t)__popc(grp[u]));
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) rank[u] = __shfl_sync(0xFFFFFFFFu, base[u], __ffs(grp[u]) - 1) + __popc(grp[u] & ((1u << lane) - 1u));
     if (full && ((reinterpret_cast<uintptr_t>(key_out) & 15) == 0) && ((reinterpret_cast<uintptr_t>(rank_out) & 15) == 0)) {
         reinterpret_cast<uint4 *>(key_out)[gtid] = make_uint4(key[0], key[1], key[2], key[3]);
         reinterpret_cast<uint4 *>(rank_out)[gtid] = make_uint4(rank[0], rank[1], rank[2], rank[3]);
@@ -223,52 +228,60 @@ __device__ void finalize_block(TreeMeta *__restrict__ meta, const uint32_t *__re
     }
 }
 
-// One tile of SCAN_TILE cells per block.  No chain between the tiles: every block publishes its tile's total, all
-// blocks meet at a grid-wide barrier (at most SCAN_MAX_TILES = 128 blocks: all resident at once), then every block
-// sums the totals before it.  Reading a counter also clears it for the next build.
-__global__ void __launch_bounds__(SCAN_THREADS) cell_scan_kernel(uint32_t *__restrict__ cell_count,
+// One tile of SCAN_TILE cells per block.  No chain between the tiles.  Up to SCAN_DIRECT_TILES tiles every block
+// simply adds up the counters of all tiles before its own (a few hundred KB out of L2) and nothing waits for anything;
+// beyond that every block publishes its tile's total and all blocks meet at a grid-wide barrier (at most
+// SCAN_MAX_TILES = 128 blocks: all resident at once).  The kernel is a handful of dependent L2 round trips.
+constexpr int SCAN_DIRECT_TILES = 32;
+__global__ void __launch_bounds__(SCAN_THREADS) cell_scan_kernel(const uint32_t *__restrict__ cell_count,
                                                                   uint32_t *__restrict__ cell_start,
                                                                   uint32_t *__restrict__ cell_list, int ncells,
-                                                                  TreeMeta *__restrict__ meta, const FinalizeParams fp) {
-    __shared__ unsigned long long s_warp[SCAN_THREADS / 32];
-    __shared__ unsigned long long s_excl;
-    __shared__ bool s_last;
+                                                                  TreeMeta *__restrict__ meta) {
+    __shared__ unsigned long long s_warp[SCAN_THREADS / 32], s_pre[SCAN_THREADS / 32];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int tile = blockIdx.x, ntiles = gridDim.x;
     const int c0 = tile * SCAN_TILE + tid * SCAN_IPT;
+    auto value = [](uint32_t c) { return (unsigned long long)c | ((unsigned long long)(c != 0) << 32); };   // particles, non-empty cells << 32
     uint32_t cnt[SCAN_IPT];
     if (c0 + SCAN_IPT <= ncells) {
         const uint4 a = __ldcg(reinterpret_cast<const uint4 *>(cell_count + c0)), b = __ldcg(reinterpret_cast<const uint4 *>(cell_count + c0) + 1);
         cnt[0] = a.x, cnt[1] = a.y, cnt[2] = a.z, cnt[3] = a.w, cnt[4] = b.x, cnt[5] = b.y, cnt[6] = b.z, cnt[7] = b.w;
-        reinterpret_cast<uint4 *>(cell_count + c0)[0] = make_uint4(0u, 0u, 0u, 0u);
-        reinterpret_cast<uint4 *>(cell_count + c0)[1] = make_uint4(0u, 0u, 0u, 0u);
     } else {
 #pragma unroll
-        for (int u = 0; u < SCAN_IPT; ++u) {
-            cnt[u] = (c0 + u < ncells) ? __ldcg(cell_count + c0 + u) : 0u;
-            if (c0 + u < ncells) cell_count[c0 + u] = 0u;
+        for (int u = 0; u < SCAN_IPT; ++u) cnt[u] = (c0 + u < ncells) ? __ldcg(cell_count + c0 + u) : 0u;
+    }
+    // sum of everything before this tile, read directly (tiles are full except the last)
+    unsigned long long before = 0;
+    if (ntiles <= SCAN_DIRECT_TILES) {
+        const uint4 *src = reinterpret_cast<const uint4 *>(cell_count);
+        for (int q = tid; q < tile * (SCAN_TILE / 4); q += SCAN_THREADS) {
+            const uint4 v = __ldcg(src + q);
+            before += value(v.x) + value(v.y) + value(v.z) + value(v.w);
         }
     }
-    // value = count in the low word, number of non-empty cells in the high word
     unsigned long long mine = 0;
 #pragma unroll
-    for (int u = 0; u < SCAN_IPT; ++u) mine += (unsigned long long)cnt[u] | ((unsigned long long)(cnt[u] != 0) << 32);
+    for (int u = 0; u < SCAN_IPT; ++u) mine += value(cnt[u]);
     unsigned long long inc = mine;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
         const unsigned long long v = __shfl_up_sync(0xFFFFFFFFu, inc, o);
         if (lane >= o) inc += v;
     }
+#pragma unroll
+    for (int o = 16; o; o >>= 1) before += __shfl_xor_sync(0xFFFFFFFFu, before, o);
     if (lane == 31) s_warp[warp] = inc;
+    if (lane == 0) s_pre[warp] = before;
     __syncthreads();
-    unsigned long long wbase = 0, total = 0;
+    unsigned long long wbase = 0, total = 0, excl = 0;
 #pragma unroll
     for (int w = 0; w < SCAN_THREADS / 32; ++w) {
         if (w < warp) wbase += s_warp[w];
         total += s_warp[w];
+        excl += s_pre[w];
     }
-    volatile unsigned long long *tot = meta->scan_status;
-    if (ntiles > 1) {
+    if (ntiles > SCAN_DIRECT_TILES) {
+        volatile unsigned long long *tot = meta->scan_status;
         if (tid == 0) {
             tot[tile] = total;
             __threadfence();
@@ -277,45 +290,29 @@ __global__ void __launch_bounds__(SCAN_THREADS) cell_scan_kernel(uint32_t *__res
             __threadfence();
         }
         __syncthreads();
-        // exclusive prefix of the tile: the totals of the tiles before it (ntiles <= 128 <= SCAN_THREADS)
-        unsigned long long v = (tid < tile) ? tot[tid] : 0ull;
+        unsigned long long v = (tid < tile) ? tot[tid] : 0ull;     // ntiles <= 128 <= SCAN_THREADS
 #pragma unroll
         for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, o);
         __syncthreads();
-        if (lane == 0) s_warp[warp] = v;
+        if (lane == 0) s_pre[warp] = v;
         __syncthreads();
-        if (tid == 0) {
-            unsigned long long e = 0;
-            for (int w = 0; w < SCAN_THREADS / 32; ++w) e += s_warp[w];
-            s_excl = e;
-        }
-    } else if (tid == 0) {
-        s_excl = 0;
+        excl = 0;
+#pragma unroll
+        for (int w = 0; w < SCAN_THREADS / 32; ++w) excl += s_pre[w];
     }
-    __syncthreads();
-    unsigned long long run = s_excl + wbase + inc - mine;
+    unsigned long long run = excl + wbase + inc - mine;
 #pragma unroll
     for (int u = 0; u < SCAN_IPT; ++u) {
         if (c0 + u < ncells) {
             cell_start[c0 + u] = (uint32_t)run;
             if (cnt[u]) cell_list[(uint32_t)(run >> 32)] = (uint32_t)(c0 + u);
         }
-        run += (unsigned long long)cnt[u] | ((unsigned long long)(cnt[u] != 0) << 32);
+        run += value(cnt[u]);
     }
     if (tile == ntiles - 1 && tid == SCAN_THREADS - 1) {
         cell_start[ncells] = (uint32_t)run;              // = N
         meta->ncell = (int32_t)(run >> 32);
     }
-    // the last block to get here finalizes.  One cumulative fence by thread 0 after the barrier orders the whole
-    // block's stores before its ticket.
-    __syncthreads();
-    if (tid == 0) {
-        __threadfence();
-        s_last = atomicAdd(&meta->scan_done, 1u) == gridDim.x - 1;
-        __threadfence();
-    }
-    __syncthreads();
-    if (s_last) finalize_block(meta, cell_start, fp);
 }
 
 // N = 0: only the bookkeeping
@@ -336,11 +333,17 @@ __global__ void finalize_empty_kernel(TreeMeta *__restrict__ meta) {
 // ------------------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) cell_scatter_kernel(const uint32_t *__restrict__ key, const uint32_t *__restrict__ rank,
                                                             int N, int cell_shift, const uint32_t *__restrict__ cell_start,
-                                                            uint2 *__restrict__ ent) {
+                                                            uint2 *__restrict__ ent, uint32_t *__restrict__ cell_count, int ncells,
+                                                            TreeMeta *__restrict__ meta, const FinalizeParams fp) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= N) return;
-    const uint32_t k = __ldg(key + i);
-    ent[__ldg(cell_start + (k >> cell_shift)) + __ldg(rank + i)] = make_uint2(k, (uint32_t)i);
+    // the counters have been scanned: clear them for the next build
+    for (int c = i; c < ncells; c += gridDim.x * blockDim.x) cell_count[c] = 0u;
+    if (i < N) {
+        const uint32_t k = __ldg(key + i);
+        ent[__ldg(cell_start + (k >> cell_shift)) + __ldg(rank + i)] = make_uint2(k, (uint32_t)i);
+    }
+    // type segments, roots, quantization frames: needed by the next launch only; one block does it on the side
+    if (blockIdx.x == gridDim.x - 1) finalize_block(meta, cell_start, fp);
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -522,9 +525,10 @@ __device__ __forceinline__ void emit_groups(TreeMeta *meta, uint2 *__restrict__ 
 // Form the parent of the adjacent children a (left) and b (right).  dL, dR: the parent's outer prefix lengths;
 // dsplit = delta(a.l, b.f): the parent's own prefix length.  rope_p: the parent's rope (and b's).  pfx(f, l): common
 // prefix length of the keys at sorted positions f and l.  Returns whether the parent is pending; ulo/uhi: its box.
-// keyat(k): key at sorted position k (asked only for a.f and for the first position of a pending child).
+// kparent: any key below the parent (entry table); keyat(k): key at sorted position k, asked for the particles of
+// pending children only.
 template <class KeyF, class PfxF>
-__device__ __forceinline__ bool form_parent(const TreeCtx &cx, int t, int s_seg, int gmax, const int32_t *rb, KeyF keyat,
+__device__ __forceinline__ bool form_parent(const TreeCtx &cx, int t, int s_seg, int gmax, const int32_t *rb, uint32_t kparent, KeyF keyat,
                                             const Child a, const Child b, int dL, int dR, int dsplit, int rope_p, PfxF pfx,
                                             uint32_t &ulo, uint32_t &uhi, int &written) {
     const int N = cx.N;
@@ -547,7 +551,7 @@ __device__ __forceinline__ bool form_parent(const TreeCtx &cx, int t, int s_seg,
         cx.parent[rc] = id;
         if (root) cx.parent[id] = -1;
         int32_t *const etab = cx.entry + t * ENTRY_CELLS;
-        if (max(dL, dR) < 2 + 3 * ENTRY_LMAX) emit_entry(etab, keyat(a.f), max(dL, dR), dsplit, id);
+        emit_entry(etab, kparent, max(dL, dR), dsplit, id);
         written = 1;
         if (a.pend) {
             cx.nodes[lc] = make_int4((int)a.wlo, (int)a.whi, ~a.f, rc);
@@ -586,21 +590,24 @@ __device__ __forceinline__ void write_pending_root(const TreeCtx &cx, int t, Key
 }
 
 // Walk up from a finished subtree (a cell root) through the levels above the cells.  The two children of a node meet at
-// slot[gamma]: the first to arrive leaves {its packed box + pending bit, the far end of its range, its outer delta,
-// the build's tag} there with ONE 128-bit atomic exchange and retires; the second takes them and forms the parent
-// ("walking up the tree from the leaf nodes").  Slots are tagged with a per-build number instead of being
-// cleared every build.  A node up here covers whole cells, so its rope follows from the cell table alone (jl: compact
-// index of its last cell): no key of a neighbouring cell is read, which may still be sorting in this very launch.  A
-// right child's "far end" travels as jl (its last position is that cell's end), a left child's as its first position.
-__device__ void walk_up(const TreeCtx &cx, Child me, int dL, int dR, int jl) {
+// slot[gamma]: the first to arrive leaves a 16-byte record there with ONE 128-bit atomic exchange and retires; the
+// second takes it and forms the parent ("walking up the tree from the leaf nodes").  Record:
+//   x = packed lower bound | pending << 31      y = packed upper bound
+//   z = far end of the range (a left child: its first position, a right child: its last)
+//   w = build tag << 14 | (dnext + 1) << 7 | (outer delta + 1)
+// dnext (right children): delta(m, m+1) for m = last + 1, the first particle of the NEXT cell, known from the cell
+// table when the cell was built (64 if that cell holds two or more particles) — with it the parent's rope needs no
+// key at all, so a level of the walk is one L2 round trip.  Slots are tagged with an 18-bit per-build number instead
+// of being cleared every build.
+static_assert(QBVH_TAG_MAX == (1u << 18) - 1, "the tag shares a word with two 7-bit prefix lengths");
+__device__ void walk_up(const TreeCtx &cx, Child me, int dL, int dR, int dnext) {
     const uint32_t *key = cx.key_sorted;
-    const uint32_t ki = key[me.f];
-    const int t = ki >> 30;
+    const uint32_t ki = key[me.f];                         // the walker's own cell: sorted before the walk starts
+    const int t = (int)(ki >> 30);
     const int s_seg = cx.meta->seg[t];
     const int gmax = cx.meta->gmax[t];
-    const int ncell = cx.meta->ncell;
     const int32_t *rb = cx.meta->rbin[t];
-    auto keyat = [&](int k) { return key[k]; };           // asked for pending children only: small cells, sorted by the previous launch
+    auto keyat = [&](int k) { return key[k]; };           // asked for a.f and for pending children only: small cells, sorted by the previous launch
     auto pfx = [&](int f, int l) { return delta_aug(key[f], f, key[l], l); };
     int written = 0;
     while (true) {
@@ -614,10 +621,10 @@ __device__ void walk_up(const TreeCtx &cx, Child me, int dL, int dR, int jl) {
         }
         const bool is_left = dR > dL;
         const int gamma = is_left ? me.l : me.f - 1;
-        const uint4 mine = make_uint4(me.wlo | (me.pend ? 0x80000000u : 0u), me.whi, (uint32_t)(is_left ? me.f : jl),
-                                      (cx.build_tag << 8) | (uint32_t)((is_left ? dL : dR) + 1));
+        const uint4 mine = make_uint4(me.wlo | (me.pend ? 0x80000000u : 0u), me.whi, (uint32_t)(is_left ? me.f : me.l),
+                                      (cx.build_tag << 14) | ((uint32_t)(dnext + 1) << 7) | (uint32_t)((is_left ? dL : dR) + 1));
         const uint4 other = exch128(cx.slot + gamma, mine);
-        if ((other.w >> 8) != cx.build_tag) break;   // first to arrive: the sibling will carry on
+        if ((other.w >> 14) != cx.build_tag) break;  // first to arrive: the sibling will carry on
         const int dsplit = is_left ? dR : dL;        // delta(gamma, gamma+1): the parent's own prefix length
         Child sib;
         sib.wlo = other.x & 0x7FFFFFFFu;
@@ -625,29 +632,21 @@ __device__ void walk_up(const TreeCtx &cx, Child me, int dL, int dR, int jl) {
         sib.pend = (other.x >> 31) != 0;
         Child a, b;
         if (is_left) {
-            jl = (int)other.z;
             sib.f = gamma + 1;
-            sib.l = (int)__ldg(cx.cell_start + __ldg(cx.cell_list + jl) + 1) - 1;
-            dR = (int)(other.w & 255u) - 1;
+            sib.l = (int)other.z;
+            dR = (int)(other.w & 127u) - 1;
+            dnext = (int)((other.w >> 7) & 127u) - 1;
             a = me, b = sib;
         } else {
             sib.f = (int)other.z;
             sib.l = gamma;
-            dL = (int)(other.w & 255u) - 1;
+            dL = (int)(other.w & 127u) - 1;
             a = sib, b = me;
         }
-        int rope_p = -1;
-        if (dR >= 0) {                               // another cell of this type follows: what starts at m = b.l + 1?
-            const int m = b.l + 1;
-            const uint32_t cn = __ldg(cx.cell_list + jl + 1);
-            int dnext = 64;                          // two or more particles in that cell: internal node m starts there
-            if (__ldg(cx.cell_start + cn + 1) - __ldg(cx.cell_start + cn) == 1u)
-                dnext = (jl + 2 < ncell) ? delta_cells(cn, __ldg(cx.cell_list + jl + 2), cx.lvl) : -1;
-            rope_p = dnext > dR ? m : cx.N - 1 + m;
-        }
+        const int rope_p = dR < 0 ? -1 : (dnext > dR ? b.l + 1 : cx.N + b.l);   // internal node m or leaf N-1+m, m = b.l + 1
         uint32_t ulo, uhi;
         int w = 0;
-        const bool pend = form_parent(cx, t, s_seg, gmax, rb, keyat, a, b, dL, dR, dsplit, rope_p, pfx, ulo, uhi, w);
+        const bool pend = form_parent(cx, t, s_seg, gmax, rb, ki, keyat, a, b, dL, dR, dsplit, rope_p, pfx, ulo, uhi, w);
         written += w;
         me.wlo = ulo, me.whi = uhi, me.f = a.f, me.l = b.l, me.pend = pend;
     }
@@ -721,8 +720,8 @@ __device__ void sort_cell(unsigned long long *kv, int n, int rank) {
 
 // A warp's cell (n <= CELL_WARP_MAX): rank by counting.  Every lane keeps its own entries in registers, every entry
 // is broadcast once from shared memory and counted against them; all keys are distinct (the index is part of them).
-__device__ __forceinline__ void sort_cell_warp(unsigned long long *kv, int n, int lane) {
-    constexpr int Q = CELL_WARP_MAX / 32;
+template <int Q>
+__device__ __forceinline__ void sort_cell_warp_q(unsigned long long *kv, int n, int lane) {
     unsigned long long mine[Q];
     int below[Q];
 #pragma unroll
@@ -731,22 +730,23 @@ __device__ __forceinline__ void sort_cell_warp(unsigned long long *kv, int n, in
         below[q] = 0;
     }
     __syncwarp();
-    if (n <= 32) {
 #pragma unroll 4
-        for (int jj = 0; jj < n; ++jj) below[0] += kv[jj] < mine[0];
-    } else {
-#pragma unroll 2
-        for (int jj = 0; jj < n; ++jj) {
-            const unsigned long long v = kv[jj];
+    for (int jj = 0; jj < n; ++jj) {
+        const unsigned long long v = kv[jj];
 #pragma unroll
-            for (int q = 0; q < Q; ++q) below[q] += v < mine[q];
-        }
+        for (int q = 0; q < Q; ++q) below[q] += v < mine[q];
     }
     __syncwarp();
 #pragma unroll
     for (int q = 0; q < Q; ++q)
         if (lane + 32 * q < n) kv[below[q]] = mine[q];
     __syncwarp();
+}
+__device__ __forceinline__ void sort_cell_warp(unsigned long long *kv, int n, int lane) {
+    static_assert(CELL_WARP_MAX == 128, "four entries per lane at most");
+    if (n <= 32) sort_cell_warp_q<1>(kv, n, lane);
+    else if (n <= 64) sort_cell_warp_q<2>(kv, n, lane);
+    else sort_cell_warp_q<4>(kv, n, lane);
 }
 
 // packed-box union of the particles at local positions [f, l] of a warp's cell
@@ -855,7 +855,7 @@ __device__ void process_cell(const TreeCtx &cx, const CellArrays A, int j, int r
         const int lane = rank;
         int written = 0;
         CellRoot r;
-        r.first = F, r.last = F + n - 1, r.dL = dLc, r.dR = dRc, r.pad[0] = r.pad[1] = 0;
+        r.first = F, r.last = F + n - 1, r.dL = dLc, r.dR = dRc, r.dnext = n_next >= 2 ? 64 : dNN, r.pad = 0;
         if (n <= cx.K) {
             uint32_t lo, hi;
             range_box(A, 0, n - 1, lane, lo, hi);
@@ -892,7 +892,7 @@ __device__ void process_cell(const TreeCtx &cx, const CellArrays A, int j, int r
                     uint32_t ulo, uhi;
                     int w = 0;
                     // cnt > K: form_parent never collapses this node; it writes it and its pending children
-                    form_parent(cx, t, s_seg, gmax, rb, keyat, a, b, dL, dR, dsplit, rope_of(l, dR), pfx, ulo, uhi, w);
+                    form_parent(cx, t, s_seg, gmax, rb, keyat(a.f), keyat, a, b, dL, dR, dsplit, rope_of(l, dR), pfx, ulo, uhi, w);
                     written += w;
                     if (f == 0 && l == n - 1) r.wlo = ulo, r.whi = uhi;
                     if (!a.pend) stack[sp] = f | (gam << 8) | ((dL + 1) << 16) | ((dsplit + 1) << 24);
@@ -932,8 +932,8 @@ __device__ void process_cell(const TreeCtx &cx, const CellArrays A, int j, int r
             const int dL = A.dL[p], dR = A.dR[s], dsplit = A.dR[p];
             uint32_t ulo, uhi;
             int w = 0;
-            const bool pend = form_parent(cx, t, s_seg, gmax, rb, keyat, a, b, dL, dR, dsplit, rope_of(b.l - F, dR), pfx,
-                                          ulo, uhi, w);
+            const bool pend = form_parent(cx, t, s_seg, gmax, rb, keyat(a.f), keyat, a, b, dL, dR, dsplit, rope_of(b.l - F, dR),
+                                          pfx, ulo, uhi, w);
             written += w;
             A.wlo[p] = ulo | (pend ? 0x80000000u : 0u);
             A.whi[p] = uhi;
@@ -951,7 +951,8 @@ __device__ void process_cell(const TreeCtx &cx, const CellArrays A, int j, int r
         r.last = F + n - 1;
         r.dL = dLc;
         r.dR = dRc;
-        r.pad[0] = r.pad[1] = 0;
+        r.dnext = n_next >= 2 ? 64 : dNN;
+        r.pad = 0;
         cx.croot[j] = r;
     }
     if (G == 32) {
@@ -1016,7 +1017,7 @@ __global__ void __launch_bounds__(TOP_THREADS) top_tree_kernel(const TreeCtx cx)
             const CellRoot r = cx.croot[j];
             Child me;
             me.wlo = r.wlo & 0x7FFFFFFFu, me.whi = r.whi, me.f = r.first, me.l = r.last, me.pend = (r.wlo >> 31) != 0;
-            walk_up(cx, me, r.dL, r.dR, j);
+            walk_up(cx, me, r.dL, r.dR, r.dnext);
         }
     }
     // ---- one thread per cell root ----
@@ -1027,7 +1028,7 @@ __global__ void __launch_bounds__(TOP_THREADS) top_tree_kernel(const TreeCtx cx)
     const CellRoot r = cx.croot[j];
     Child me;
     me.wlo = r.wlo & 0x7FFFFFFFu, me.whi = r.whi, me.f = r.first, me.l = r.last, me.pend = (r.wlo >> 31) != 0;
-    walk_up(cx, me, r.dL, r.dR, j);
+    walk_up(cx, me, r.dL, r.dR, r.dnext);
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -1079,8 +1080,8 @@ cudaError_t launch_build(const void *pos, const int32_t *type, const BuildParams
     fp.N = N, fp.T = p.T, fp.lvl = lvl, fp.warp_slots = traverse_warp_slots();
     for (int t = 0; t < QBVH_TMAX; ++t) fp.r_hint[t] = p.r_hint[t];
     const int tiles = (ncells + SCAN_TILE - 1) / SCAN_TILE;
-    cell_scan_kernel<<<tiles, SCAN_THREADS, 0, st>>>(b.cell_count, b.cell_start, b.cell_list, ncells, b.meta, fp);
-    cell_scatter_kernel<<<(N + 255) / 256, 256, 0, st>>>(b.key, b.rank, N, cell_shift, b.cell_start, b.ent);
+    cell_scan_kernel<<<tiles, SCAN_THREADS, 0, st>>>(b.cell_count, b.cell_start, b.cell_list, ncells, b.meta);
+    cell_scatter_kernel<<<(N + 255) / 256, 256, 0, st>>>(b.key, b.rank, N, cell_shift, b.cell_start, b.ent, b.cell_count, ncells, b.meta, fp);
     TreeCtx cx;
     cx.pos = pos, cx.f64 = p.f64 ? 1 : 0, cx.N = N, cx.K = p.K, cx.lvl = lvl, cx.build_tag = p.build_tag;
     cx.cell_start = b.cell_start, cx.cell_list = b.cell_list, cx.ent = b.ent;

@@ -62,6 +62,9 @@ __device__ inline float ord2f(uint32_t o) {
 // for the whole group (traverse_kernels.cu).
 constexpr int GROUP_MAX = 32;
 
+// ---- build tag of the meeting slots (top_tree_kernel): 18 bits; the slot area is cleared when it wraps ----
+constexpr uint32_t QBVH_TAG_MAX = (1u << 18) - 1;
+
 // ---- entry table: node of every cell of the 2^l-per-axis Morton grids, l = 2..5, per type ----
 constexpr int ENTRY_LMIN = 2, ENTRY_LMAX = 5;
 __host__ __device__ constexpr int entry_offset(int l) {   // cells of the levels below l: 64 + 512 + ...
@@ -93,7 +96,8 @@ struct __align__(16) CellRoot {
     int32_t first;     // sorted positions covered
     int32_t last;
     int32_t dL, dR;    // common prefix lengths with the neighbouring cells (-1 beyond the type segment)
-    int32_t pad[2];
+    int32_t dnext;     // delta(m, m+1) for m = last + 1: 64 if the next cell holds >= 2 particles, else its delta to the one after (-1: none)
+    int32_t pad;
 };
 
 // Z-ordered fp64 particle record of a double-precision build (qbvh_build_f64)

@@ -461,7 +461,8 @@ def test_rebuild_in_place_on_one_workspace():
     """What an MD code does: qbvh_build again and again on ONE workspace.  The meeting slots of the tree builder are
     not cleared between builds, stale ones are told apart by a per-build tag.  Same N, different
     positions / types / K each time, nodes, parents and lists compared with the oracle after every build, and the
-    24-bit tag driven through its wrap."""
+    18-bit tag driven through its wrap."""
+    TAG_MAX = (1 << 18) - 1
     import torch
     from paper_1901_08088_b200 import qbvh
     dev = torch.device("cuda:0")
@@ -481,7 +482,7 @@ def test_rebuild_in_place_on_one_workspace():
         qbvh.qbvh_set_option(qbvh.OPT_LEAF_COLLAPSE, K)
         if it == 3:
             nl._activate()
-            qbvh.qbvh_set_option(qbvh.OPT_DEBUG_BUILD_TAG, 0xFFFFFE)   # this build: 0xFFFFFE, next: 0xFFFFFF, then the wrap
+            qbvh.qbvh_set_option(qbvh.OPT_DEBUG_BUILD_TAG, TAG_MAX - 1)   # this build: max - 1, next: max, then the wrap
         nl.build(torch.from_numpy(pos).to(dev), torch.from_numpy(typ).to(dev), box)
         tags.append(qbvh.qbvh_get_option(qbvh.OPT_DEBUG_BUILD_TAG))
         w = W.Workload(f"rebuild{it}", pos, typ, box, r, 256)
@@ -495,7 +496,7 @@ def test_rebuild_in_place_on_one_workspace():
         M = nl.neighbors(r, retry=False)
         out = {"M": M, "max_neigh": nl.max_neigh, "nlist": nl.nlist.cpu().numpy()[:N], "n_neigh": nl.n_neigh.cpu().numpy()[:N]}
         compare_with_oracle(w, out, ON.neighbor_list(pos, typ, box, r))
-    assert tags == [1, 2, 3, 0xFFFFFE, 0xFFFFFF, 1, 2], tags      # no clearing between builds except at the wrap
+    assert tags == [1, 2, 3, TAG_MAX - 1, TAG_MAX, 1, 2], tags    # no clearing between builds except at the wrap
     qbvh.qbvh_set_option(qbvh.OPT_LEAF_COLLAPSE, 32)
 
 
