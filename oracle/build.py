@@ -13,7 +13,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 LIB = os.path.join(HERE, "liboracle.so")
-SRCS = [os.path.join(HERE, "neighbors.c"), os.path.join(HERE, "tree.c")]
+SRCS = [os.path.join(HERE, "neighbors.c"), os.path.join(HERE, "neighbors_f64.c"), os.path.join(HERE, "tree.c")]
 CFLAGS = ["-O2", "-fopenmp", "-ffp-contract=off", "-frounding-math", "-fno-fast-math",
           "-shared", "-fPIC", "-Wall", "-Wno-unknown-pragmas"]
 

@@ -31,6 +31,13 @@ def lib() -> C.CDLL:
         _lib.oracle_pair.restype = C.c_int
         _lib.oracle_pair.argtypes = [f32p, f32p, f32p, C.c_float, f32p, C.POINTER(C.c_double)]
         _lib.oracle_num_threads.restype = C.c_int
+        f64p = C.POINTER(C.c_double)
+        for name in ("oracle_brute_force_f64", "oracle_cell_list_f64"):
+            fn = getattr(_lib, name)
+            fn.restype = C.c_int64
+            fn.argtypes = [f64p, i32p, C.c_int64, f64p, f64p, C.c_int32, i32p, i64p, i32p]
+        _lib.oracle_pair_f64.restype = C.c_int
+        _lib.oracle_pair_f64.argtypes = [f64p, f64p, f64p, C.c_double, f64p]
     return _lib
 
 
@@ -99,3 +106,46 @@ def neighbor_list(pos, type, box, r_list, method: str = "auto", with_band: bool 
 def counts(pos, type, box, r_list, method: str = "auto") -> np.ndarray:
     row_ptr, _, _ = neighbor_list(pos, type, box, r_list, method=method, with_band=False)
     return np.diff(row_ptr).astype(np.int32)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# double-precision particle data (oracle/neighbors_f64.c)
+# ---------------------------------------------------------------------------------------------------------
+def pair_f64(pi, pj, box, r):
+    """O1-64 on one pair: returns (is_neighbor, d2_fp64)."""
+    pi = np.ascontiguousarray(pi, np.float64)
+    pj = np.ascontiguousarray(pj, np.float64)
+    box = np.ascontiguousarray(box, np.float64)
+    d2 = C.c_double()
+    ok = lib().oracle_pair_f64(_p(pi, C.c_double), _p(pj, C.c_double), _p(box, C.c_double), C.c_double(float(r)), C.byref(d2))
+    return bool(ok), float(d2.value)
+
+
+def neighbor_list_f64(pos, type, box, r_list, method: str = "auto", timing: dict | None = None):
+    """CSR neighbor list of fp64 positions by the definition in fp64.  Returns (row_ptr, nbr)."""
+    pos = np.ascontiguousarray(pos, np.float64)
+    N = pos.shape[0]
+    assert pos.shape == (N, 3)
+    type = None if type is None else np.ascontiguousarray(type, np.int32)
+    box = np.ascontiguousarray(box, np.float64)
+    r_list = np.ascontiguousarray(r_list, np.float64)
+    T = r_list.shape[0]
+    assert r_list.shape == (T, T)
+    if method == "auto":
+        method = "brute" if N <= 16384 else "cell"
+    fn = {"brute": lib().oracle_brute_force_f64, "cell": lib().oracle_cell_list_f64}[method]
+    t0 = time.perf_counter()
+    n_neigh = np.zeros(max(N, 1), np.int32)
+    args = [_p(pos, C.c_double), _p(type, C.c_int32), N, _p(box, C.c_double), _p(r_list, C.c_double), T]
+    total = fn(*args, _p(n_neigh, C.c_int32), None, None)
+    assert total >= 0
+    row_ptr = np.zeros(N + 1, np.int64)
+    np.cumsum(n_neigh[:N], out=row_ptr[1:])
+    nbr = np.empty(max(int(total), 1), np.int32)
+    total2 = fn(*args, _p(n_neigh, C.c_int32), _p(row_ptr, C.c_int64), _p(nbr, C.c_int32))
+    assert total2 == total
+    if timing is not None:
+        timing["seconds"] = time.perf_counter() - t0
+        timing["threads"] = num_threads()
+        timing["method"] = method
+    return row_ptr, nbr[:total]
