@@ -116,6 +116,20 @@ int qbvh_build(const float *pos, const int32_t *type, int64_t N, const float *bo
  * n_neigh[i] > max_neigh hold max_neigh true neighbors; re-allocate with capacity >= M and call again. */
 int qbvh_neighbors(const float *r_list_ij, int32_t *nlist, int32_t *n_neigh, int32_t max_neigh);
 
+/* ---- double-precision particle data -----------------------------
+ * The tree stays what it is — fp32 frames, 10-bit quantized boxes, 16-byte nodes, built from the positions rounded to
+ * fp32 — "the sphere radius is padded to account for uncertainty from loss of precision when the particle data is
+ * double precision", and the exact leaf test is the fp64 minimum-image predicate:
+ *   D_d = p_j[d] - p_i[d], wrapped once by L_d;  d2 = fma(Dz,Dz, fma(Dy,Dy, Dx Dx));  neighbor <=> d2 <= r_ij^2  (fp64)
+ * A pair is first judged in fp32 on the rounded positions with the cutoff widened / narrowed by 8 ulp32(M)
+ * (M = max_d(|lo_d| + 2 L_d)); only pairs inside that band (about one in two thousand) are decided in fp64.
+ *   pos   DEVICE  N x 3 fp64 row-major, wrapped into [lo_d, lo_d + L_d).   box  HOST 6 doubles {lo_xyz, L_xyz}.
+ *   r_list_ij HOST T x T fp64.   nlist / n_neigh / max_neigh / return value: as for qbvh_neighbors.
+ * qbvh_neighbors_f64 requires the last build to be qbvh_build_f64 (and qbvh_neighbors a qbvh_build): otherwise
+ * QBVH_ERR_INVALID_ARG.  QBVH_OPT_VARIANT must be 1. */
+int qbvh_build_f64(const double *pos, const int32_t *type, int64_t N, const double *box);
+int qbvh_neighbors_f64(const double *r_list_ij, int32_t *nlist, int32_t *n_neigh, int32_t max_neigh);
+
 /* The paper's own operating mode ("the object in the leaf node is processed as a neighbor" without a
  * distance check, positions are not loaded; the benchmarks only count): Algorithm 1 as printed, one
  * thread per particle in Z-order, accepting every particle whose (collapsed) leaf box overlaps the padded search

@@ -25,6 +25,7 @@ struct Context {
     bool built = false;
     int64_t N = 0;
     float box[6] = {0, 0, 0, 0, 0, 0};
+    double box64[6] = {0, 0, 0, 0, 0, 0};   // the box of a double-precision build
     float scale[3] = {0, 0, 0};
     BuildBuffers buf{};
     uint32_t build_tag = 0;      // tag of the last build's meeting slots; 0: the slot area has to be cleared first
@@ -103,41 +104,81 @@ float padded_radius(float r, const float *box) {
     return up_to_f32(sum);
 }
 
+// largest fp32 value <= x
+float down_to_f32(double x) {
+    float f = (float)x;
+    if ((double)f > x) f = std::nextafterf(f, -INFINITY);
+    return f;
+}
+
+// ulp32(M), M = max_d(|lo_d| + 2 L_d): the spacing of fp32 numbers at the largest coordinate the traversal can form
+double box_ulp32(const float *box) {
+    double M = 0.0;
+    for (int d = 0; d < 3; ++d) M = std::fmax(M, std::fabs((double)box[d]) + 2.0 * (double)box[3 + d]);
+    return std::scalbn(1.0, std::ilogb(M) - 23);
+}
+
 // a * b rounded up (the product of two fp32 values is exact in fp64)
 float mul_ru(float a, float b) { return up_to_f32((double)a * (double)b); }
 
-// r_list -> the traversal's parameter block (exact r^2, padded pruning radius, Morton binning of the build)
-int make_params(const float *r_list, TraverseParams &P) {
+// r_list -> the traversal's parameter block (exact r^2, padded pruning radius, Morton binning of the build).
+// f64 (qbvh_neighbors_f64): the fp32 kernel runs on the positions rounded to fp32 with the cutoff
+// widened by B = 8 ulp32(M) — |d_fp32 - d_fp64| < 5 ulp32(M): two position roundings, the rounding of L and two
+// subtractions per axis (2.5 ulp, times sqrt 3), plus the rounding of the squared sum — so nothing it rejects can be
+// an fp64 neighbor; what it finds within r - B certainly is one; the pairs in between go through the fp64 predicate.
+template <typename RT>
+int make_params(const RT *r_list, bool f64, TraverseParams &P) {
     for (int d = 0; d < 3; ++d) {
         P.L[d] = g.box[3 + d];
         P.box_lo[d] = g.box[d];
         P.scale[d] = g.scale[d];
+        P.L64[d] = g.box64[3 + d];
     }
-    for (int k = 0; k < QBVH_TMAX * QBVH_TMAX; ++k) P.r2[k] = P.R2[k] = P.Rp[k] = -1.0f;
+    const double B = f64 ? 8.0 * box_ulp32(g.box) : 0.0;
+    for (int k = 0; k < QBVH_TMAX * QBVH_TMAX; ++k) {
+        P.r2[k] = P.R2[k] = P.Rp[k] = P.r2lo[k] = -1.0f;
+        P.r2_64[k] = -1.0;
+    }
     for (int a = 0; a < g.T; ++a)
         for (int b = 0; b < g.T; ++b) {
-            const float r = r_list[a * g.T + b];
-            if (!(r > 0.0f)) continue;
+            const RT r = r_list[a * g.T + b];
+            if (!(r > 0)) continue;
             if (!std::isfinite(r)) return QBVH_ERR_INVALID_ARG;
-            const float rp = padded_radius(r, g.box);
+            const int k = a * QBVH_TMAX + b;
+            float r_cut;                       // cutoff of the fp32 predicate
+            if (f64) {
+                r_cut = up_to_f32((double)r + B);
+                const double rlo = (double)r - B;
+                P.r2[k] = up_to_f32((double)r_cut * (double)r_cut);
+                P.r2lo[k] = rlo > 0.0 ? down_to_f32(rlo * rlo * (1.0 - 0x1p-50)) : -1.0f;
+                volatile double r2 = (double)r * (double)r;      // fp64 RN
+                P.r2_64[k] = r2;
+            } else {
+                r_cut = (float)r;
+                volatile float r2 = r_cut * r_cut;               // fp32 RN
+                P.r2[k] = r2;
+                P.r2lo[k] = r2;
+            }
+            const float rp = padded_radius(r_cut, g.box);
             for (int d = 0; d < 3; ++d)
                 if (!(rp < 0.5f * g.box[3 + d])) return QBVH_ERR_CUTOFF_TOO_LARGE;
-            volatile float r2 = r * r;
-            P.r2[a * QBVH_TMAX + b] = r2;
-            P.R2[a * QBVH_TMAX + b] = mul_ru(rp, rp);
-            P.Rp[a * QBVH_TMAX + b] = rp;
+            P.R2[k] = mul_ru(rp, rp);
+            P.Rp[k] = rp;
         }
     P.N = (int32_t)g.N;
     P.K = g.K_built;
     return QBVH_OK;
 }
 
-int neighbors_impl(const float *r_list, int32_t *nlist, int32_t *n_neigh, int32_t max_neigh) {
+template <typename RT>
+int neighbors_impl(const RT *r_list, bool f64, int32_t *nlist, int32_t *n_neigh, int32_t max_neigh) {
     if (!g.built) return QBVH_ERR_NOT_BUILT;
     if (!r_list || max_neigh < 0) return QBVH_ERR_INVALID_ARG;
+    if (f64 != g.f64_built) return QBVH_ERR_INVALID_ARG;          // qbvh_build_f64 pairs with qbvh_neighbors_f64
+    if (f64 && g.variant != 1) return QBVH_ERR_INVALID_ARG;       // Algorithm 1 as printed (variant 0) is the fp32 path
     if (g.N > 0 && (!n_neigh || (!nlist && max_neigh > 0))) return QBVH_ERR_INVALID_ARG;
     TraverseParams P{};
-    const int prc = make_params(r_list, P);
+    const int prc = make_params(r_list, f64, P);
     if (prc != QBVH_OK) return prc;
     P.N = (int32_t)g.N;
     P.max_neigh = max_neigh;
@@ -150,7 +191,7 @@ int neighbors_impl(const float *r_list, int32_t *nlist, int32_t *n_neigh, int32_
         e = cudaMemsetAsync(g.buf.meta->stats, 0, sizeof(g.buf.meta->stats), g.stream);
         if (e != cudaSuccess) return cuda_fail(e, "memset stats");
     }
-    e = launch_traverse(P, g.buf, nlist, n_neigh, g.stats, g.variant, g.stream);
+    e = launch_traverse(P, g.buf, nlist, n_neigh, g.stats, g.variant, f64, g.stream);
     if (e != cudaSuccess) return cuda_fail(e, "traverse launch");
     e = cudaMemcpyAsync(g.pinned, &g.buf.meta->max_count, 2 * sizeof(int32_t), cudaMemcpyDeviceToHost, g.stream);
     if (e != cudaSuccess) return cuda_fail(e, "copy max_count");
@@ -315,7 +356,24 @@ int qbvh_set_collapse_hint(const float *r_hint, int32_t n) {
 }
 
 int qbvh_neighbors(const float *r_list_ij, int32_t *nlist, int32_t *n_neigh, int32_t max_neigh) {
-    int rc = neighbors_impl(r_list_ij, nlist, n_neigh, max_neigh);
+    int rc = neighbors_impl(r_list_ij, false, nlist, n_neigh, max_neigh);
+    if (rc != QBVH_OK) return rc;
+    return finish_neighbors();
+}
+
+int qbvh_build_f64(const double *pos, const int32_t *type, int64_t N, const double *box) {
+    if (!box) return QBVH_ERR_INVALID_ARG;
+    float box32[6];
+    for (int d = 0; d < 6; ++d) {
+        if (!std::isfinite(box[d])) return QBVH_ERR_INVALID_ARG;
+        box32[d] = (float)box[d];                     // the tree lives in fp32: Morton bins and frames from rounded values
+    }
+    std::memcpy(g.box64, box, sizeof(g.box64));
+    return build_impl(pos, true, type, N, box32);
+}
+
+int qbvh_neighbors_f64(const double *r_list_ij, int32_t *nlist, int32_t *n_neigh, int32_t max_neigh) {
+    int rc = neighbors_impl(r_list_ij, true, nlist, n_neigh, max_neigh);
     if (rc != QBVH_OK) return rc;
     return finish_neighbors();
 }
@@ -324,7 +382,8 @@ int qbvh_count_overlaps(const float *r_list_ij, int32_t *n_overlap) {
     if (!g.built) return QBVH_ERR_NOT_BUILT;
     if (!r_list_ij || (g.N > 0 && !n_overlap)) return QBVH_ERR_INVALID_ARG;
     TraverseParams P{};
-    const int prc = make_params(r_list_ij, P);
+    if (g.f64_built) return QBVH_ERR_INVALID_ARG;
+    const int prc = make_params(r_list_ij, false, P);
     if (prc != QBVH_OK) return prc;
     P.max_neigh = 0;
     cudaError_t e = cudaMemsetAsync(&g.buf.meta->group_cursor, 0, 2 * sizeof(int32_t), g.stream);
@@ -378,7 +437,7 @@ int qbvh_neighbors_host(const float *r_list_ij, int32_t *nlist, int32_t *n_neigh
     int32_t *dcnt = reinterpret_cast<int32_t *>(s + align256(12 * n1) + align256(4 * n1) +
                                                 align256(4 * n1 * (int64_t)(max_neigh > 0 ? max_neigh : 1)));
     if (N > 0 && (!n_neigh || (!nlist && max_neigh > 0))) return QBVH_ERR_INVALID_ARG;
-    int rc = neighbors_impl(r_list_ij, dlist, dcnt, max_neigh);
+    int rc = neighbors_impl(r_list_ij, false, dlist, dcnt, max_neigh);
     if (rc != QBVH_OK) return rc;
     if (N > 0) {
         cudaError_t e = cudaMemcpyAsync(n_neigh, dcnt, 4 * N, cudaMemcpyDeviceToHost, g.stream);

@@ -87,6 +87,12 @@ struct TraverseParams {
     int32_t N;
     int32_t max_neigh;
     int32_t K;                         // leaf-collapse cap used by the build
+    // double-precision particle data (qbvh_neighbors_f64): r2 above is then (r + B)^2 rounded up — whatever fails it
+    // in fp32 on the rounded positions cannot be a neighbor in fp64 —, r2lo = (r - B)^2 rounded down — whatever passes
+    // it certainly is one —, and only the pairs in between are decided by the fp64 predicate.
+    float r2lo[QBVH_TMAX * QBVH_TMAX];
+    double r2_64[QBVH_TMAX * QBVH_TMAX];
+    double L64[3];
 };
 
 // record a cell's root hands to the top-level walk (cell_tree_kernel -> top_tree_kernel)
@@ -137,7 +143,7 @@ struct BuildParams {
 int pick_cell_level(int64_t N, int T);
 cudaError_t launch_build(const void *pos, const int32_t *type, const BuildParams &p, const BuildBuffers &b, cudaStream_t st);
 cudaError_t launch_traverse(const TraverseParams &p, const BuildBuffers &b, int32_t *nlist, int32_t *n_neigh,
-                            bool stats, int variant, cudaStream_t st);
+                            bool stats, int variant, bool f64, cudaStream_t st);
 cudaError_t launch_count_overlaps(const TraverseParams &p, const BuildBuffers &b, int32_t *n_overlap, cudaStream_t st);
 int traverse_warp_slots();      // warps the production traversal keeps resident on this device
 static_assert(offsetof(TreeMeta, group_count) % 128 == 0, "the atomic counters start a 128-byte line");

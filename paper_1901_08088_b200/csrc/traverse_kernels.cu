@@ -301,9 +301,26 @@ __device__ __forceinline__ void ring_put(uint32_t ring_s, uint32_t &po, int32_t 
 // canonical predicate
 //   D = (p_j - p_i) [- s L];  d2 = fma(Dz, Dz, fma(Dy, Dy, Dx*Dx));  d2 <= r^2
 // evaluated for two candidates per instruction.  SELF: the tile holds the members of the group itself.
-template <bool SHIFTED, bool SELF, int NC>
+// What the fp64 path adds (qbvh_neighbors_f64): the pair is first judged in fp32 on the positions
+// rounded to fp32; only if its squared distance falls between r2lo and r2 (about one pair in two thousand) the
+// canonical fp64 predicate decides, on the Z-ordered double positions.
+struct F64Ctx {
+    const Pos64 *sp64;     // Z-ordered fp64 positions
+    const int32_t *tp;     // sorted position of every candidate of the tile ring
+    int ksort_i;           // sorted position of this lane's particle
+    double s0, s1, s2;     // image shift (exactly 0 or +-L)
+    double r2_64;
+    float r2lo;
+};
+__device__ __noinline__ bool exact_pair_f64(const Pos64 *__restrict__ sp64, int ki, int kj, double s0, double s1, double s2, double r2) {
+    const Pos64 a = sp64[ki], b = sp64[kj];
+    const double dx = __dsub_rn(__dsub_rn(b.x, a.x), s0), dy = __dsub_rn(__dsub_rn(b.y, a.y), s1), dz = __dsub_rn(__dsub_rn(b.z, a.z), s2);
+    return __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx))) <= r2;
+}
+
+template <bool SHIFTED, bool SELF, int NC, bool F64>
 __device__ __forceinline__ void check_tile(const GwShared &sm, int base, u64 nmx, u64 nmy, u64 nmz, u64 ns0, u64 ns1,
-                                        u64 ns2, float r2, int orig_i, uint32_t ring_s, uint32_t &po) {
+                                        u64 ns2, float r2, int orig_i, uint32_t ring_s, uint32_t &po, const F64Ctx &fx) {
 #pragma unroll
     for (int j = 0; j < NC / 4; ++j) {
         const float4 X = *reinterpret_cast<const float4 *>(&sm.tx[base + 4 * j]);
@@ -323,10 +340,14 @@ __device__ __forceinline__ void check_tile(const GwShared &sm, int base, u64 nmx
         float d0, d1, d2, d3;
         upk2(dd0, d0, d1);
         upk2(dd1, d2, d3);
-        if (d0 <= r2 && (!SELF || I.x != orig_i)) { ring_put(ring_s, po, I.x); }
-        if (d1 <= r2 && (!SELF || I.y != orig_i)) { ring_put(ring_s, po, I.y); }
-        if (d2 <= r2 && (!SELF || I.z != orig_i)) { ring_put(ring_s, po, I.z); }
-        if (d3 <= r2 && (!SELF || I.w != orig_i)) { ring_put(ring_s, po, I.w); }
+        auto sure = [&](float d, int c) -> bool {
+            if (!F64) return true;
+            return d <= fx.r2lo || exact_pair_f64(fx.sp64, fx.ksort_i, fx.tp[base + 4 * j + c], fx.s0, fx.s1, fx.s2, fx.r2_64);
+        };
+        if (d0 <= r2 && (!SELF || I.x != orig_i) && sure(d0, 0)) { ring_put(ring_s, po, I.x); }
+        if (d1 <= r2 && (!SELF || I.y != orig_i) && sure(d1, 1)) { ring_put(ring_s, po, I.y); }
+        if (d2 <= r2 && (!SELF || I.z != orig_i) && sure(d2, 2)) { ring_put(ring_s, po, I.z); }
+        if (d3 <= r2 && (!SELF || I.w != orig_i) && sure(d3, 3)) { ring_put(ring_s, po, I.w); }
     }
 }
 
@@ -385,15 +406,17 @@ __device__ __forceinline__ bool point_in_reach(const float4 p, const float blo[3
 
 // WS: collapsed leaves are gathered in fixed slots of WS lanes each (WS >= K, 32 / WS leaves per batch, two batches
 // per step so that two 16-byte position loads per lane are in flight).
-template <bool STATS, int WS>
+template <bool STATS, int WS, bool F64>
 __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseParams P, const int4 *__restrict__ nodes,
                                                                         const float4 *__restrict__ sorted_pos,
+                                                                        const Pos64 *__restrict__ sorted_pos64,
                                                                         const uint2 *__restrict__ groups,
                                                                         const int32_t *__restrict__ entry,
                                                                         TreeMeta *__restrict__ meta,
                                                                         int32_t *__restrict__ nlist,
                                                                         int32_t *__restrict__ n_neigh) {
     __shared__ GwShared s_all[GW_WARPS];
+    __shared__ int32_t s_tp[GW_WARPS][F64 ? GW_TILE : 1];   // fp64 only: sorted position of every candidate in the tile ring
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const uint32_t FULL = 0xFFFFFFFFu;
     const uint32_t lt_mask = (1u << lane) - 1u;
@@ -483,6 +506,11 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
             const float fdl[3] = {fr[6], fr[7], fr[8]};
             const int seg_end = meta->seg[tb + 1];
             const int32_t *const etab = entry + tb * ENTRY_CELLS;
+            F64Ctx fx;
+            if (F64) {
+                fx.sp64 = sorted_pos64, fx.tp = s_tp[warp], fx.ksort_i = gfirst + (live ? lane : 0);
+                fx.r2_64 = P.r2_64[ta * QBVH_TMAX + tb], fx.r2lo = P.r2lo[ta * QBVH_TMAX + tb];
+            }
             // ---- Alg. 1 line 4: lane j tests image j of the group box against the root node; the vote is the bitset ----
             uint32_t bset;
             {
@@ -506,6 +534,7 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
                 const float blo[3] = {__fadd_rn(glo[0], s0), __fadd_rn(glo[1], s1), __fadd_rn(glo[2], s2)};
                 const float bhi[3] = {__fadd_rn(ghi[0], s0), __fadd_rn(ghi[1], s1), __fadd_rn(ghi[2], s2)};
                 const u64 ns0 = pk2(-s0, -s0), ns1 = pk2(-s1, -s1), ns2 = pk2(-s2, -s2);
+                if (F64) fx.s0 = (double)(img % 3 - 1) * P.L64[0], fx.s1 = (double)((img / 3) % 3 - 1) * P.L64[1], fx.s2 = (double)(img / 9 - 1) * P.L64[2];
                 // the group's own particles are found by the walk only here: in its own tree, unshifted.  They are
                 // checked first, as one tile (self excluded by index), and their leaves are skipped below.
                 // (A sparse type has groups smaller than the collapsed leaves, meta->gmax < K: then a leaf may hold the
@@ -517,10 +546,11 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
                     sm.ty[lane] = me.y;
                     sm.tz[lane] = me.z;
                     sm.ti[lane] = orig_i;
+                    if (F64) s_tp[warp][lane] = gfirst + lane;
                     __syncwarp();
 #pragma unroll 1
                     for (int h = 0; h < 32 / CHUNK; ++h) {
-                        check_tile<false, true, CHUNK>(sm, CHUNK * h, nmx, nmy, nmz, ns0, ns1, ns2, r2, orig_i, ring_s, po);
+                        check_tile<false, true, CHUNK, F64>(sm, CHUNK * h, nmx, nmy, nmz, ns0, ns1, ns2, r2, orig_i, ring_s, po, fx);
                         if (__any_sync(FULL, (int)((po - rot) >> 2) - flushed >= GW_RING - CHUNK)) flush_blocks();
                     }
                     if (STATS) st_checks += (unsigned long long)gcnt * (unsigned)gcnt;
@@ -577,11 +607,11 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
 #pragma unroll 1
                         for (int h = 0; h < 32 / CHUNK; ++h) {
                             if (shifted)
-                                check_tile<true, false, CHUNK>(sm, thead + CHUNK * h, nmx, nmy, nmz, ns0, ns1, ns2, r2, orig_i, ring_s, po);
+                                check_tile<true, false, CHUNK, F64>(sm, thead + CHUNK * h, nmx, nmy, nmz, ns0, ns1, ns2, r2, orig_i, ring_s, po, fx);
                             else if (self_all)
-                                check_tile<false, true, CHUNK>(sm, thead + CHUNK * h, nmx, nmy, nmz, ns0, ns1, ns2, r2, orig_i, ring_s, po);
+                                check_tile<false, true, CHUNK, F64>(sm, thead + CHUNK * h, nmx, nmy, nmz, ns0, ns1, ns2, r2, orig_i, ring_s, po, fx);
                             else
-                                check_tile<false, false, CHUNK>(sm, thead + CHUNK * h, nmx, nmy, nmz, ns0, ns1, ns2, r2, orig_i, ring_s, po);
+                                check_tile<false, false, CHUNK, F64>(sm, thead + CHUNK * h, nmx, nmy, nmz, ns0, ns1, ns2, r2, orig_i, ring_s, po, fx);
                             // flush as soon as another chunk could overrun a ring
                             if (__any_sync(FULL, (int)((po - rot) >> 2) - flushed >= GW_RING - CHUNK)) flush_blocks();
                         }
@@ -675,6 +705,7 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
                                 sm.ty[slot] = pc[u].y;
                                 sm.tz[slot] = pc[u].z;
                                 sm.ti[slot] = __float_as_int(pc[u].w);
+                                if (F64) s_tp[warp][slot] = (int32_t)lf[u].x + sub;
                             }
                             nkept += __popc(kb);
                         }
@@ -735,30 +766,35 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
 }
 
 // persistent grid of the group kernel: as many blocks as fit on the device at once
-template <bool STATS, int WS>
+template <bool STATS, int WS, bool F64>
 static int group_grid_blocks() {
     static int c = 0;
     if (c == 0) {
         int dev = 0, sms = 148, per_sm = 1;
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, traverse_group_kernel<STATS, WS>, GW_WARPS * 32, 0);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, traverse_group_kernel<STATS, WS, F64>, GW_WARPS * 32, 0);
         c = sms * (per_sm > 0 ? per_sm : 1);
     }
     return c;
 }
 
-template <bool STATS, int WS>
+template <bool STATS, int WS, bool F64>
 static void launch_group(const TraverseParams &p, const BuildBuffers &b, int32_t *nlist, int32_t *n_neigh, cudaStream_t st) {
-    const int gb = min(group_grid_blocks<STATS, WS>(), (p.N + GW_WARPS - 1) / GW_WARPS);
-    traverse_group_kernel<STATS, WS><<<gb, GW_WARPS * 32, 0, st>>>(p, b.nodes, b.sorted_pos, b.groups, b.entry, b.meta, nlist, n_neigh);
+    const int gb = min(group_grid_blocks<STATS, WS, F64>(), (p.N + GW_WARPS - 1) / GW_WARPS);
+    traverse_group_kernel<STATS, WS, F64><<<gb, GW_WARPS * 32, 0, st>>>(p, b.nodes, b.sorted_pos, b.sorted_pos64, b.groups, b.entry, b.meta, nlist, n_neigh);
+}
+template <bool STATS, int WS>
+static void launch_group_p(const TraverseParams &p, const BuildBuffers &b, int32_t *nlist, int32_t *n_neigh, bool f64, cudaStream_t st) {
+    if (f64) launch_group<STATS, WS, true>(p, b, nlist, n_neigh, st);
+    else launch_group<STATS, WS, false>(p, b, nlist, n_neigh, st);
 }
 
 // warps the production traversal keeps resident (the build sizes query groups of small systems by it)
-int traverse_warp_slots() { return group_grid_blocks<false, 32>() * GW_WARPS; }
+int traverse_warp_slots() { return group_grid_blocks<false, 32, false>() * GW_WARPS; }
 
 cudaError_t launch_traverse(const TraverseParams &p, const BuildBuffers &b, int32_t *nlist, int32_t *n_neigh,
-                            bool stats, int variant, cudaStream_t st) {
+                            bool stats, int variant, bool f64, cudaStream_t st) {
     if (p.N == 0) return cudaSuccess;
     const int threads = 128;
     const int blocks = (p.N + threads - 1) / threads;
@@ -776,13 +812,13 @@ cudaError_t launch_traverse(const TraverseParams &p, const BuildBuffers &b, int3
         traverse_kernel<true><<<blocks, threads, 0, st>>>(p, b.nodes, b.sorted_pos, b.meta, nlist, n_neigh);
         cudaError_t e = cudaMemsetAsync(&b.meta->group_cursor, 0, 2 * sizeof(int32_t), st);
         if (e != cudaSuccess) return e;
-        if (ws == 32) launch_group<true, 32>(p, b, nlist, n_neigh, st);
-        else if (ws == 16) launch_group<true, 16>(p, b, nlist, n_neigh, st);
-        else launch_group<true, 8>(p, b, nlist, n_neigh, st);
+        if (ws == 32) launch_group_p<true, 32>(p, b, nlist, n_neigh, f64, st);
+        else if (ws == 16) launch_group_p<true, 16>(p, b, nlist, n_neigh, f64, st);
+        else launch_group_p<true, 8>(p, b, nlist, n_neigh, f64, st);
     } else {
-        if (ws == 32) launch_group<false, 32>(p, b, nlist, n_neigh, st);
-        else if (ws == 16) launch_group<false, 16>(p, b, nlist, n_neigh, st);
-        else launch_group<false, 8>(p, b, nlist, n_neigh, st);
+        if (ws == 32) launch_group_p<false, 32>(p, b, nlist, n_neigh, f64, st);
+        else if (ws == 16) launch_group_p<false, 16>(p, b, nlist, n_neigh, f64, st);
+        else launch_group_p<false, 8>(p, b, nlist, n_neigh, f64, st);
     }
     return cudaGetLastError();
 }

@@ -24,7 +24,7 @@ EXPORT_KEYS_SORTED, EXPORT_PERM, EXPORT_NODES, EXPORT_PARENT, EXPORT_FRAMES, EXP
 SYMBOLS = ("qbvh_set_stream", "qbvh_set_num_types", "qbvh_workspace_bytes", "qbvh_set_workspace",
            "qbvh_set_option", "qbvh_get_option", "qbvh_build", "qbvh_neighbors", "qbvh_count_overlaps", "qbvh_staging_bytes",
            "qbvh_set_staging", "qbvh_build_host", "qbvh_neighbors_host", "qbvh_get_stats", "qbvh_debug_export",
-           "qbvh_error_string", "qbvh_padded_radius", "qbvh_set_collapse_hint")
+           "qbvh_error_string", "qbvh_padded_radius", "qbvh_set_collapse_hint", "qbvh_build_f64", "qbvh_neighbors_f64")
 
 
 class QbvhStats(C.Structure):
@@ -56,6 +56,8 @@ _lib.qbvh_set_collapse_hint.argtypes = [_vp, _i32]
 _lib.qbvh_build.argtypes = [_vp, _vp, _i64, _vp]
 _lib.qbvh_neighbors.argtypes = [_vp, _vp, _vp, _i32]
 _lib.qbvh_count_overlaps.argtypes = [_vp, _vp]
+_lib.qbvh_build_f64.argtypes = [_vp, _vp, _i64, _vp]
+_lib.qbvh_neighbors_f64.argtypes = [_vp, _vp, _vp, _i32]
 _lib.qbvh_staging_bytes.argtypes = [_i64, _i32]
 _lib.qbvh_staging_bytes.restype = _i64
 _lib.qbvh_set_staging.argtypes = [_vp, _i64]
@@ -162,6 +164,21 @@ def qbvh_neighbors(r_list_ij, nlist, n_neigh, max_neigh: int) -> int:
     return _check(_lib.qbvh_neighbors(r.ctypes.data, _ptr(nlist), _ptr(n_neigh), max_neigh), "qbvh_neighbors")
 
 
+def qbvh_build_f64(pos, type, N: int, box) -> int:
+    """pos: DEVICE float64 N x 3; type: DEVICE int32 N or None; box: 6 host doubles."""
+    box = np.ascontiguousarray(box, dtype=np.float64).reshape(-1)
+    assert box.size == 6
+    return _check(_lib.qbvh_build_f64(_ptr(pos), _ptr(type), N, box.ctypes.data), "qbvh_build_f64")
+
+
+def qbvh_neighbors_f64(r_list_ij, nlist, n_neigh, max_neigh: int) -> int:
+    """r_list_ij: host T x T float64; otherwise as qbvh_neighbors."""
+    r = np.ascontiguousarray(r_list_ij, dtype=np.float64)
+    if r.size != _num_types * _num_types:
+        raise ValueError(f"r_list_ij holds {r.size} values; qbvh_set_num_types({_num_types}) needs {_num_types}x{_num_types}")
+    return _check(_lib.qbvh_neighbors_f64(r.ctypes.data, _ptr(nlist), _ptr(n_neigh), max_neigh), "qbvh_neighbors_f64")
+
+
 def qbvh_count_overlaps(r_list_ij, n_overlap) -> int:
     """The paper's accept-on-leaf-overlap count.  n_overlap: DEVICE int32 tensor of N."""
     r = _r_list(r_list_ij)
@@ -263,16 +280,19 @@ class NeighborList:
             pass
 
     def build(self, pos, type, box):
-        assert pos.is_cuda and pos.dtype == self.torch.float32 and tuple(pos.shape) == (self.N, 3)
+        """pos: CUDA float32 (qbvh_build) or float64 (qbvh_build_f64) N x 3."""
+        assert pos.is_cuda and pos.dtype in (self.torch.float32, self.torch.float64) and tuple(pos.shape) == (self.N, 3)
         assert type is None or (type.is_cuda and type.dtype == self.torch.int32)
         self._activate()
-        return qbvh_build(pos, type, self.N, box)
+        self.f64 = pos.dtype == self.torch.float64
+        return (qbvh_build_f64 if self.f64 else qbvh_build)(pos, type, self.N, box)
 
     def neighbors(self, r_list, retry: bool = True) -> int:
-        M = qbvh_neighbors(r_list, self.nlist, self.n_neigh, self.max_neigh)
+        call = qbvh_neighbors_f64 if getattr(self, "f64", False) else qbvh_neighbors
+        M = call(r_list, self.nlist, self.n_neigh, self.max_neigh)
         while retry and M > self.max_neigh:
             self.retries += 1
             self.max_neigh = int((M + 7) // 8 * 8)
             self.nlist = self.torch.empty((max(self.N, 1), self.max_neigh), dtype=self.torch.int32, device=self.device)
-            M = qbvh_neighbors(r_list, self.nlist, self.n_neigh, self.max_neigh)
+            M = call(r_list, self.nlist, self.n_neigh, self.max_neigh)
         return M

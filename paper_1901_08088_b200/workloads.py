@@ -95,6 +95,21 @@ def shifted(w: "Workload", lo) -> "Workload":
                     w.max_neigh, dict(w.meta))
 
 
+def as_f64(w: "Workload", seed: int = 0) -> tuple[np.ndarray, np.ndarray, np.ndarray]:
+    """Double-precision stand-in for a workload: every coordinate moved inside its own fp32 rounding interval by a
+    seeded uniform fraction of the spacing (so it is no longer an fp32 number but still rounds to the fp32 input), kept
+    inside the box.  Returns (pos64, box64, r_list64)."""
+    rng = np.random.default_rng([9064, seed])
+    p32 = w.pos
+    sp = np.spacing(np.abs(p32)).astype(np.float64)
+    pos = p32.astype(np.float64) + (rng.random(p32.shape) - 0.5) * 0.9 * sp
+    box = w.box.astype(np.float64)
+    pos = np.maximum(pos, box[:3])
+    pos = np.minimum(pos, np.nextafter(box[:3] + box[3:], -np.inf))
+    r = w.r_list.astype(np.float64) * (1.0 + 1e-9)      # a cutoff that is not an fp32 number either
+    return np.ascontiguousarray(pos), box, r
+
+
 def _rng(config_id: int, seed: int) -> np.random.Generator:
     return np.random.default_rng([config_id, seed])
 

@@ -518,3 +518,86 @@ def test_collapse_heuristic_build_and_lists(cid, K):
     assert emitted.sum() >= plain.sum()
     if cid == 3 and K == 32:
         assert emitted.sum() > plain.sum()
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# double-precision particle data (fp32 tree, padded fp32 search, fp64 leaf predicate)
+# ---------------------------------------------------------------------------------------------------------------
+def gpu_run_f64(pos64, typ, box64, r64, T, max_neigh, K=32):
+    import torch
+    from paper_1901_08088_b200 import qbvh
+    dev = torch.device("cuda:0")
+    N = len(pos64)
+    qbvh.qbvh_set_option(qbvh.OPT_LEAF_COLLAPSE, K)
+    qbvh.qbvh_set_option(qbvh.OPT_STATS, 0)
+    qbvh.qbvh_set_collapse_hint(None)
+    nl = qbvh.NeighborList(N, T=T, max_neigh=max_neigh, device=dev)
+    nl.build(torch.from_numpy(pos64).to(dev), None if typ is None else torch.from_numpy(typ).to(dev), box64)
+    nl.n_neigh.fill_(-7)
+    nl.nlist.fill_(-1)
+    M = nl.neighbors(r64, retry=False)
+    torch.cuda.synchronize()
+    out = {"M": M, "max_neigh": nl.max_neigh, "nlist": nl.nlist.cpu().numpy()[:N], "n_neigh": nl.n_neigh.cpu().numpy()[:N]}
+    out["keys_sorted"] = qbvh.qbvh_debug_export(qbvh.EXPORT_KEYS_SORTED, N)
+    out["nodes"] = qbvh.qbvh_debug_export(qbvh.EXPORT_NODES, N)
+    out["perm"] = qbvh.qbvh_debug_export(qbvh.EXPORT_PERM, N)
+    return out
+
+
+@pytest.mark.parametrize("K", [1, 32])
+@pytest.mark.parametrize("cid", [1, 2, 3, 4, 5])
+def test_f64_particles_parity_small(cid, K):
+    """qbvh_build_f64 / qbvh_neighbors_f64 against the fp64 oracle: identical sets, zero mismatches (both sides evaluate
+    the same fp64 predicate; the fp32 stage only prunes).  The tree must be the fp32 tree of the rounded positions."""
+    w = W.make_config(cid, small=True)
+    pos64, box64, r64 = W.as_f64(w)
+    out = gpu_run_f64(pos64, w.type, box64, r64, w.T, w.max_neigh, K=K)
+    w64 = W.Workload(w.name + "_f64", w.pos, w.type, w.box, w.r_list, w.max_neigh)
+    rp, nb = ON.neighbor_list_f64(pos64, w.type, box64, r64)
+    compare_with_oracle(w64, out, (rp, nb, np.zeros(len(nb), np.uint8)))
+    t = OT.build(pos64.astype(np.float32), w.type, box64.astype(np.float32), T=w.T)     # the fp32 tree of the rounded positions
+    exp, emitted = expected_nodes(t, K)
+    assert np.array_equal(out["keys_sorted"], t.key_sorted) and np.array_equal(out["perm"].astype(np.int64), t.perm)
+    assert np.array_equal(out["nodes"][emitted], exp[emitted])
+
+
+def test_f64_resolves_what_fp32_cannot():
+    """Pairs placed r (1 -+ 1e-10) apart at coordinates near 1000 (where fp32 resolves 6e-5): the fp64 path must accept
+    the inner and reject the outer ones; through faces and a corner as well."""
+    rng = np.random.default_rng(3)
+    r = 2.5
+    lo = np.array([990.0, -5.0, 300.0])
+    L = np.array([40.0, 40.0, 40.0])
+    box64 = np.concatenate([lo, L])
+    base = lo + np.array([[0.3, 0.3, 0.3], [20.0, 0.2, 39.9], [39.8, 39.7, 39.9], [7.0, 21.0, 33.0]])
+    pts, expect_pairs = [], []
+    for b in base:
+        i = len(pts)
+        pts.append(b)
+        for sgn in (+1, -1):
+            for eps, inside in ((-1e-10, True), (+1e-10, False), (-3e-6, True), (+3e-6, False)):
+                u = rng.normal(size=3)
+                u /= np.linalg.norm(u)
+                q = b + sgn * r * (1 + eps) * u
+                q = lo + np.mod(q - lo, L)
+                pts.append(q)
+                if inside:
+                    expect_pairs.append((i, len(pts) - 1))
+    pos64 = np.array(pts)
+    r64 = np.array([[r]])
+    out = gpu_run_f64(pos64, None, box64, r64, 1, 32, K=4)
+    rp, nb = ON.neighbor_list_f64(pos64, None, box64, r64, method="brute")
+    w = W.Workload("f64pairs", pos64.astype(np.float32), None, box64.astype(np.float32), r64.astype(np.float32), 32)
+    compare_with_oracle(w, out, (rp, nb, np.zeros(len(nb), np.uint8)))
+    for i, j in expect_pairs:
+        assert j in out["nlist"][i, : out["n_neigh"][i]]
+    assert len(nb) >= 2 * len(expect_pairs)
+
+
+def test_f64_full_size_config2():
+    w = W.make_config(2)
+    pos64, box64, r64 = W.as_f64(w)
+    out = gpu_run_f64(pos64, None, box64, r64, 1, w.max_neigh, K=32)
+    rp, nb = ON.neighbor_list_f64(pos64, None, box64, r64, method="cell")
+    rep = compare_with_oracle(w, out, (rp, nb, np.zeros(len(nb), np.uint8)))
+    assert rep["rows_checked"] == w.N
