@@ -24,7 +24,7 @@ sys.path.insert(0, ROOT)
 
 METRIC = "neighbor-list build+traverse ns/particle at 1M LJ"
 UNIT = "ns/particle"
-KERNELS_PER_STEP = 7    # morton_hist (+finalize in its last block), 4 x onesweep, tree (hierarchy+fit+quantize), traverse_group
+KERNELS_PER_STEP = 6    # morton_cell, cell_scan, cell_scatter, cell_tree, top_tree, traverse_group
 
 
 def measured_peaks():
@@ -100,8 +100,9 @@ def whole_job_value(ms_per_step: float, n_per_rank: int, world: int) -> float:
 def reference_sample(cid: int):
     """Bounded sample of the workload for the oracle arm: same recipe, density, cutoff; fewer particles."""
     from paper_1901_08088_b200 import workloads as W
-    if cid == 2:
-        return W.lj_lattice(N=131072, n_lat=51), "config-2 recipe at N=131,072 (n_lat=51), same density/jitter/cutoff"
+    if cid in (1, 2):
+        w = W.make_config(cid)
+        return w, f"the full workload (N={w.N}), one pass of the cell-list oracle per step"
     w = W.make_config(cid, small=True)
     return w, f"config-{cid} recipe at reduced size N={w.N}"
 
@@ -133,8 +134,9 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": False,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": f"BASELINE.json configs[{args.config - 1}] (bounded sample: {what})",
-                       "N_sample": w.N},
+            "config": {"workload": f"BASELINE.json configs[{args.config - 1}]: {w.name}", "N": w.N, "types": w.T,
+                       "r_list": [float(x) for x in np.asarray(w.r_list).reshape(-1)], "max_neigh": w.max_neigh,
+                       "sample": what},
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": what},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -163,13 +165,18 @@ def run_gpu(args):
     qbvh.qbvh_set_option(qbvh.OPT_LEAF_COLLAPSE, args.leaf_collapse)
     qbvh.qbvh_set_option(qbvh.OPT_STATS, 0)
     nl = qbvh.NeighborList(N, T=T, max_neigh=cap, device=dev)
-    pos = torch.from_numpy(w.pos).to(dev)
+    f64 = args.dtype == "f64"
+    if f64:                                            # fp64 particles, fp32 tree (an extra, not the headline)
+        pos64, box, r_list = W.as_f64(w, seed=rank)
+        pos = torch.from_numpy(pos64).to(dev)
+    else:
+        pos, box, r_list = torch.from_numpy(w.pos).to(dev), w.box, w.r_list
     typ = None if w.type is None else torch.from_numpy(w.type).to(dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
 
     def step():
-        nl.build(pos, typ, w.box)
-        return nl.neighbors(w.r_list, retry=False)
+        nl.build(pos, typ, box)
+        return nl.neighbors(r_list, retry=False)
 
     M = 0
     for _ in range(max(args.warmup, 3)):
@@ -189,9 +196,9 @@ def run_gpu(args):
     for s in range(K):
         flush.zero_()                                  # L2 flush between timed iterations (outside the events)
         ev[s][0].record()
-        nl.build(pos, typ, w.box)
+        nl.build(pos, typ, box)
         ev[s][1].record()
-        nl.neighbors(w.r_list, retry=False)
+        nl.neighbors(r_list, retry=False)
         ev[s][2].record()
     torch.cuda.synchronize()
     wall = time.perf_counter() - wall0
@@ -205,14 +212,16 @@ def run_gpu(args):
 
     # ---- statistics of the run (one instrumented pass, outside the timed region) ----
     qbvh.qbvh_set_option(qbvh.OPT_STATS, 1)
-    nl.neighbors(w.r_list, retry=False)
+    nl.neighbors(r_list, retry=False)
     stats = qbvh.qbvh_get_stats()
     qbvh.qbvh_set_option(qbvh.OPT_STATS, 0)
-    nn = stats["neighbors"] / N
+    nn = float(nl.n_neigh[:N].sum().item()) / N
+    counts = qbvh.qbvh_debug_export(qbvh.EXPORT_COUNTS, N)      # nodes written, query groups, cells, cell level
 
     # ---- end to end through the HOST-buffer C-ABI calls ----
     e2e_ms = None
-    if not args.no_e2e:
+    d2h = 0
+    if not args.no_e2e and not f64:
         stg = torch.empty(qbvh.qbvh_staging_bytes(N, cap), dtype=torch.uint8, device=dev)
         qbvh.qbvh_set_staging(stg)
         hpos = torch.from_numpy(w.pos).pin_memory()
@@ -233,10 +242,10 @@ def run_gpu(args):
         torch.cuda.synchronize()
         e2e_ms = e0.elapsed_time(e1) / Ke
         e2e_ms = max_over_ranks(e2e_ms, world, dev)
+        d2h = qbvh.qbvh_last_d2h_bytes()               # n_neigh + the min(M, max_neigh) columns actually copied + 8
         qbvh.qbvh_set_staging(None)
     clocks = sampler.stop()
     h2d = 12 * N + (4 * N if w.type is not None else 0)
-    d2h = 4 * N * cap + 4 * N + 8
 
     # ---- roofline of the dominant kernel (traverse_kernel), algorithmic bytes per SURVEY.md §8(d) ----
     peak, peak_src = measured_peaks()
@@ -244,22 +253,25 @@ def run_gpu(args):
     build_bytes = N * (188.0 + (4.0 if w.type is not None else 0.0))
     trav_ms, build_ms = float(np.mean(t_trav)), float(np.mean(t_build))
     ach = trav_bytes / (trav_ms * 1e-3) / 1e9
-    traffic = None
+    # DRAM traffic of one traversal launch: a STORED ncu measurement (dram__bytes_read.sum + dram__bytes_write.sum,
+    # profiles/), valid for config 2 / fp32 at the commit named beside it; null for anything else
+    traffic = traffic_commit = None
     tp = os.path.join(ROOT, "profiles", "traverse_traffic_bytes.txt")
-    if os.path.exists(tp):
+    if os.path.exists(tp) and args.config == 2 and not f64:
         try:
-            traffic = float(open(tp).read().split()[0])
+            tok = open(tp).read().split()
+            traffic, traffic_commit = float(tok[0]), (tok[1] if len(tok) > 1 else None)
         except Exception:
-            traffic = None
+            traffic = traffic_commit = None
     roofline = {"bound": "hbm", "kernel": "traverse_group_kernel", "achieved": ach, "peak": peak, "unit": "GB/s",
-                "frac": ach / peak, "traffic": traffic, "peak_source": peak_src,
-                "algorithmic_bytes_per_launch": trav_bytes}
+                "frac": ach / peak, "traffic": traffic, "traffic_source": "stored ncu capture", "traffic_commit": traffic_commit,
+                "peak_source": peak_src, "algorithmic_bytes_per_launch": trav_bytes}
     # plain-ALU view of the same kernel: thread-instructions issued / (148 SM x 128 lanes x f)
     whole = (trav_bytes + build_bytes) / (ms_per_step * 1e-3) / 1e9
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": max(args.warmup, 3),
             "ms_per_step": ms_per_step, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f32", "data": "synthetic",
+            "dtype": "f64 particles / f32 tree" if f64 else "f32", "data": "synthetic",
             "config": {"workload": f"BASELINE.json configs[{args.config - 1}]: {w.name}", "N": N, "types": T,
                        "r_list": [float(x) for x in np.asarray(w.r_list).reshape(-1)], "max_neigh": cap,
                        "leaf_collapse": args.leaf_collapse, "l2": "flushed between timed iterations (256 MiB memset)",
@@ -267,8 +279,15 @@ def run_gpu(args):
             "build_ms": build_ms, "traverse_ms": trav_ms,
             "build_ns_per_particle": 1e6 * build_ms / N, "traverse_ns_per_particle": 1e6 * trav_ms / N,
             "neighbors_per_particle": nn, "max_neighbors": int(M),
-            "dist_checks_per_s": stats["dist_checks"] / (trav_ms * 1e-3),
-            "node_tests_per_particle": stats["node_tests"] / N, "dist_checks_per_particle": stats["dist_checks"] / N,
+            # the timed (production) kernel: pair-predicate evaluations and node tests of the group walk
+            "dist_checks_per_s": stats["group_dist_checks"] / (trav_ms * 1e-3),
+            "dist_checks_per_particle": stats["group_dist_checks"] / N,
+            "node_tests_per_particle": stats["group_node_tests"] / N,
+            # census of Algorithm 1 walked once per particle on the same tree (the paper's kernel; not the timed one)
+            "census_node_tests_per_particle": stats["node_tests"] / N,
+            "census_dist_checks_per_particle": stats["dist_checks"] / N,
+            "nodes_written": int(counts[0]), "node_bytes": 16 * int(counts[0]), "node_bytes_uncollapsed": 16 * (2 * N - 1),
+            "query_groups": int(counts[1]), "morton_cells": int(counts[2]), "cell_level": int(counts[3]),
             "roofline": roofline,
             "roofline_whole_path": {"bound": "hbm", "achieved": whole, "peak": peak, "unit": "GB/s", "frac": whole / peak,
                                     "algorithmic_bytes_per_step": trav_bytes + build_bytes},
@@ -279,11 +298,71 @@ def run_gpu(args):
 
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         ws, what = (w, "the full workload, one pass (best of 2)") if N <= (1 << 21) else reference_sample(args.config)
-        t = time_oracle(ws, repeats=2)
+        if f64:
+            from oracle import neighbors as ON
+            t = {}
+            ON.neighbor_list_f64(pos64, w.type, box, r_list, method="cell", timing=t)
+            what = "the full fp64 workload, one pass of the fp64 cell-list oracle"
+        else:
+            t = time_oracle(ws, repeats=2)
         line["cpu_baseline"] = {"value": 1e9 * t["seconds"] / ws.N, "unit": UNIT, "cores": t["threads"],
                                 "kind": "oracle", "sample": what, "seconds": t["seconds"]}
     if rank == 0:
         print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def run_sharded(args):
+    """Strong-scaling extra (not the headline): the config's particles split over the ranks, one
+    all-gather of positions per step (NCCL), the full build on every rank, the traversal of the rank's Z-order slice."""
+    import torch
+    import torch.distributed as dist
+    from paper_1901_08088_b200 import qbvh, sharded
+    from paper_1901_08088_b200 import workloads as W
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    w = W.make_config(args.config, seed=0)              # ONE system, the same on every rank
+    qbvh.qbvh_set_option(qbvh.OPT_LEAF_COLLAPSE, args.leaf_collapse)
+    snl = sharded.ShardedNeighborList(w.N, T=w.T, max_neigh=w.max_neigh, device=dev)
+    lo, cnt = snl.own_first, snl.own_count
+    pos = torch.from_numpy(w.pos[lo:lo + cnt]).to(dev)
+    typ = None if w.type is None else torch.from_numpy(w.type[lo:lo + cnt]).to(dev)
+    nlist = torch.empty((max(snl.count, 1), w.max_neigh), dtype=torch.int32, device=dev)
+    n_neigh = torch.zeros(max(snl.count, 1), dtype=torch.int32, device=dev)
+
+    def step():
+        snl.build(pos, typ, w.box)
+        return qbvh.qbvh_neighbors_range(w.r_list, nlist, n_neigh, w.max_neigh, snl.first, snl.count)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    ms = max_over_ranks(e0.elapsed_time(e1) / args.steps, world, dev)
+    if rank == 0:
+        print(json.dumps({"metric": METRIC, "value": 1e6 * ms / w.N, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                          "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": False, "scaling": "strong",
+                          "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                          "config": {"workload": f"BASELINE.json configs[{args.config - 1}]: {w.name}", "N": w.N,
+                                     "parallelism": f"query sharding over {world} rank(s): all-gather of positions, full build per rank, Z-order slice per rank",
+                                     "l2": "not flushed (back-to-back steps)"},
+                          "gpu_launches": KERNELS_PER_STEP * args.steps}))
     if world > 1:
         dist.destroy_process_group()
     return 0
@@ -299,9 +378,13 @@ def main():
     ap.add_argument("--leaf-collapse", type=int, default=32)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg (profiling runs)")
+    ap.add_argument("--sharded", action="store_true", help="extra: query sharding over the ranks (strong scaling) instead of replicas")
+    ap.add_argument("--dtype", default="f32", choices=["f32", "f64"], help="f64: double-precision particles on the fp32 tree (an extra line)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.sharded:
+        return run_sharded(args)
     return run_gpu(args)
 
 

@@ -116,6 +116,14 @@ int qbvh_build(const float *pos, const int32_t *type, int64_t N, const float *bo
  * n_neigh[i] > max_neigh hold max_neigh true neighbors; re-allocate with capacity >= M and call again. */
 int qbvh_neighbors(const float *r_list_ij, int32_t *nlist, int32_t *n_neigh, int32_t max_neigh);
 
+/* Query sharding ("straightforwardly generalized to execute on multiple GPUs"): the
+ * same traversal for the particles at sorted (Z-order) positions [first, first + count) only.  Row k of nlist and
+ * n_neigh[k] belong to the particle at sorted position first + k, whose original index is QBVH_EXPORT_PERM[first + k];
+ * entries are ORIGINAL indices as always.  nlist: DEVICE count x max_neigh; n_neigh: DEVICE count.  Returns the
+ * maximum count over the range.  Every GPU of a sharded run holds all positions (one all-gather), builds the same
+ * tree and calls this for its own slice (paper_1901_08088_b200/sharded.py). */
+int qbvh_neighbors_range(const float *r_list_ij, int32_t *nlist, int32_t *n_neigh, int32_t max_neigh, int64_t first, int64_t count);
+
 /* ---- double-precision particle data -----------------------------
  * The tree stays what it is — fp32 frames, 10-bit quantized boxes, 16-byte nodes, built from the positions rounded to
  * fp32 — "the sphere radius is padded to account for uncertainty from loss of precision when the particle data is
@@ -147,8 +155,12 @@ int64_t qbvh_staging_bytes(int64_t N, int32_t max_neigh);
 int qbvh_set_staging(void *dev_ptr, int64_t bytes);
 /* pos, type: HOST (pinned memory makes the copies asynchronous).  Otherwise as qbvh_build. */
 int qbvh_build_host(const float *pos, const int32_t *type, int64_t N, const float *box);
-/* nlist, n_neigh: HOST.  Copies N x max_neigh + N int32 back after the traversal.  Otherwise as qbvh_neighbors. */
+/* nlist, n_neigh: HOST (N x max_neigh and N int32).  After the traversal n_neigh and the first min(M, max_neigh)
+ * columns of every row are copied back (M = the return value); columns beyond are left untouched.  Otherwise as
+ * qbvh_neighbors. */
 int qbvh_neighbors_host(const float *r_list_ij, int32_t *nlist, int32_t *n_neigh, int32_t max_neigh);
+/* Bytes the last qbvh_neighbors_host call copied from the device. */
+int64_t qbvh_last_d2h_bytes(void);
 
 /* ---- inspection ----------------------------------------------------------------------------- */
 

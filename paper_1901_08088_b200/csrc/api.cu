@@ -19,6 +19,7 @@ struct Context {
     int K_built = 1;
     float r_hint[QBVH_TMAX] = {0, 0, 0, 0};   // collapse heuristic: expected query radius against each tree (<= 0: none)
     bool f64_built = false;
+    int64_t last_d2h_bytes = 0;   // bytes the last qbvh_neighbors_host copied back
     int lvl_built = 0;
     bool stats = false;
     int variant = 1;
@@ -171,7 +172,8 @@ int make_params(const RT *r_list, bool f64, TraverseParams &P) {
 }
 
 template <typename RT>
-int neighbors_impl(const RT *r_list, bool f64, int32_t *nlist, int32_t *n_neigh, int32_t max_neigh) {
+int neighbors_impl(const RT *r_list, bool f64, int32_t *nlist, int32_t *n_neigh, int32_t max_neigh, int64_t q_first = 0,
+                   int64_t q_count = -1) {
     if (!g.built) return QBVH_ERR_NOT_BUILT;
     if (!r_list || max_neigh < 0) return QBVH_ERR_INVALID_ARG;
     if (f64 != g.f64_built) return QBVH_ERR_INVALID_ARG;          // qbvh_build_f64 pairs with qbvh_neighbors_f64
@@ -183,6 +185,9 @@ int neighbors_impl(const RT *r_list, bool f64, int32_t *nlist, int32_t *n_neigh,
     P.N = (int32_t)g.N;
     P.max_neigh = max_neigh;
     P.K = g.K_built;
+    P.q_first = (int32_t)q_first;
+    P.q_count = (int32_t)q_count;
+    if (q_count >= 0 && (g.variant != 1 || q_first < 0 || q_first + q_count > g.N)) return QBVH_ERR_INVALID_ARG;
     cudaError_t e;
     // reset group_cursor and max_count (+ stats) of the previous traversal
     e = cudaMemsetAsync(&g.buf.meta->group_cursor, 0, 2 * sizeof(int32_t), g.stream);
@@ -361,6 +366,13 @@ int qbvh_neighbors(const float *r_list_ij, int32_t *nlist, int32_t *n_neigh, int
     return finish_neighbors();
 }
 
+int qbvh_neighbors_range(const float *r_list_ij, int32_t *nlist, int32_t *n_neigh, int32_t max_neigh, int64_t first, int64_t count) {
+    if (count < 0) return QBVH_ERR_INVALID_ARG;
+    int rc = neighbors_impl(r_list_ij, false, nlist, n_neigh, max_neigh, first, count);
+    if (rc != QBVH_OK) return rc;
+    return finish_neighbors();
+}
+
 int qbvh_build_f64(const double *pos, const int32_t *type, int64_t N, const double *box) {
     if (!box) return QBVH_ERR_INVALID_ARG;
     float box32[6];
@@ -386,6 +398,7 @@ int qbvh_count_overlaps(const float *r_list_ij, int32_t *n_overlap) {
     const int prc = make_params(r_list_ij, false, P);
     if (prc != QBVH_OK) return prc;
     P.max_neigh = 0;
+    P.q_first = 0, P.q_count = -1;
     cudaError_t e = cudaMemsetAsync(&g.buf.meta->group_cursor, 0, 2 * sizeof(int32_t), g.stream);
     if (e != cudaSuccess) return cuda_fail(e, "memset max_count");
     e = launch_count_overlaps(P, g.buf, n_overlap, g.stream);
@@ -439,16 +452,28 @@ int qbvh_neighbors_host(const float *r_list_ij, int32_t *nlist, int32_t *n_neigh
     if (N > 0 && (!n_neigh || (!nlist && max_neigh > 0))) return QBVH_ERR_INVALID_ARG;
     int rc = neighbors_impl(r_list_ij, false, dlist, dcnt, max_neigh);
     if (rc != QBVH_OK) return rc;
+    cudaError_t e = cudaSuccess;
     if (N > 0) {
-        cudaError_t e = cudaMemcpyAsync(n_neigh, dcnt, 4 * N, cudaMemcpyDeviceToHost, g.stream);
+        e = cudaMemcpyAsync(n_neigh, dcnt, 4 * N, cudaMemcpyDeviceToHost, g.stream);
         if (e != cudaSuccess) return cuda_fail(e, "D2H n_neigh");
-        if (max_neigh > 0) {
-            e = cudaMemcpyAsync(nlist, dlist, 4 * N * (int64_t)max_neigh, cudaMemcpyDeviceToHost, g.stream);
-            if (e != cudaSuccess) return cuda_fail(e, "D2H nlist");
-        }
     }
-    return finish_neighbors();
+    const int M = finish_neighbors();          // synchronises: the longest row is known now
+    if (M < 0) return M;
+    g.last_d2h_bytes = 4 * N + 8;
+    if (N > 0 && max_neigh > 0 && M > 0) {
+        // only the columns that were produced: rows hold at most min(M, max_neigh) entries (the rest is unspecified)
+        const int64_t cols = M < max_neigh ? M : max_neigh;
+        e = cudaMemcpy2DAsync(nlist, (size_t)4 * max_neigh, dlist, (size_t)4 * max_neigh, (size_t)4 * cols, (size_t)N,
+                              cudaMemcpyDeviceToHost, g.stream);
+        if (e != cudaSuccess) return cuda_fail(e, "D2H nlist");
+        e = cudaStreamSynchronize(g.stream);
+        if (e != cudaSuccess) return cuda_fail(e, "stream synchronize");
+        g.last_d2h_bytes += 4 * cols * N;
+    }
+    return M;
 }
+
+int64_t qbvh_last_d2h_bytes(void) { return g.last_d2h_bytes; }
 
 float qbvh_padded_radius(float r, const float *box) {
     if (!box || !(r > 0.0f) || !std::isfinite(r)) return -1.0f;

@@ -87,6 +87,7 @@ struct TraverseParams {
     int32_t N;
     int32_t max_neigh;
     int32_t K;                         // leaf-collapse cap used by the build
+    int32_t q_first, q_count;          // query sharding: only these sorted positions are queries, row = position - q_first; q_count < 0: all, row = original index
     // double-precision particle data (qbvh_neighbors_f64): r2 above is then (r + B)^2 rounded up — whatever fails it
     // in fp32 on the rounded positions cannot be a neighbor in fp64 —, r2lo = (r - B)^2 rounded down — whatever passes
     // it certainly is one —, and only the pairs in between are decided by the fp64 predicate.

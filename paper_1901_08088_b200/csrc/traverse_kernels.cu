@@ -443,9 +443,14 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
         if (g >= ngroups) break;
         const uint2 grp = __ldg(groups + g);
         const int gfirst = (int)grp.x, gcnt = (int)grp.y;
-        const bool live = lane < gcnt;
-        const float4 me = live ? __ldg(sorted_pos + gfirst + lane) : make_float4(0.f, 0.f, 0.f, 0.f);
-        const int orig_i = live ? __float_as_int(me.w) : -1;
+        // query sharding (qbvh_neighbors_range): only the particles at sorted positions [q_first, q_first + q_count)
+        // are queries; the other members of a group that straddles the edge stay candidates
+        if (P.q_count >= 0 && (gfirst + gcnt <= P.q_first || gfirst >= P.q_first + P.q_count)) continue;
+        const bool member = lane < gcnt;
+        const bool live = member && (P.q_count < 0 || (unsigned)(gfirst + lane - P.q_first) < (unsigned)P.q_count);
+        const float4 me = member ? __ldg(sorted_pos + gfirst + lane) : make_float4(0.f, 0.f, 0.f, 0.f);
+        const int orig_i = member ? __float_as_int(me.w) : -1;
+        const int row_i = P.q_count < 0 ? orig_i : gfirst + lane - P.q_first;   // row of the list this lane writes
         int ta = 0;
 #pragma unroll
         for (int t = 1; t < QBVH_TMAX; ++t) ta += (gfirst >= meta->seg[t]) ? 1 : 0;
@@ -460,7 +465,7 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
                 ghi[d] = ord2f(__reduce_max_sync(FULL, live ? f2ord(v[d]) : 0u));
             }
         }
-        int32_t *const row = nlist + (size_t)(live ? orig_i : 0) * (size_t)cap;
+        int32_t *const row = nlist + (size_t)(live ? row_i : 0) * (size_t)cap;
         const u64 nmx = pk2(-me.x, -me.x), nmy = pk2(-me.y, -me.y), nmz = pk2(-me.z, -me.z);
         uint32_t po = rot;               // ring byte offset: rot + 4 x neighbors found so far for this lane's particle
         int flushed = 0;                 // neighbors already written to the list row (a multiple of 16)
@@ -508,7 +513,7 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
             const int32_t *const etab = entry + tb * ENTRY_CELLS;
             F64Ctx fx;
             if (F64) {
-                fx.sp64 = sorted_pos64, fx.tp = s_tp[warp], fx.ksort_i = gfirst + (live ? lane : 0);
+                fx.sp64 = sorted_pos64, fx.tp = s_tp[warp], fx.ksort_i = gfirst + (member ? lane : 0);
                 fx.r2_64 = P.r2_64[ta * QBVH_TMAX + tb], fx.r2lo = P.r2lo[ta * QBVH_TMAX + tb];
             }
             // ---- Alg. 1 line 4: lane j tests image j of the group box against the root node; the vote is the bitset ----
@@ -542,7 +547,7 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
                 const bool own_image = (tb == ta) && !shifted;
                 const bool own_tree = own_image && aligned, self_all = own_image && !aligned;
                 if (own_tree) {
-                    sm.tx[lane] = live ? me.x : __int_as_float(0x7FC00000);   // NaN: never accepted
+                    sm.tx[lane] = member ? me.x : __int_as_float(0x7FC00000);   // NaN: never accepted
                     sm.ty[lane] = me.y;
                     sm.tz[lane] = me.z;
                     sm.ti[lane] = orig_i;
@@ -747,7 +752,7 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
                         if (4 * j + 3 < rem && o + 3 < cap) row[o + 3] = v.w;
                     }
                 }
-            if (live) n_neigh[orig_i] = cnt;
+            if (live) n_neigh[row_i] = cnt;
             wmax = max(wmax, live ? cnt : 0);
         }
         __syncwarp();

@@ -24,7 +24,7 @@ EXPORT_KEYS_SORTED, EXPORT_PERM, EXPORT_NODES, EXPORT_PARENT, EXPORT_FRAMES, EXP
 SYMBOLS = ("qbvh_set_stream", "qbvh_set_num_types", "qbvh_workspace_bytes", "qbvh_set_workspace",
            "qbvh_set_option", "qbvh_get_option", "qbvh_build", "qbvh_neighbors", "qbvh_count_overlaps", "qbvh_staging_bytes",
            "qbvh_set_staging", "qbvh_build_host", "qbvh_neighbors_host", "qbvh_get_stats", "qbvh_debug_export",
-           "qbvh_error_string", "qbvh_padded_radius", "qbvh_set_collapse_hint", "qbvh_build_f64", "qbvh_neighbors_f64")
+           "qbvh_error_string", "qbvh_padded_radius", "qbvh_set_collapse_hint", "qbvh_build_f64", "qbvh_neighbors_f64", "qbvh_last_d2h_bytes", "qbvh_neighbors_range")
 
 
 class QbvhStats(C.Structure):
@@ -56,6 +56,7 @@ _lib.qbvh_set_collapse_hint.argtypes = [_vp, _i32]
 _lib.qbvh_build.argtypes = [_vp, _vp, _i64, _vp]
 _lib.qbvh_neighbors.argtypes = [_vp, _vp, _vp, _i32]
 _lib.qbvh_count_overlaps.argtypes = [_vp, _vp]
+_lib.qbvh_neighbors_range.argtypes = [_vp, _vp, _vp, _i32, _i64, _i64]
 _lib.qbvh_build_f64.argtypes = [_vp, _vp, _i64, _vp]
 _lib.qbvh_neighbors_f64.argtypes = [_vp, _vp, _vp, _i32]
 _lib.qbvh_staging_bytes.argtypes = [_i64, _i32]
@@ -63,6 +64,8 @@ _lib.qbvh_staging_bytes.restype = _i64
 _lib.qbvh_set_staging.argtypes = [_vp, _i64]
 _lib.qbvh_build_host.argtypes = [_vp, _vp, _i64, _vp]
 _lib.qbvh_neighbors_host.argtypes = [_vp, _vp, _vp, _i32]
+_lib.qbvh_last_d2h_bytes.argtypes = []
+_lib.qbvh_last_d2h_bytes.restype = _i64
 _lib.qbvh_get_stats.argtypes = [C.POINTER(QbvhStats)]
 _lib.qbvh_debug_export.argtypes = [_i32, _vp, _i64]
 _lib.qbvh_debug_export.restype = _i64
@@ -164,6 +167,13 @@ def qbvh_neighbors(r_list_ij, nlist, n_neigh, max_neigh: int) -> int:
     return _check(_lib.qbvh_neighbors(r.ctypes.data, _ptr(nlist), _ptr(n_neigh), max_neigh), "qbvh_neighbors")
 
 
+def qbvh_neighbors_range(r_list_ij, nlist, n_neigh, max_neigh: int, first: int, count: int) -> int:
+    """Lists of the particles at sorted positions [first, first + count) only (row k = sorted position first + k)."""
+    r = _r_list(r_list_ij)
+    return _check(_lib.qbvh_neighbors_range(r.ctypes.data, _ptr(nlist), _ptr(n_neigh), max_neigh, first, count),
+                  "qbvh_neighbors_range")
+
+
 def qbvh_build_f64(pos, type, N: int, box) -> int:
     """pos: DEVICE float64 N x 3; type: DEVICE int32 N or None; box: 6 host doubles."""
     box = np.ascontiguousarray(box, dtype=np.float64).reshape(-1)
@@ -213,6 +223,10 @@ def qbvh_padded_radius(r: float, box) -> float:
     if v < 0:
         raise QbvhError(ERR_INVALID_ARG, "qbvh_padded_radius")
     return v
+
+
+def qbvh_last_d2h_bytes() -> int:
+    return int(_lib.qbvh_last_d2h_bytes())
 
 
 def qbvh_get_stats() -> dict:

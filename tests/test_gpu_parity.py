@@ -601,3 +601,35 @@ def test_f64_full_size_config2():
     rp, nb = ON.neighbor_list_f64(pos64, None, box64, r64, method="cell")
     rep = compare_with_oracle(w, out, (rp, nb, np.zeros(len(nb), np.uint8)))
     assert rep["rows_checked"] == w.N
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# query sharding.  One GPU here, so the ranks' calls are made one after another on one tree:
+# qbvh_neighbors_range for every Z-order slice, merged, must be the oracle's list.
+# ---------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("world", [2, 3, 7])
+@pytest.mark.parametrize("cid", [1, 3, 5])
+def test_query_sharding_slices_merge_to_the_oracle(cid, world):
+    import torch
+    from paper_1901_08088_b200 import qbvh, sharded
+    w = W.make_config(cid, small=True)
+    dev = torch.device("cuda:0")
+    qbvh.qbvh_set_option(qbvh.OPT_LEAF_COLLAPSE, 32)
+    qbvh.qbvh_set_collapse_hint(None)
+    be = sharded.CudaBackend(w.N, w.T, 16, dev)                    # capacity too small on purpose: the retry path
+    be.build(torch.from_numpy(w.pos).to(dev), None if w.type is None else torch.from_numpy(w.type).to(dev), w.box)
+    parts = []
+    for g in range(world):
+        first, count = sharded.slice_bounds(w.N, world, g)
+        rows, n_neigh, nlist, M = be.neighbors_range(w.r_list, first, count)
+        parts.append((rows.numpy(), n_neigh.cpu().numpy(), nlist.cpu().numpy()))
+        assert M == (int(n_neigh.max().item()) if count else 0)
+    n_all, l_all = sharded.merge_slices(w.N, parts)
+    out = {"M": int(n_all.max()), "max_neigh": l_all.shape[1], "nlist": l_all, "n_neigh": n_all}
+    compare_with_oracle(w, out, ON.neighbor_list(w.pos, w.type, w.box, w.r_list))
+    # world size 1 through the distributed wrapper (no process group: a single rank)
+    snl = sharded.ShardedNeighborList(w.N, T=w.T, max_neigh=w.max_neigh, device=dev)
+    snl.build(torch.from_numpy(w.pos).to(dev), None if w.type is None else torch.from_numpy(w.type).to(dev), w.box)
+    rows, n_neigh, nlist, M = snl.neighbors(w.r_list)
+    n1, l1 = sharded.merge_slices(w.N, [(rows.numpy(), n_neigh.cpu().numpy(), nlist.cpu().numpy())])
+    assert np.array_equal(n1, n_all)
