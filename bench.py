@@ -164,6 +164,8 @@ def run_gpu(args):
     N, T, cap = w.N, w.T, w.max_neigh
     qbvh.qbvh_set_option(qbvh.OPT_LEAF_COLLAPSE, args.leaf_collapse)
     qbvh.qbvh_set_option(qbvh.OPT_STATS, 0)
+    if args.variant is not None:
+        qbvh.qbvh_set_option(qbvh.OPT_VARIANT, args.variant)
     nl = qbvh.NeighborList(N, T=T, max_neigh=cap, device=dev)
     f64 = args.dtype == "f64"
     if f64:                                            # fp64 particles, fp32 tree (an extra, not the headline)
@@ -378,6 +380,7 @@ def main():
     ap.add_argument("--leaf-collapse", type=int, default=32)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg (profiling runs)")
+    ap.add_argument("--variant", type=int, default=None, help="traversal kernel (QBVH_OPT_VARIANT); default: the library's")
     ap.add_argument("--sharded", action="store_true", help="extra: query sharding over the ranks (strong scaling) instead of replicas")
     ap.add_argument("--dtype", default="f32", choices=["f32", "f64"], help="f64: double-precision particles on the fp32 tree (an extra line)")
     args = ap.parse_args()

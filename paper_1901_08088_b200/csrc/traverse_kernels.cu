@@ -468,32 +468,33 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
         int32_t *const row = nlist + (size_t)(live ? row_i : 0) * (size_t)cap;
         const u64 nmx = pk2(-me.x, -me.x), nmy = pk2(-me.y, -me.y), nmz = pk2(-me.z, -me.z);
         uint32_t po = rot;               // ring byte offset: rot + 4 x neighbors found so far for this lane's particle
-        int flushed = 0;                 // neighbors already written to the list row (a multiple of 16)
+        int flushed = 0;                 // neighbors already written to the list row (a multiple of 8)
         int thead = 0, tcount = 0;       // candidate tile ring: first slot (a multiple of 32), number of candidates
         if (STATS) ++st_groups;
 
-        // lanes write their complete 64-byte blocks of staged neighbors to their list rows
+        // Lanes write their complete 32-byte blocks (one sector, one 256-bit store) of staged neighbors to their list
+        // rows.  Called when SOME lane runs out of ring space; EVERY lane with a complete block joins in, so the lanes
+        // stay in step and a visit serves most of them (a visit per lane and block cost 3x the instructions).
         auto flush_blocks = [&]() {
-            while (__any_sync(FULL, (int)((po - rot) >> 2) - flushed >= 16)) {
-                if ((int)((po - rot) >> 2) - flushed >= 16) {
+            while (__any_sync(FULL, (int)((po - rot) >> 2) - flushed >= 8)) {
+                if ((int)((po - rot) >> 2) - flushed >= 8) {
                     const uint32_t off = rot + 4u * (uint32_t)flushed;
-                    int4 v[4];
+                    int4 v[2];
 #pragma unroll
-                    for (int j = 0; j < 4; ++j)
+                    for (int j = 0; j < 2; ++j)
                         v[j] = *static_cast<const int4 *>(
                             __cvta_shared_to_generic((size_t)(ring_s | ((off + 16u * j) & (GW_RING_BYTES - 16)))));
-                    if (vec256_ok && flushed + 16 <= cap) {       // the common case: two aligned 256-bit stores (sm_100)
+                    if (vec256_ok && flushed + 8 <= cap) {        // the common case: one aligned 256-bit store (sm_100)
                         st_global_256(row + flushed, v[0], v[1]);
-                        st_global_256(row + flushed + 8, v[2], v[3]);
-                    } else if (vec_ok && flushed + 16 <= cap) {   // four aligned 128-bit stores
+                    } else if (vec_ok && flushed + 8 <= cap) {    // two aligned 128-bit stores
                         int4 *dst = reinterpret_cast<int4 *>(row + flushed);
-#pragma unroll
-                        for (int j = 0; j < 4; ++j) dst[j] = v[j];
+                        dst[0] = v[0];
+                        dst[1] = v[1];
                     } else {
-#pragma unroll
-                        for (int j = 0; j < 4; ++j) store4(row, flushed + 4 * j, cap, false, v[j]);
+                        store4(row, flushed, cap, false, v[0]);
+                        store4(row, flushed + 4, cap, false, v[1]);
                     }
-                    flushed += 16;
+                    flushed += 8;
                 }
             }
         };

@@ -4,7 +4,7 @@ from __future__ import annotations
 import numpy as np
 
 
-def gpu_run(w, K=4, max_neigh=None, stats=False, export=False, retry=False, hint=None):
+def gpu_run(w, K=4, max_neigh=None, stats=False, export=False, retry=False, hint=None, variant=None):
     """Build + traverse workload `w` on cuda:0.  Returns dict(nlist, n_neigh, M, [exports], [stats])."""
     import torch
     from paper_1901_08088_b200 import qbvh
@@ -14,6 +14,9 @@ def gpu_run(w, K=4, max_neigh=None, stats=False, export=False, retry=False, hint
     qbvh.qbvh_set_option(qbvh.OPT_LEAF_COLLAPSE, K)
     qbvh.qbvh_set_option(qbvh.OPT_STATS, int(stats))
     qbvh.qbvh_set_collapse_hint(hint)
+    prev_variant = qbvh.qbvh_get_option(qbvh.OPT_VARIANT)
+    if variant is not None:
+        qbvh.qbvh_set_option(qbvh.OPT_VARIANT, variant)
     nl = qbvh.NeighborList(w.N, T=w.T, max_neigh=max_neigh, device=dev)
     pos = torch.from_numpy(w.pos).to(dev)
     typ = None if w.type is None else torch.from_numpy(w.type).to(dev)
@@ -41,6 +44,7 @@ def gpu_run(w, K=4, max_neigh=None, stats=False, export=False, retry=False, hint
         out["stats"] = qbvh.qbvh_get_stats()
     qbvh.qbvh_set_option(qbvh.OPT_STATS, 0)
     qbvh.qbvh_set_collapse_hint(None)
+    qbvh.qbvh_set_option(qbvh.OPT_VARIANT, prev_variant)
     return out
 
 
