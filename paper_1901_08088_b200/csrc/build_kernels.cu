@@ -237,6 +237,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) cell_scan_kernel(const uint32_t 
                                                                   uint32_t *__restrict__ cell_start,
                                                                   uint32_t *__restrict__ cell_list, int ncells,
                                                                   TreeMeta *__restrict__ meta) {
+    cudaGridDependencySynchronize();
     __shared__ unsigned long long s_warp[SCAN_THREADS / 32], s_pre[SCAN_THREADS / 32];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int tile = blockIdx.x, ntiles = gridDim.x;
@@ -335,6 +336,7 @@ __global__ void __launch_bounds__(256) cell_scatter_kernel(const uint32_t *__res
                                                             int N, int cell_shift, const uint32_t *__restrict__ cell_start,
                                                             uint2 *__restrict__ ent, uint32_t *__restrict__ cell_count, int ncells,
                                                             TreeMeta *__restrict__ meta, const FinalizeParams fp) {
+    cudaGridDependencySynchronize();
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     // the counters have been scanned: clear them for the next build
     for (int c = i; c < ncells; c += gridDim.x * blockDim.x) cell_count[c] = 0u;
@@ -965,6 +967,7 @@ __device__ void process_cell(const TreeCtx &cx, const CellArrays A, int j, int r
 
 constexpr int CELL_WARPS = 4;
 __global__ void __launch_bounds__(CELL_WARPS * 32) cell_tree_kernel(const TreeCtx cx) {
+    cudaGridDependencySynchronize();
     __shared__ __align__(16) unsigned char s_mem[CELL_WARPS][CELL_WARP_MAX * CELL_BYTES_PER_SLOT];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int j = blockIdx.x * CELL_WARPS + warp;
@@ -980,6 +983,7 @@ __global__ void __launch_bounds__(CELL_WARPS * 32) cell_tree_kernel(const TreeCt
 
 constexpr int TOP_THREADS = 512;
 __global__ void __launch_bounds__(TOP_THREADS) top_tree_kernel(const TreeCtx cx) {
+    cudaGridDependencySynchronize();
     extern __shared__ __align__(16) unsigned char s_dyn[];
     // ---- cells too large for one warp (rare: strongly clustered input), one block each ----
     const int nbig = cx.meta->nbig;
@@ -1032,6 +1036,21 @@ __global__ void __launch_bounds__(TOP_THREADS) top_tree_kernel(const TreeCtx cx)
 }
 
 // ------------------------------------------------------------------------------------------------------------
+// The build is a chain of five dependent launches.  The four dependents are launched with programmatic stream
+// serialization (programmatic dependent launch): their blocks may be scheduled while the predecessor drains and wait in
+// cudaGridDependencySynchronize() — the first statement of each of those kernels — until the predecessor's memory is
+// visible, which takes the launch latency off the critical path.
+template <typename... KArgs, typename... Args>
+static cudaError_t launch_dependent(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid, cfg.blockDim = block, cfg.dynamicSmemBytes = smem, cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr, cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
 int pick_cell_level(int64_t N, int T) {
     // the smallest grid with at most ~48 particles per cell on average, T * 8^lvl <= CELL_MAX_TOTAL
     int lvl = CELL_LMIN;
@@ -1080,8 +1099,11 @@ cudaError_t launch_build(const void *pos, const int32_t *type, const BuildParams
     fp.N = N, fp.T = p.T, fp.lvl = lvl, fp.warp_slots = traverse_warp_slots();
     for (int t = 0; t < QBVH_TMAX; ++t) fp.r_hint[t] = p.r_hint[t];
     const int tiles = (ncells + SCAN_TILE - 1) / SCAN_TILE;
-    cell_scan_kernel<<<tiles, SCAN_THREADS, 0, st>>>(b.cell_count, b.cell_start, b.cell_list, ncells, b.meta);
-    cell_scatter_kernel<<<(N + 255) / 256, 256, 0, st>>>(b.key, b.rank, N, cell_shift, b.cell_start, b.ent, b.cell_count, ncells, b.meta, fp);
+    err = launch_dependent(cell_scan_kernel, dim3(tiles), dim3(SCAN_THREADS), 0, st, b.cell_count, b.cell_start, b.cell_list, ncells, b.meta);
+    if (err != cudaSuccess) return err;
+    err = launch_dependent(cell_scatter_kernel, dim3((N + 255) / 256), dim3(256), 0, st, b.key, b.rank, N, cell_shift, b.cell_start, b.ent,
+                           b.cell_count, ncells, b.meta, fp);
+    if (err != cudaSuccess) return err;
     TreeCtx cx;
     cx.pos = pos, cx.f64 = p.f64 ? 1 : 0, cx.N = N, cx.K = p.K, cx.lvl = lvl, cx.build_tag = p.build_tag;
     cx.cell_start = b.cell_start, cx.cell_list = b.cell_list, cx.ent = b.ent;
@@ -1090,7 +1112,10 @@ cudaError_t launch_build(const void *pos, const int32_t *type, const BuildParams
     cx.nodes = b.nodes, cx.parent = b.parent, cx.slot = b.slot, cx.groups = b.groups, cx.entry = b.entry;
     cx.big_list = b.big_list, cx.croot = b.croot, cx.scratch = b.scratch, cx.meta = b.meta;
     const int max_cells = min(N, ncells);
-    cell_tree_kernel<<<(max_cells + CELL_WARPS - 1) / CELL_WARPS, CELL_WARPS * 32, 0, st>>>(cx);
-    top_tree_kernel<<<(max_cells + TOP_THREADS - 1) / TOP_THREADS, TOP_THREADS, CELL_BLOCK_MAX * CELL_BYTES_PER_SLOT, st>>>(cx);
+    err = launch_dependent(cell_tree_kernel, dim3((max_cells + CELL_WARPS - 1) / CELL_WARPS), dim3(CELL_WARPS * 32), 0, st, cx);
+    if (err != cudaSuccess) return err;
+    err = launch_dependent(top_tree_kernel, dim3((max_cells + TOP_THREADS - 1) / TOP_THREADS), dim3(TOP_THREADS),
+                           (size_t)CELL_BLOCK_MAX * CELL_BYTES_PER_SLOT, st, cx);
+    if (err != cudaSuccess) return err;
     return cudaGetLastError();
 }
