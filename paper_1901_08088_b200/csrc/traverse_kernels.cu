@@ -302,8 +302,10 @@ __device__ __forceinline__ void ring_put(uint32_t ring_s, uint32_t &po, int32_t 
 //   D = (p_j - p_i) [- s L];  d2 = fma(Dz, Dz, fma(Dy, Dy, Dx*Dx));  d2 <= r^2
 // evaluated for two candidates per instruction.  SELF: the tile holds the members of the group itself.
 // What the fp64 path adds (qbvh_neighbors_f64): the pair is first judged in fp32 on the positions
-// rounded to fp32; only if its squared distance falls between r2lo and r2 (about one pair in two thousand) the
-// canonical fp64 predicate decides, on the Z-ordered double positions.
+// rounded to fp32.  d2 <= r2lo: certainly a neighbor, appended as in the fp32 kernel.  r2lo < d2 <= r2 (the band, about
+// one pair per query group): its tile slot is remembered in a bit mask — one predicated instruction, no branch in the
+// loop — and after the chunk the lanes that have any decide theirs with the canonical fp64 predicate
+// on the Z-ordered double positions.
 struct F64Ctx {
     const Pos64 *sp64;     // Z-ordered fp64 positions
     const int32_t *tp;     // sorted position of every candidate of the tile ring
@@ -321,6 +323,8 @@ __device__ __noinline__ bool exact_pair_f64(const Pos64 *__restrict__ sp64, int 
 template <bool SHIFTED, bool SELF, int NC, bool F64>
 __device__ __forceinline__ void check_tile(const GwShared &sm, int base, u64 nmx, u64 nmy, u64 nmz, u64 ns0, u64 ns1,
                                         u64 ns2, float r2, int orig_i, uint32_t ring_s, uint32_t &po, const F64Ctx &fx) {
+    const float r2a = F64 ? fx.r2lo : r2;        // what is appended without further ado
+    uint32_t band = 0;
 #pragma unroll
     for (int j = 0; j < NC / 4; ++j) {
         const float4 X = *reinterpret_cast<const float4 *>(&sm.tx[base + 4 * j]);
@@ -340,14 +344,24 @@ __device__ __forceinline__ void check_tile(const GwShared &sm, int base, u64 nmx
         float d0, d1, d2, d3;
         upk2(dd0, d0, d1);
         upk2(dd1, d2, d3);
-        auto sure = [&](float d, int c) -> bool {
-            if (!F64) return true;
-            return d <= fx.r2lo || exact_pair_f64(fx.sp64, fx.ksort_i, fx.tp[base + 4 * j + c], fx.s0, fx.s1, fx.s2, fx.r2_64);
-        };
-        if (d0 <= r2 && (!SELF || I.x != orig_i) && sure(d0, 0)) { ring_put(ring_s, po, I.x); }
-        if (d1 <= r2 && (!SELF || I.y != orig_i) && sure(d1, 1)) { ring_put(ring_s, po, I.y); }
-        if (d2 <= r2 && (!SELF || I.z != orig_i) && sure(d2, 2)) { ring_put(ring_s, po, I.z); }
-        if (d3 <= r2 && (!SELF || I.w != orig_i) && sure(d3, 3)) { ring_put(ring_s, po, I.w); }
+        const bool s0 = !SELF || I.x != orig_i, s1 = !SELF || I.y != orig_i, s2 = !SELF || I.z != orig_i, s3 = !SELF || I.w != orig_i;
+        if (d0 <= r2a && s0) { ring_put(ring_s, po, I.x); }
+        if (d1 <= r2a && s1) { ring_put(ring_s, po, I.y); }
+        if (d2 <= r2a && s2) { ring_put(ring_s, po, I.z); }
+        if (d3 <= r2a && s3) { ring_put(ring_s, po, I.w); }
+        if (F64) {
+            if (d0 <= r2 && !(d0 <= r2a) && s0) band |= 1u << (4 * j + 0);
+            if (d1 <= r2 && !(d1 <= r2a) && s1) band |= 1u << (4 * j + 1);
+            if (d2 <= r2 && !(d2 <= r2a) && s2) band |= 1u << (4 * j + 2);
+            if (d3 <= r2 && !(d3 <= r2a) && s3) band |= 1u << (4 * j + 3);
+        }
+    }
+    if (F64 && __any_sync(0xFFFFFFFFu, band != 0)) {
+        while (band) {
+            const int slot = base + __ffs(band) - 1;
+            band &= band - 1;
+            if (exact_pair_f64(fx.sp64, fx.ksort_i, fx.tp[slot], fx.s0, fx.s1, fx.s2, fx.r2_64)) ring_put(ring_s, po, sm.ti[slot]);
+        }
     }
 }
 
@@ -515,7 +529,7 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
             F64Ctx fx;
             if (F64) {
                 fx.sp64 = sorted_pos64, fx.tp = s_tp[warp], fx.ksort_i = gfirst + (member ? lane : 0);
-                fx.r2_64 = P.r2_64[ta * QBVH_TMAX + tb], fx.r2lo = P.r2lo[ta * QBVH_TMAX + tb];
+                fx.r2_64 = P.r2_64[ta * QBVH_TMAX + tb], fx.r2lo = live ? P.r2lo[ta * QBVH_TMAX + tb] : -1.0f;   // idle lanes never accept
             }
             // ---- Alg. 1 line 4: lane j tests image j of the group box against the root node; the vote is the bitset ----
             uint32_t bset;
