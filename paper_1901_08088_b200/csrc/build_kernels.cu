@@ -857,7 +857,8 @@ __device__ void process_cell(const TreeCtx &cx, const CellArrays A, int j, int r
         const int lane = rank;
         int written = 0;
         CellRoot r;
-        r.first = F, r.last = F + n - 1, r.dL = dLc, r.dR = dRc, r.dnext = n_next >= 2 ? 64 : dNN, r.pad = 0;
+        r.first = F, r.last = F + n - 1, r.d = cell_root_d(dLc, dRc, n_next >= 2 ? 64 : dNN, false);
+        r.key0 = (uint32_t)(A.kv[0] >> 32), r.pad[0] = r.pad[1] = 0u;
         if (n <= cx.K) {
             uint32_t lo, hi;
             range_box(A, 0, n - 1, lane, lo, hi);
@@ -951,10 +952,8 @@ __device__ void process_cell(const TreeCtx &cx, const CellArrays A, int j, int r
         r.whi = A.whi[0];
         r.first = F;
         r.last = F + n - 1;
-        r.dL = dLc;
-        r.dR = dRc;
-        r.dnext = n_next >= 2 ? 64 : dNN;
-        r.pad = 0;
+        r.d = cell_root_d(dLc, dRc, n_next >= 2 ? 64 : dNN, G != 32);
+        r.key0 = (uint32_t)(A.kv[0] >> 32), r.pad[0] = r.pad[1] = 0u;
         cx.croot[j] = r;
     }
     if (G == 32) {
@@ -975,7 +974,10 @@ __global__ void __launch_bounds__(CELL_WARPS * 32) cell_tree_kernel(const TreeCt
     const uint32_t c = __ldg(cx.cell_list + j);
     const int n = (int)(__ldg(cx.cell_start + c + 1) - __ldg(cx.cell_start + c));
     if (n > CELL_WARP_MAX) {                        // too large for a warp: a whole block takes it in the next launch
-        if (lane == 0) cx.big_list[atomicAdd(&cx.meta->nbig, 1)] = j;
+        if (lane == 0) {
+            cx.big_list[atomicAdd(&cx.meta->nbig, 1)] = j;
+            cx.croot[j].d = CELL_ROOT_BIG;
+        }
         return;
     }
     process_cell<32>(cx, carve_cell_arrays(s_mem[warp], CELL_WARP_MAX), j, lane, false);
@@ -1021,18 +1023,63 @@ __global__ void __launch_bounds__(TOP_THREADS) top_tree_kernel(const TreeCtx cx)
             const CellRoot r = cx.croot[j];
             Child me;
             me.wlo = r.wlo & 0x7FFFFFFFu, me.whi = r.whi, me.f = r.first, me.l = r.last, me.pend = (r.wlo >> 31) != 0;
-            walk_up(cx, me, r.dL, r.dR, r.dnext);
+            walk_up(cx, me, (int)(r.d & 255u) - 1, (int)((r.d >> 8) & 255u) - 1, (int)((r.d >> 16) & 255u) - 1);
         }
     }
-    // ---- one thread per cell root ----
+    // ---- one thread per cell root.  The 32 cell roots of a warp are consecutive in Z-order, so the lowest levels above
+    //      the cells are merged inside the warp first, by the same rounds as inside a cell (a segment that is a left child
+    //      merges with the segment starting right after it if that one is a right child), the state exchanged by
+    //      shuffles: about five levels fewer for the atomic walk, whose length is pure latency. ----
+    const int lane = threadIdx.x & 31;
+    const uint32_t FULL = 0xFFFFFFFFu;
     const int j = blockIdx.x * TOP_THREADS + threadIdx.x;
-    if (j >= cx.meta->ncell) return;
-    const uint32_t c = __ldg(cx.cell_list + j);
-    if (__ldg(cx.cell_start + c + 1) - __ldg(cx.cell_start + c) > (uint32_t)CELL_WARP_MAX) return;   // walked by the block that built it
-    const CellRoot r = cx.croot[j];
+    bool alive = false;
     Child me;
-    me.wlo = r.wlo & 0x7FFFFFFFu, me.whi = r.whi, me.f = r.first, me.l = r.last, me.pend = (r.wlo >> 31) != 0;
-    walk_up(cx, me, r.dL, r.dR, r.dnext);
+    me.wlo = me.whi = 0u, me.f = me.l = 0, me.pend = false;
+    int dL = -1, dR = -1, dnext = -1, t = 0;
+    uint32_t ki = 0;
+    if (j < cx.meta->ncell) {
+        const CellRoot r = cx.croot[j];
+        if (!(r.d & CELL_ROOT_BIG)) {                // a large cell is walked by the block that builds it (the bit says so whichever of the two wrote last)
+            me.wlo = r.wlo & 0x7FFFFFFFu, me.whi = r.whi, me.f = r.first, me.l = r.last, me.pend = (r.wlo >> 31) != 0;
+            dL = (int)(r.d & 255u) - 1, dR = (int)((r.d >> 8) & 255u) - 1, dnext = (int)((r.d >> 16) & 255u) - 1;
+            ki = r.key0;
+            t = (int)(ki >> 30);
+            alive = true;
+        }
+    }
+    const int s_seg = cx.meta->seg[t], gmax = cx.meta->gmax[t];
+    const int32_t *rb = cx.meta->rbin[t];
+    const uint32_t *key = cx.key_sorted;
+    auto keyat = [&](int k) { return key[k]; };
+    auto pfx = [&](int f, int l) { return delta_aug(key[f], f, key[l], l); };
+    int lastl = lane;                                // last lane of this lane's segment
+    int written = 0;
+    while (true) {
+        const int sc = min(lastl + 1, 31);           // head of the segment that starts right after mine
+        const int p_alive = __shfl_sync(FULL, (int)alive, sc), p_dL = __shfl_sync(FULL, dL, sc), p_dR = __shfl_sync(FULL, dR, sc);
+        const bool merge = alive && dR > dL && lastl < 31 && p_alive && !(p_dR > p_dL);
+        if (!__any_sync(FULL, merge)) break;
+        Child b;
+        b.wlo = __shfl_sync(FULL, me.wlo, sc), b.whi = __shfl_sync(FULL, me.whi, sc);
+        b.l = __shfl_sync(FULL, me.l, sc), b.pend = __shfl_sync(FULL, (int)me.pend, sc) != 0;
+        const int p_dnext = __shfl_sync(FULL, dnext, sc), p_lastl = __shfl_sync(FULL, lastl, sc);
+        const uint32_t kill = __reduce_or_sync(FULL, merge ? (1u << sc) : 0u);
+        if (merge) {
+            b.f = me.l + 1;
+            const int dsplit = dR;                   // delta(gamma, gamma+1): the parent's own prefix length
+            dR = p_dR, dnext = p_dnext, lastl = p_lastl;
+            const int rope_p = dR < 0 ? -1 : (dnext > dR ? b.l + 1 : cx.N + b.l);
+            uint32_t ulo, uhi;
+            int w = 0;
+            const bool pend = form_parent(cx, t, s_seg, gmax, rb, ki, keyat, me, b, dL, dR, dsplit, rope_p, pfx, ulo, uhi, w);
+            written += w;
+            me.wlo = ulo, me.whi = uhi, me.l = b.l, me.pend = pend;
+        }
+        if ((kill >> lane) & 1u) alive = false;
+    }
+    if (written) atomicAdd(&cx.meta->nodes_emitted, written);
+    if (alive) walk_up(cx, me, dL, dR, dnext);
 }
 
 // ------------------------------------------------------------------------------------------------------------

@@ -102,10 +102,17 @@ struct __align__(16) CellRoot {
     uint32_t whi;
     int32_t first;     // sorted positions covered
     int32_t last;
-    int32_t dL, dR;    // common prefix lengths with the neighbouring cells (-1 beyond the type segment)
-    int32_t dnext;     // delta(m, m+1) for m = last + 1: 64 if the next cell holds >= 2 particles, else its delta to the one after (-1: none)
-    int32_t pad;
+    uint32_t d;        // (dL+1) | (dR+1) << 8 | (dnext+1) << 16 | big << 31.  dL, dR: common prefix lengths with the
+                       // neighbouring cells (-1 beyond the type segment); dnext: delta(m, m+1) for m = last + 1 (64 if the
+                       // next cell holds >= 2 particles, else its delta to the one after, -1: none); big: a cell too large
+                       // for a warp, built and walked by a whole block of top_tree_kernel (set by cell_tree_kernel already)
+    uint32_t key0;     // key of the cell's first particle (type, entry-table cells)
+    uint32_t pad[2];
 };
+constexpr uint32_t CELL_ROOT_BIG = 1u << 31;
+__host__ __device__ inline uint32_t cell_root_d(int dL, int dR, int dnext, bool big) {
+    return (uint32_t)(dL + 1) | ((uint32_t)(dR + 1) << 8) | ((uint32_t)(dnext + 1) << 16) | (big ? CELL_ROOT_BIG : 0u);
+}
 
 // Z-ordered fp64 particle record of a double-precision build (qbvh_build_f64)
 struct __align__(32) Pos64 {
