@@ -396,6 +396,18 @@ __device__ __forceinline__ uint32_t quant_hi(float b, float lo, float delta, flo
     }
     return quant_hi_bisect(b, lo, delta);
 }
+// q_hi of the same value whose q_lo is known (a point: its box is one bin, Fig. 3c): the first guess is q_lo
+// itself or the bin line above it
+__device__ __forceinline__ uint32_t quant_hi_from_lo(float b, float lo, float delta, uint32_t qlo) {
+    int q = (int)qlo;
+    if (__fmaf_ru((float)q, delta, lo) >= b) {
+        if (q == 0 || __fmaf_ru((float)(q - 1), delta, lo) < b) return (uint32_t)q;
+    } else if (q < 1023) {
+        ++q;
+        if (__fmaf_ru((float)q, delta, lo) >= b) return (uint32_t)q;   // D_hi(q - 1) < b was just seen
+    }
+    return quant_hi_bisect(b, lo, delta);
+}
 __device__ __forceinline__ uint32_t pack_min(uint32_t a, uint32_t b) {
     return min(a & 0x3FFu, b & 0x3FFu) | min(a & 0xFFC00u, b & 0xFFC00u) | min(a & 0x3FF00000u, b & 0x3FF00000u);
 }
@@ -803,6 +815,8 @@ __device__ void process_cell(const TreeCtx &cx, const CellArrays A, int j, int r
         sort_cell<G>(A.kv, n, rank);
     }
     const float *fr = cx.meta->frames[t];
+    // collapse by size alone, query groups at least as large as the range leaves: the top-down path below
+    const bool by_size = G == 32 && cx.K > 1 && rb[0] < 0 && gmax >= cx.K;
     // ---- a2' gather, a6 quantize, leaf state ----
     for (int p = rank; p < n; p += G) {
         const unsigned long long kvp = A.kv[p];
@@ -823,13 +837,17 @@ __device__ void process_cell(const TreeCtx &cx, const CellArrays A, int j, int r
             x = pp[0], y = pp[1], z = pp[2];
         }
         cx.sorted_pos[k] = make_float4(x, y, z, __uint_as_float(idx));
-        const uint32_t wlo = quant_lo(x, fr[0], fr[6], fr[9]) | (quant_lo(y, fr[1], fr[7], fr[10]) << 10) | (quant_lo(z, fr[2], fr[8], fr[11]) << 20);
-        const uint32_t whi = quant_hi(x, fr[0], fr[6], fr[9]) | (quant_hi(y, fr[1], fr[7], fr[10]) << 10) | (quant_hi(z, fr[2], fr[8], fr[11]) << 20);
+        const uint32_t qx = quant_lo(x, fr[0], fr[6], fr[9]), qy = quant_lo(y, fr[1], fr[7], fr[10]), qz = quant_lo(z, fr[2], fr[8], fr[11]);
+        const uint32_t wlo = qx | (qy << 10) | (qz << 20);
+        const uint32_t whi = quant_hi_from_lo(x, fr[0], fr[6], qx) | (quant_hi_from_lo(y, fr[1], fr[7], qy) << 10) |
+                             (quant_hi_from_lo(z, fr[2], fr[8], qz) << 20);
         A.wlo[p] = wlo | 0x80000000u;                    // a single particle is pending
         A.whi[p] = whi;
-        A.e[p] = p;
-        A.dL[p] = (int8_t)(p > 0 ? delta_aug(ki, k, (uint32_t)(A.kv[p - 1] >> 32), k - 1) : dLc);
-        A.dR[p] = (int8_t)(p < n - 1 ? delta_aug(ki, k, (uint32_t)(A.kv[p + 1] >> 32), k + 1) : dRc);
+        if (!by_size) {                                  // segment state of the rounds
+            A.e[p] = p;
+            A.dL[p] = (int8_t)(p > 0 ? delta_aug(ki, k, (uint32_t)(A.kv[p - 1] >> 32), k - 1) : dLc);
+            A.dR[p] = (int8_t)(p < n - 1 ? delta_aug(ki, k, (uint32_t)(A.kv[p + 1] >> 32), k + 1) : dRc);
+        }
         if (k == e_seg && k < N - 1) {                   // no internal node carries the index of a segment end
             cx.nodes[k] = make_int4(0, 0, 0, -1);
             cx.parent[k] = -1;
@@ -848,7 +866,7 @@ __device__ void process_cell(const TreeCtx &cx, const CellArrays A, int j, int r
     };
     auto keyat = [&](int k) { return (uint32_t)(A.kv[k - F] >> 32); };
     auto pfx = [&](int f, int l) { return delta_aug(keyat(f), f, keyat(l), l); };
-    if (G == 32 && cx.K > 1 && rb[0] < 0 && gmax >= cx.K) {
+    if (by_size) {
         // (gmax >= K: query groups are unions of range leaves, so none has to be cut out of a leaf's inside)
         // ---- Collapse by size alone (no cost hint): a node is a range leaf iff it holds <= K particles, so only the
         //      nodes with more than K particles exist as internal nodes.  They are split top down — the split of a
