@@ -30,7 +30,8 @@ def gpu_run(w, K=4, max_neigh=None, stats=False, export=False, retry=False, hint
         out["frames"] = qbvh.qbvh_debug_export(qbvh.EXPORT_FRAMES, w.N)
         out["segments"] = qbvh.qbvh_debug_export(qbvh.EXPORT_SEGMENTS, w.N)
         out["sorted_pos"] = qbvh.qbvh_debug_export(qbvh.EXPORT_SORTED_POS, w.N)
-        out["nodes_emitted"] = int(qbvh.qbvh_debug_export(qbvh.EXPORT_COUNTS, w.N)[0])
+        out["counts"] = qbvh.qbvh_debug_export(qbvh.EXPORT_COUNTS, w.N)    # nodes written, query groups, cells, cell level
+        out["nodes_emitted"] = int(out["counts"][0])
     nl.n_neigh.fill_(-7)
     nl.nlist.fill_(-1)
     M = nl.neighbors(w.r_list, retry=retry)

@@ -633,3 +633,19 @@ def test_query_sharding_slices_merge_to_the_oracle(cid, world):
     rows, n_neigh, nlist, M = snl.neighbors(w.r_list)
     n1, l1 = sharded.merge_slices(w.N, [(rows.numpy(), n_neigh.cpu().numpy(), nlist.cpu().numpy())])
     assert np.array_equal(n1, n_all)
+
+
+@pytest.mark.parametrize("N,T,lvl", [(1, 1, 2), (3072, 1, 2), (3073, 1, 3), (200_000, 1, 5), (200_000, 4, 5), (1_600_000, 1, 6), (1_600_000, 2, 5)])
+def test_cell_grid_level_choice(N, T, lvl):
+    """The Morton-cell grid of the build: the smallest 2^lvl-per-axis grid with at most 48 particles per
+    cell on average, lvl in [2, 6], T * 8^lvl <= 2^18 — and the build is correct on every side of those thresholds
+    (counts against the oracle; the build products are compared bitwise in the other tests)."""
+    rng = np.random.default_rng(N + T)
+    L = max(4.0, (N / 0.85) ** (1 / 3))
+    pos, box = W._finish(rng.random((N, 3)) * L, L)
+    typ = None if T == 1 else rng.integers(0, T, N).astype(np.int32)
+    r = np.full((T, T), 1.3, np.float32)
+    w = W.Workload(f"lvl{N}_{T}", pos, typ, box, r, 40)
+    out = gpu_run(w, K=32, export=True)
+    assert int(out["counts"][3]) == lvl
+    compare_with_oracle(w, out, ON.neighbor_list(pos, typ, box, r), allow_overflow=True)
