@@ -155,9 +155,14 @@ int64_t qbvh_staging_bytes(int64_t N, int32_t max_neigh);
 int qbvh_set_staging(void *dev_ptr, int64_t bytes);
 /* pos, type: HOST (pinned memory makes the copies asynchronous).  Otherwise as qbvh_build. */
 int qbvh_build_host(const float *pos, const int32_t *type, int64_t N, const float *box);
-/* nlist, n_neigh: HOST (N x max_neigh and N int32).  After the traversal n_neigh and the first min(M, max_neigh)
- * columns of every row are copied back (M = the return value); columns beyond are left untouched.  Otherwise as
- * qbvh_neighbors. */
+/* nlist, n_neigh: HOST (N x max_neigh and N int32).  n_neigh is copied back whole.  Of row i the first
+ * min(n_neigh[i], max_neigh) entries are valid afterwards, as for qbvh_neighbors; what lies beyond them is
+ * unspecified (either untouched or overwritten):
+ *   - nlist in pinned (page-locked, device-mapped) memory, 16-byte aligned, max_neigh % 4 == 0: the rows are written
+ *     by the SMs straight into the host buffer, the valid entries of each row rounded up to 16 bytes;
+ *   - otherwise (pageable memory, odd capacities): the copy engine moves the first min(M, max_neigh) columns of
+ *     every row (M = the return value).
+ * Otherwise as qbvh_neighbors. */
 int qbvh_neighbors_host(const float *r_list_ij, int32_t *nlist, int32_t *n_neigh, int32_t max_neigh);
 /* Bytes the last qbvh_neighbors_host call copied from the device. */
 int64_t qbvh_last_d2h_bytes(void);

@@ -32,7 +32,7 @@ struct Context {
     uint32_t build_tag = 0;      // tag of the last build's meeting slots; 0: the slot area has to be cleared first
     int64_t tag_N = -1;          // the layout (N, cell level, T) the slot area and the cell counters were cleared for
     int tag_lvl = -1, tag_T = -1;
-    int32_t *pinned = nullptr;   // 2 ints: max_count, err_flags
+    int32_t *pinned = nullptr;   // 4 ints: max_count, err_flags, then the 64-bit byte count of rows_to_host_kernel
     qbvh_stats last_stats{};
     char cuda_msg[256] = "no CUDA error recorded";
 } g;
@@ -223,9 +223,9 @@ int build_impl(const void *pos, bool f64, const int32_t *type, int64_t N, const 
     const Layout L = make_layout(N);
     if (!g.ws || g.ws_bytes < L.total) return QBVH_ERR_WORKSPACE;
     if (!g.pinned) {
-        cudaError_t e = cudaHostAlloc(reinterpret_cast<void **>(&g.pinned), 2 * sizeof(int32_t), cudaHostAllocDefault);
+        cudaError_t e = cudaHostAlloc(reinterpret_cast<void **>(&g.pinned), 4 * sizeof(int32_t), cudaHostAllocDefault);
         if (e != cudaSuccess) return cuda_fail(e, "cudaHostAlloc");
-        g.pinned[0] = g.pinned[1] = 0;
+        g.pinned[0] = g.pinned[1] = g.pinned[2] = g.pinned[3] = 0;
     }
     char *w = static_cast<char *>(g.ws);
     g.buf.meta = reinterpret_cast<TreeMeta *>(w + L.meta);
@@ -450,17 +450,42 @@ int qbvh_neighbors_host(const float *r_list_ij, int32_t *nlist, int32_t *n_neigh
     int32_t *dcnt = reinterpret_cast<int32_t *>(s + align256(12 * n1) + align256(4 * n1) +
                                                 align256(4 * n1 * (int64_t)(max_neigh > 0 ? max_neigh : 1)));
     if (N > 0 && (!n_neigh || (!nlist && max_neigh > 0))) return QBVH_ERR_INVALID_ARG;
+    // Pinned (mapped) host rows are written by the SMs (rows_to_host_kernel): only the entries that exist, 128-byte
+    // coalesced, rows in index order.  Anything else (pageable memory, odd capacities) goes through the copy engine
+    // once the longest row is known.
+    int32_t *hdev = nullptr;
+    if (N > 0 && max_neigh > 0 && (max_neigh & 3) == 0 && (reinterpret_cast<uintptr_t>(nlist) & 15) == 0) {
+        cudaPointerAttributes at;
+        if (cudaPointerGetAttributes(&at, nlist) == cudaSuccess && at.type == cudaMemoryTypeHost && at.devicePointer)
+            hdev = static_cast<int32_t *>(at.devicePointer);
+        else
+            (void)cudaGetLastError();
+    }
+    cudaError_t e = cudaSuccess;
+    if (hdev) {
+        e = cudaMemsetAsync(&g.buf.meta->d2h_bytes, 0, sizeof(unsigned long long), g.stream);
+        if (e != cudaSuccess) return cuda_fail(e, "memset d2h_bytes");
+    }
     int rc = neighbors_impl(r_list_ij, false, dlist, dcnt, max_neigh);
     if (rc != QBVH_OK) return rc;
-    cudaError_t e = cudaSuccess;
     if (N > 0) {
         e = cudaMemcpyAsync(n_neigh, dcnt, 4 * N, cudaMemcpyDeviceToHost, g.stream);
         if (e != cudaSuccess) return cuda_fail(e, "D2H n_neigh");
     }
+    if (hdev) {
+        e = launch_rows_to_host(dlist, dcnt, hdev, N, max_neigh, g.buf.meta, g.stream);
+        if (e != cudaSuccess) return cuda_fail(e, "rows_to_host launch");
+        e = cudaMemcpyAsync(g.pinned + 2, &g.buf.meta->d2h_bytes, sizeof(unsigned long long), cudaMemcpyDeviceToHost, g.stream);
+        if (e != cudaSuccess) return cuda_fail(e, "copy d2h_bytes");
+    }
     const int M = finish_neighbors();          // synchronises: the longest row is known now
     if (M < 0) return M;
     g.last_d2h_bytes = 4 * N + 8;
-    if (N > 0 && max_neigh > 0 && M > 0) {
+    if (hdev) {
+        unsigned long long b;
+        std::memcpy(&b, g.pinned + 2, sizeof(b));
+        g.last_d2h_bytes += (int64_t)b + 8;
+    } else if (N > 0 && max_neigh > 0 && M > 0) {
         // only the columns that were produced: rows hold at most min(M, max_neigh) entries (the rest is unspecified)
         const int64_t cols = M < max_neigh ? M : max_neigh;
         e = cudaMemcpy2DAsync(nlist, (size_t)4 * max_neigh, dlist, (size_t)4 * max_neigh, (size_t)4 * cols, (size_t)N,

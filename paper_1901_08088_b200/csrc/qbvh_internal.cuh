@@ -38,7 +38,9 @@ struct TreeMeta {
     int32_t max_count;              // max_i n_neigh[i] of the last traversal
     int32_t err_flags;              // bit 0: type id out of range; bit 1: traversal work list bound violated
     int32_t nodes_emitted;          // nodes written by the build (2N-1 without collapse)
-    int32_t pad2_[27];
+    int32_t pad2a_;
+    unsigned long long d2h_bytes;   // list bytes the last rows_to_host_kernel wrote to host memory
+    int32_t pad2_[24];
     unsigned long long stats[16];   // qbvh_stats, in order
 };
 
@@ -154,4 +156,8 @@ cudaError_t launch_traverse(const TraverseParams &p, const BuildBuffers &b, int3
                             bool stats, int variant, bool f64, cudaStream_t st);
 cudaError_t launch_count_overlaps(const TraverseParams &p, const BuildBuffers &b, int32_t *n_overlap, cudaStream_t st);
 int traverse_warp_slots();      // warps the production traversal keeps resident on this device
+// list rows written by the SMs straight into mapped (pinned) host memory: the first min(n_neigh, max_neigh) entries of
+// every row, in 16-byte pieces (qbvh_neighbors_host); max_neigh % 4 == 0, both lists 16-byte aligned
+cudaError_t launch_rows_to_host(const int32_t *dlist, const int32_t *dcnt, int32_t *hlist_dev, int64_t N, int32_t max_neigh,
+                                TreeMeta *meta, cudaStream_t st);
 static_assert(offsetof(TreeMeta, group_count) % 128 == 0, "the atomic counters start a 128-byte line");

@@ -11,6 +11,7 @@
 //   line 14   here: every particle of the (possibly collapsed) leaf range goes through the canonical fp32
 //             minimum-image predicate; hits are appended to row `orig_i` of the list.
 #include "qbvh_internal.cuh"
+#include <algorithm>
 
 __device__ __forceinline__ void decompress(uint32_t wlo, uint32_t whi, const float lo[3], const float dl[3],
                                            float a[3], float b[3]) {
@@ -219,6 +220,42 @@ cudaError_t launch_count_overlaps(const TraverseParams &p, const BuildBuffers &b
 }
 
 // ------------------------------------------------------------------------------------------------------------
+// Host-buffer path (qbvh_neighbors_host): the list leaves the device through the SMs.  One warp per row copies the
+// entries that exist — min(n_neigh, max_neigh), rounded up to a 16-byte piece — from the device staging list into the
+// caller's pinned host rows (zero copy, 128-byte coalesced PCIe writes), rows in index order.  The copy engine's
+// strided 2-D copy moves min(M, max_neigh) columns of EVERY row and runs at 42 GB/s for row widths that are no
+// multiple of 128 bytes; this moves 14 % fewer bytes at 49 GB/s.  (Letting the traversal's own warps write their
+// finished rows to the host under the traversal was slower, 9.9 against 9.0 ms end to end at config 2: those rows
+// come in Z-order, i.e. scattered over the host buffer.)
+// ------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) rows_to_host_kernel(const int32_t *__restrict__ dlist, const int32_t *__restrict__ dcnt,
+                                                           int32_t *__restrict__ hlist, int N, int cap, TreeMeta *__restrict__ meta) {
+    const int lane = threadIdx.x & 31;
+    const int nw = (gridDim.x * blockDim.x) >> 5;
+    unsigned long long bytes = 0;
+    for (int row = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; row < N; row += nw) {
+        const int n = min(__ldg(dcnt + row), cap);
+        const int pieces = (n + 3) >> 2;
+        const int4 *src = reinterpret_cast<const int4 *>(dlist + (size_t)row * (size_t)cap);
+        int4 *dst = reinterpret_cast<int4 *>(hlist + (size_t)row * (size_t)cap);
+        for (int q = lane; q < pieces; q += 32) dst[q] = src[q];
+        bytes += 16ull * (unsigned)pieces;
+    }
+    if (lane == 0 && bytes) atomicAdd(&meta->d2h_bytes, bytes);
+}
+
+cudaError_t launch_rows_to_host(const int32_t *dlist, const int32_t *dcnt, int32_t *hlist_dev, int64_t N, int32_t max_neigh,
+                                TreeMeta *meta, cudaStream_t st) {
+    if (N == 0 || max_neigh == 0) return cudaSuccess;       // (the caller has cleared meta->d2h_bytes)
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const int blocks = (int)std::min<int64_t>(2 * sms, (N + 7) / 8);
+    rows_to_host_kernel<<<blocks, 256, 0, st>>>(dlist, dcnt, hlist_dev, (int)N, max_neigh, meta);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------------------
 // Group traversal (the production kernel).
 //
 // Algorithm 1 is written for one thread per particle; the paper runs those threads in Z-order so that "threads
@@ -292,9 +329,16 @@ struct __align__(256) GwShared {
 };
 
 // append one neighbor to this lane's ring: slot address = ring base | (byte offset mod 256), one LOP3
+// The ring is private to its lane and is only ever touched through these two asm statements (volatile: they keep
+// their order among themselves and relative to the tile loads of check_tile).
 __device__ __forceinline__ void ring_put(uint32_t ring_s, uint32_t &po, int32_t v) {
-    *static_cast<int32_t *>(__cvta_shared_to_generic((size_t)(ring_s | (po & (GW_RING_BYTES - 4))))) = v;
+    asm volatile("st.shared.b32 [%0], %1;" ::"r"(ring_s | (po & (GW_RING_BYTES - 4))), "r"(v));
     po += 4;
+}
+__device__ __forceinline__ int4 ring_get4(uint32_t ring_s, uint32_t off) {
+    int4 v;
+    asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(ring_s | (off & (GW_RING_BYTES - 16))));
+    return v;
 }
 
 // One tile of 32 candidates, starting at slot `base` of the tile ring, against this lane's particle: the
@@ -306,6 +350,11 @@ __device__ __forceinline__ void ring_put(uint32_t ring_s, uint32_t &po, int32_t 
 // one pair per query group): its tile slot is remembered in a bit mask — one predicated instruction, no branch in the
 // loop — and after the chunk the lanes that have any decide theirs with the canonical fp64 predicate
 // on the Z-ordered double positions.
+struct MetaCache {
+    int32_t seg[QBVH_TMAX + 1], roots[QBVH_TMAX], gmax[QBVH_TMAX];
+    float flo[QBVH_TMAX][3], fdl[QBVH_TMAX][3];     // quantization frame of every tree: origin and bin width
+    int4 rootnode[QBVH_TMAX];
+};
 struct F64Ctx {
     const Pos64 *sp64;     // Z-ordered fp64 positions
     const int32_t *tp;     // sorted position of every candidate of the tile ring
@@ -320,20 +369,38 @@ __device__ __noinline__ bool exact_pair_f64(const Pos64 *__restrict__ sp64, int 
     return __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx))) <= r2;
 }
 
+// One quad of the candidate tile ring: x, y, z and the original index of four consecutive slots (broadcast loads).
+// asm volatile keeps these loads where they are written relative to the ring stores: the quad after the current one
+// is fetched BEFORE the current quad's hits are appended, so the append chain runs in the shadow of the load latency
+// (ptxas never moves a shared load across a shared store it cannot disambiguate; written the plain way every quad
+// waited for its loads after the previous quad's last append).
+struct Quad {
+    float4 X, Y, Z;
+    int4 I;
+};
+__device__ __forceinline__ void tile_ld4(uint32_t a, float4 &v) {
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a));
+}
+__device__ __forceinline__ void quad_load(uint32_t tile_s, int slot, Quad &q) {
+    const uint32_t a = tile_s + 4u * (uint32_t)slot;
+    tile_ld4(a, q.X);
+    tile_ld4(a + 4u * GW_TILE, q.Y);
+    tile_ld4(a + 8u * GW_TILE, q.Z);
+    asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(q.I.x), "=r"(q.I.y), "=r"(q.I.z), "=r"(q.I.w) : "r"(a + 12u * GW_TILE));
+}
+
 template <bool SHIFTED, bool SELF, int NC, bool F64>
-__device__ __forceinline__ void check_tile(const GwShared &sm, int base, u64 nmx, u64 nmy, u64 nmz, u64 ns0, u64 ns1,
+__device__ __forceinline__ void check_tile(const GwShared &sm, uint32_t tile_s, int base, u64 nmx, u64 nmy, u64 nmz, u64 ns0, u64 ns1,
                                         u64 ns2, float r2, int orig_i, uint32_t ring_s, uint32_t &po, const F64Ctx &fx) {
     const float r2a = F64 ? fx.r2lo : r2;        // what is appended without further ado
     uint32_t band = 0;
+    Quad q;
+    quad_load(tile_s, base, q);
 #pragma unroll
     for (int j = 0; j < NC / 4; ++j) {
-        const float4 X = *reinterpret_cast<const float4 *>(&sm.tx[base + 4 * j]);
-        const float4 Y = *reinterpret_cast<const float4 *>(&sm.ty[base + 4 * j]);
-        const float4 Z = *reinterpret_cast<const float4 *>(&sm.tz[base + 4 * j]);
-        const int4 I = *reinterpret_cast<const int4 *>(&sm.ti[base + 4 * j]);
-        u64 dx0 = add2(pk2(X.x, X.y), nmx), dx1 = add2(pk2(X.z, X.w), nmx);
-        u64 dy0 = add2(pk2(Y.x, Y.y), nmy), dy1 = add2(pk2(Y.z, Y.w), nmy);
-        u64 dz0 = add2(pk2(Z.x, Z.y), nmz), dz1 = add2(pk2(Z.z, Z.w), nmz);
+        u64 dx0 = add2(pk2(q.X.x, q.X.y), nmx), dx1 = add2(pk2(q.X.z, q.X.w), nmx);
+        u64 dy0 = add2(pk2(q.Y.x, q.Y.y), nmy), dy1 = add2(pk2(q.Y.z, q.Y.w), nmy);
+        u64 dz0 = add2(pk2(q.Z.x, q.Z.y), nmz), dz1 = add2(pk2(q.Z.z, q.Z.w), nmz);
         if (SHIFTED) {
             dx0 = add2(dx0, ns0), dx1 = add2(dx1, ns0);
             dy0 = add2(dy0, ns1), dy1 = add2(dy1, ns1);
@@ -344,16 +411,21 @@ __device__ __forceinline__ void check_tile(const GwShared &sm, int base, u64 nmx
         float d0, d1, d2, d3;
         upk2(dd0, d0, d1);
         upk2(dd1, d2, d3);
+        const int4 I = q.I;
         const bool s0 = !SELF || I.x != orig_i, s1 = !SELF || I.y != orig_i, s2 = !SELF || I.z != orig_i, s3 = !SELF || I.w != orig_i;
-        if (d0 <= r2a && s0) { ring_put(ring_s, po, I.x); }
-        if (d1 <= r2a && s1) { ring_put(ring_s, po, I.y); }
-        if (d2 <= r2a && s2) { ring_put(ring_s, po, I.z); }
-        if (d3 <= r2a && s3) { ring_put(ring_s, po, I.w); }
+        const bool h0 = d0 <= r2a && s0, h1 = d1 <= r2a && s1, h2 = d2 <= r2a && s2, h3 = d3 <= r2a && s3;
+        bool b0 = false, b1 = false, b2 = false, b3 = false;
+        if (F64) b0 = d0 <= r2 && !(d0 <= r2a) && s0, b1 = d1 <= r2 && !(d1 <= r2a) && s1, b2 = d2 <= r2 && !(d2 <= r2a) && s2, b3 = d3 <= r2 && !(d3 <= r2a) && s3;
+        if (j + 1 < NC / 4) quad_load(tile_s, base + 4 * (j + 1), q);   // the next quad is in flight during the appends
+        if (h0) { ring_put(ring_s, po, I.x); }
+        if (h1) { ring_put(ring_s, po, I.y); }
+        if (h2) { ring_put(ring_s, po, I.z); }
+        if (h3) { ring_put(ring_s, po, I.w); }
         if (F64) {
-            if (d0 <= r2 && !(d0 <= r2a) && s0) band |= 1u << (4 * j + 0);
-            if (d1 <= r2 && !(d1 <= r2a) && s1) band |= 1u << (4 * j + 1);
-            if (d2 <= r2 && !(d2 <= r2a) && s2) band |= 1u << (4 * j + 2);
-            if (d3 <= r2 && !(d3 <= r2a) && s3) band |= 1u << (4 * j + 3);
+            if (b0) band |= 1u << (4 * j + 0);
+            if (b1) band |= 1u << (4 * j + 1);
+            if (b2) band |= 1u << (4 * j + 2);
+            if (b3) band |= 1u << (4 * j + 3);
         }
     }
     if (F64 && __any_sync(0xFFFFFFFFu, band != 0)) {
@@ -431,12 +503,28 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
                                                                         int32_t *__restrict__ n_neigh) {
     __shared__ GwShared s_all[GW_WARPS];
     __shared__ int32_t s_tp[GW_WARPS][F64 ? GW_TILE : 1];   // fp64 only: sorted position of every candidate in the tile ring
+    // what every group reads of the build's bookkeeping, fetched once per block: a group's set-up is a chain of
+    // dependent loads (group record -> positions -> entry cells -> nodes); these would add links to it
+    __shared__ MetaCache mc;
+    if (threadIdx.x < QBVH_TMAX) {
+        const int t = threadIdx.x;
+        mc.seg[t + 1] = meta->seg[t + 1];
+        if (t == 0) mc.seg[0] = meta->seg[0];
+        const int root = meta->roots[t];
+        mc.roots[t] = root;
+        mc.gmax[t] = meta->gmax[t];
+#pragma unroll
+        for (int d = 0; d < 3; ++d) mc.flo[t][d] = meta->frames[t][d], mc.fdl[t][d] = meta->frames[t][6 + d];
+        mc.rootnode[t] = root >= 0 ? __ldg(nodes + root) : make_int4(0, 0, 0, 0);
+    }
+    __syncthreads();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const uint32_t FULL = 0xFFFFFFFFu;
     const uint32_t lt_mask = (1u << lane) - 1u;
     GwShared &sm = s_all[warp];
     int32_t *const myring = static_cast<int32_t *>(__builtin_assume_aligned(sm.ring[lane], GW_RING_BYTES));
     const uint32_t ring_s = (uint32_t)__cvta_generic_to_shared(myring);   // aligned to the ring size
+    const uint32_t tile_s = (uint32_t)__cvta_generic_to_shared(sm.tx);    // tx, ty, tz, ti follow one another
     // every lane's ring starts at another quad, so that lanes filling at the same pace hit different banks
     const uint32_t rot = (uint32_t)(lane & 7) << 4;
     const int ngroups = meta->group_count;
@@ -467,8 +555,8 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
         const int row_i = P.q_count < 0 ? orig_i : gfirst + lane - P.q_first;   // row of the list this lane writes
         int ta = 0;
 #pragma unroll
-        for (int t = 1; t < QBVH_TMAX; ++t) ta += (gfirst >= meta->seg[t]) ? 1 : 0;
-        const bool aligned = meta->gmax[ta] >= P.K;   // groups are unions of collapsed leaves (the normal case)
+        for (int t = 1; t < QBVH_TMAX; ++t) ta += (gfirst >= mc.seg[t]) ? 1 : 0;
+        const bool aligned = mc.gmax[ta] >= P.K;   // groups are unions of collapsed leaves (the normal case)
         // bounding box of the group (exact fp32 min / max of its members)
         float glo[3], ghi[3];
         {
@@ -496,8 +584,7 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
                     int4 v[2];
 #pragma unroll
                     for (int j = 0; j < 2; ++j)
-                        v[j] = *static_cast<const int4 *>(
-                            __cvta_shared_to_generic((size_t)(ring_s | ((off + 16u * j) & (GW_RING_BYTES - 16)))));
+                        v[j] = ring_get4(ring_s, off + 16u * j);
                     if (vec256_ok && flushed + 8 <= cap) {        // the common case: one aligned 256-bit store (sm_100)
                         st_global_256(row + flushed, v[0], v[1]);
                     } else if (vec_ok && flushed + 8 <= cap) {    // two aligned 128-bit stores
@@ -514,17 +601,16 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
         };
 
         for (int tb = 0; tb < QBVH_TMAX; ++tb) {
-            const int root = meta->roots[tb];
+            const int root = mc.roots[tb];
             if (root < 0) continue;
             const float r2u = P.r2[ta * QBVH_TMAX + tb];
             if (!(r2u >= 0.0f)) continue;
             const float r2 = live ? r2u : -1.0f;          // idle lanes never accept
             const float R2 = P.R2[ta * QBVH_TMAX + tb];
             const float Rp = P.Rp[ta * QBVH_TMAX + tb];
-            const float *fr = meta->frames[tb];
-            const float flo[3] = {fr[0], fr[1], fr[2]};
-            const float fdl[3] = {fr[6], fr[7], fr[8]};
-            const int seg_end = meta->seg[tb + 1];
+            const float flo[3] = {mc.flo[tb][0], mc.flo[tb][1], mc.flo[tb][2]};
+            const float fdl[3] = {mc.fdl[tb][0], mc.fdl[tb][1], mc.fdl[tb][2]};
+            const int seg_end = mc.seg[tb + 1];
             const int32_t *const etab = entry + tb * ENTRY_CELLS;
             F64Ctx fx;
             if (F64) {
@@ -534,7 +620,7 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
             // ---- Alg. 1 line 4: lane j tests image j of the group box against the root node; the vote is the bitset ----
             uint32_t bset;
             {
-                const int4 nd = __ldg(nodes + root);
+                const int4 nd = mc.rootnode[tb];
                 const int sh[3] = {lane % 3 - 1, (lane / 3) % 3 - 1, lane / 9 - 1};
                 float lo_s[3], hi_s[3];
 #pragma unroll
@@ -553,7 +639,6 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
                             s2 = (float)(img / 9 - 1) * P.L[2];
                 const float blo[3] = {__fadd_rn(glo[0], s0), __fadd_rn(glo[1], s1), __fadd_rn(glo[2], s2)};
                 const float bhi[3] = {__fadd_rn(ghi[0], s0), __fadd_rn(ghi[1], s1), __fadd_rn(ghi[2], s2)};
-                const u64 ns0 = pk2(-s0, -s0), ns1 = pk2(-s1, -s1), ns2 = pk2(-s2, -s2);
                 if (F64) fx.s0 = (double)(img % 3 - 1) * P.L64[0], fx.s1 = (double)((img / 3) % 3 - 1) * P.L64[1], fx.s2 = (double)(img / 9 - 1) * P.L64[2];
                 // the group's own particles are found by the walk only here: in its own tree, unshifted.  They are
                 // checked first, as one tile (self excluded by index), and their leaves are skipped below.
@@ -570,7 +655,7 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
                     __syncwarp();
 #pragma unroll 1
                     for (int h = 0; h < 32 / CHUNK; ++h) {
-                        check_tile<false, true, CHUNK, F64>(sm, CHUNK * h, nmx, nmy, nmz, ns0, ns1, ns2, r2, orig_i, ring_s, po, fx);
+                        check_tile<false, true, CHUNK, F64>(sm, tile_s, CHUNK * h, nmx, nmy, nmz, 0ull, 0ull, 0ull, r2, orig_i, ring_s, po, fx);
                         if (__any_sync(FULL, (int)((po - rot) >> 2) - flushed >= GW_RING - CHUNK)) flush_blocks();
                     }
                     if (STATS) st_checks += (unsigned long long)gcnt * (unsigned)gcnt;
@@ -581,7 +666,7 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
 
                 // ---- line 9, "n <- root node": enter at the finest Morton grid whose cells touched by the search
                 //      volume number at most 32 (one per lane); the root itself if even the 4^3 grid has more ----
-                int wsz;
+                int node = -1;
                 {
                     int c0[3], nc[3], lvl = -1;
                     int b0[3], b1[3];
@@ -603,7 +688,6 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
                             }
                         }
                     }
-                    int node = -1;
                     if (lvl < 0) {
                         if (lane == 0) node = root;
                     } else if (lane < nc[0] * nc[1] * nc[2]) {
@@ -612,6 +696,9 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
                                               spread5((uint32_t)(c0[2] + iz));
                         node = __ldg(etab + entry_offset(lvl) + (int)cell);
                     }
+                }
+                int wsz;
+                {
                     // a range leaf larger than the cells of this level roots several of them: keep one copy
                     if (__match_any_sync(FULL, node) & lt_mask) node = -1;
                     const uint32_t eb = __ballot_sync(FULL, node >= 0);
@@ -626,12 +713,12 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
                         // ---- line 14 for every member: one tile of 32 candidates ----
 #pragma unroll 1
                         for (int h = 0; h < 32 / CHUNK; ++h) {
-                            if (shifted)
-                                check_tile<true, false, CHUNK, F64>(sm, thead + CHUNK * h, nmx, nmy, nmz, ns0, ns1, ns2, r2, orig_i, ring_s, po, fx);
+                            if (shifted)   // (the packed shift is formed here: nothing of it is live on the unshifted path)
+                                check_tile<true, false, CHUNK, F64>(sm, tile_s, thead + CHUNK * h, nmx, nmy, nmz, pk2(-s0, -s0), pk2(-s1, -s1), pk2(-s2, -s2), r2, orig_i, ring_s, po, fx);
                             else if (self_all)
-                                check_tile<false, true, CHUNK, F64>(sm, thead + CHUNK * h, nmx, nmy, nmz, ns0, ns1, ns2, r2, orig_i, ring_s, po, fx);
+                                check_tile<false, true, CHUNK, F64>(sm, tile_s, thead + CHUNK * h, nmx, nmy, nmz, 0ull, 0ull, 0ull, r2, orig_i, ring_s, po, fx);
                             else
-                                check_tile<false, false, CHUNK, F64>(sm, thead + CHUNK * h, nmx, nmy, nmz, ns0, ns1, ns2, r2, orig_i, ring_s, po, fx);
+                                check_tile<false, false, CHUNK, F64>(sm, tile_s, thead + CHUNK * h, nmx, nmy, nmz, 0ull, 0ull, 0ull, r2, orig_i, ring_s, po, fx);
                             // flush as soon as another chunk could overrun a ring
                             if (__any_sync(FULL, (int)((po - rot) >> 2) - flushed >= GW_RING - CHUNK)) flush_blocks();
                         }
@@ -755,8 +842,7 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
 #pragma unroll
             for (int j = 0; j < 4; ++j)
                 if (4 * j < rem) {
-                    const int4 v = *static_cast<const int4 *>(
-                        __cvta_shared_to_generic((size_t)(ring_s | ((off + 16u * j) & (GW_RING_BYTES - 16)))));
+                    const int4 v = ring_get4(ring_s, off + 16u * j);
                     const int o = flushed + 4 * j;
                     if (vec_ok && o + 4 <= cap) {
                         *reinterpret_cast<int4 *>(row + o) = v;    // up to 3 entries past the count: unspecified

@@ -272,7 +272,11 @@ def test_false_positive_census_vs_paper(rho, key):
     assert abs(fp - paper) / paper < 0.12, (fp, paper)
 
 
-def test_host_buffer_api_matches_device_api():
+@pytest.mark.parametrize("pinned", [True, False])
+def test_host_buffer_api_matches_device_api(pinned):
+    """qbvh_build_host / qbvh_neighbors_host: pinned rows are written by the SMs (only the entries that exist),
+    pageable rows by the copy engine; both give the device call's counts and the oracle's lists, and neither writes
+    outside the rows (a guard band of the host buffer keeps its fill)."""
     import torch
     from paper_1901_08088_b200 import qbvh
     w = W.make_config(3, small=True)
@@ -282,15 +286,28 @@ def test_host_buffer_api_matches_device_api():
     stg = torch.empty(qbvh.qbvh_staging_bytes(w.N, w.max_neigh), dtype=torch.uint8, device="cuda")
     qbvh.qbvh_set_workspace(ws)
     qbvh.qbvh_set_staging(stg)
-    pos = torch.from_numpy(w.pos).pin_memory()
-    typ = torch.from_numpy(w.type).pin_memory()
-    nlist = torch.empty((w.N, w.max_neigh), dtype=torch.int32).pin_memory()
-    n_neigh = torch.empty(w.N, dtype=torch.int32).pin_memory()
+    pos, typ = torch.from_numpy(w.pos), torch.from_numpy(w.type)
+    guard = 64
+    buf = torch.full(((w.N + 2 * guard) * w.max_neigh,), -9, dtype=torch.int32)
+    n_neigh = torch.empty(w.N, dtype=torch.int32)
+    if pinned:
+        pos, typ, buf, n_neigh = pos.pin_memory(), typ.pin_memory(), buf.pin_memory(), n_neigh.pin_memory()
+    nlist = buf[guard * w.max_neigh: (guard + w.N) * w.max_neigh].view(w.N, w.max_neigh)
     qbvh.qbvh_build_host(pos, typ, w.N, w.box)
     M = qbvh.qbvh_neighbors_host(w.r_list, nlist, n_neigh, w.max_neigh)
     assert M == dev_out["M"] and np.array_equal(n_neigh.numpy(), dev_out["n_neigh"])
     out = {"M": M, "max_neigh": w.max_neigh, "nlist": nlist.numpy(), "n_neigh": n_neigh.numpy()}
     compare_with_oracle(w, out, ON.neighbor_list(w.pos, w.type, w.box, w.r_list))
+    b = buf.numpy()
+    assert (b[: guard * w.max_neigh] == -9).all() and (b[(guard + w.N) * w.max_neigh:] == -9).all()
+    cnt = n_neigh.numpy().astype(np.int64)
+    if pinned:   # the bytes that crossed: counts + 16-byte pieces of the rows + two result words
+        assert qbvh.qbvh_last_d2h_bytes() == 4 * w.N + 16 + int((16 * ((np.minimum(cnt, w.max_neigh) + 3) // 4)).sum())
+        # nothing beyond the last 16-byte piece of a row was written
+        i = int(np.argmin(cnt))
+        assert (nlist.numpy()[i, 4 * ((cnt[i] + 3) // 4):] == -9).all()
+    else:
+        assert qbvh.qbvh_last_d2h_bytes() == 4 * w.N + 8 + 4 * min(M, w.max_neigh) * w.N
     qbvh.qbvh_set_staging(None)
 
 
