@@ -576,24 +576,32 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
 
         // Lanes write their complete 32-byte blocks (one sector, one 256-bit store) of staged neighbors to their list
         // rows.  Called when SOME lane runs out of ring space; EVERY lane with a complete block joins in, so the lanes
-        // stay in step and a visit serves most of them (a visit per lane and block cost 3x the instructions).
+        // stay in step and a visit serves most of them (a visit per lane and block cost 3x the instructions).  The lane
+        // that triggered the visit holds two blocks, most others one: both leave in the same straight-line pass; what
+        // is left after it (a third block, a row at its capacity, an unaligned list) takes the general loop.
         auto flush_blocks = [&]() {
+            if (vec256_ok) {
+#pragma unroll
+                for (int b = 0; b < 2; ++b) {
+                    if ((int)((po - rot) >> 2) - flushed >= 8 && flushed + 8 <= cap) {
+                        const uint32_t off = rot + 4u * (uint32_t)flushed;
+                        const int4 v0 = ring_get4(ring_s, off), v1 = ring_get4(ring_s, off + 16u);
+                        st_global_256(row + flushed, v0, v1);
+                        flushed += 8;
+                    }
+                }
+            }
             while (__any_sync(FULL, (int)((po - rot) >> 2) - flushed >= 8)) {
                 if ((int)((po - rot) >> 2) - flushed >= 8) {
                     const uint32_t off = rot + 4u * (uint32_t)flushed;
-                    int4 v[2];
-#pragma unroll
-                    for (int j = 0; j < 2; ++j)
-                        v[j] = ring_get4(ring_s, off + 16u * j);
-                    if (vec256_ok && flushed + 8 <= cap) {        // the common case: one aligned 256-bit store (sm_100)
-                        st_global_256(row + flushed, v[0], v[1]);
-                    } else if (vec_ok && flushed + 8 <= cap) {    // two aligned 128-bit stores
+                    const int4 v0 = ring_get4(ring_s, off), v1 = ring_get4(ring_s, off + 16u);
+                    if (vec_ok && flushed + 8 <= cap) {           // two aligned 128-bit stores
                         int4 *dst = reinterpret_cast<int4 *>(row + flushed);
-                        dst[0] = v[0];
-                        dst[1] = v[1];
+                        dst[0] = v0;
+                        dst[1] = v1;
                     } else {
-                        store4(row, flushed, cap, false, v[0]);
-                        store4(row, flushed + 4, cap, false, v[1]);
+                        store4(row, flushed, cap, false, v0);
+                        store4(row, flushed + 4, cap, false, v1);
                     }
                     flushed += 8;
                 }
@@ -691,7 +699,11 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
                     if (lvl < 0) {
                         if (lane == 0) node = root;
                     } else if (lane < nc[0] * nc[1] * nc[2]) {
-                        const int ix = lane % nc[0], iy = (lane / nc[0]) % nc[1], iz = lane / (nc[0] * nc[1]);
+                        // lane -> (ix, iy, iz); quotients of integers below 32 through a float reciprocal (exact: the
+                        // true quotient of lane + 0.5 is at least 1/64 away from an integer)
+                        const int qy = (int)(((float)lane + 0.5f) * __frcp_rn((float)nc[0]));           // lane / nc0
+                        const int iz = (int)(((float)qy + 0.5f) * __frcp_rn((float)nc[1]));             // lane / (nc0 nc1)
+                        const int ix = lane - qy * nc[0], iy = qy - iz * nc[1];
                         const uint32_t cell = (spread5((uint32_t)(c0[0] + ix)) << 2) | (spread5((uint32_t)(c0[1] + iy)) << 1) |
                                               spread5((uint32_t)(c0[2] + iz));
                         node = __ldg(etab + entry_offset(lvl) + (int)cell);
