@@ -200,8 +200,16 @@ def run_gpu(args):
         ev[s][0].record()
         nl.build(pos, typ, box)
         ev[s][1].record()
-        nl.neighbors(r_list, retry=False)
-        ev[s][2].record()
+        if f64:
+            nl.neighbors(r_list, retry=False)          # (the fp64 call has no enqueue form: its event follows the wait)
+            ev[s][2].record()
+        else:
+            # the traversal is enqueued, the closing event recorded behind it on the stream, and only then does the
+            # host wait for M: the events bracket the device work, not the host's wake-up after the synchronise
+            nl.neighbors_enqueue(r_list)
+            ev[s][2].record()
+            if nl.neighbors_result() > cap:
+                raise SystemExit("overflow inside the timed loop")
     torch.cuda.synchronize()
     wall = time.perf_counter() - wall0
     if world > 1:

@@ -116,6 +116,18 @@ int qbvh_build(const float *pos, const int32_t *type, int64_t N, const float *bo
  * n_neigh[i] > max_neigh hold max_neigh true neighbors; re-allocate with capacity >= M and call again. */
 int qbvh_neighbors(const float *r_list_ij, int32_t *nlist, int32_t *n_neigh, int32_t max_neigh);
 
+/* The same call in two halves, for callers that keep the stream busy (an MD step enqueues its force kernels behind
+ * the list) and for timing the device work without a host round trip inside it:
+ *   qbvh_neighbors_enqueue  checks its arguments, enqueues the traversal on the stream and returns QBVH_OK (or < 0)
+ *                           without waiting; arguments as for qbvh_neighbors (nlist, n_neigh stay in use until the
+ *                           result has been taken);
+ *   qbvh_neighbors_result   synchronises the stream and returns what qbvh_neighbors would have returned for the last
+ *                           enqueue (M >= 0, or QBVH_ERR_TYPE_RANGE / QBVH_ERR_INTERNAL / QBVH_ERR_CUDA);
+ *                           QBVH_ERR_NOT_BUILT if nothing was enqueued since the last result.
+ * qbvh_neighbors is exactly enqueue followed by result. */
+int qbvh_neighbors_enqueue(const float *r_list_ij, int32_t *nlist, int32_t *n_neigh, int32_t max_neigh);
+int qbvh_neighbors_result(void);
+
 /* Query sharding ("straightforwardly generalized to execute on multiple GPUs"): the
  * same traversal for the particles at sorted (Z-order) positions [first, first + count) only.  Row k of nlist and
  * n_neigh[k] belong to the particle at sorted position first + k, whose original index is QBVH_EXPORT_PERM[first + k];

@@ -24,6 +24,9 @@ struct Context {
     bool stats = false;
     int variant = 1;
     bool built = false;
+    bool enqueued = false;       // a qbvh_neighbors_enqueue whose result has not been taken
+    bool counters_armed = false; // group_cursor, max_count, warps_done of the tree are zero (after a build, after a production traversal)
+    int32_t *pinned_dev = nullptr;   // device-side address of `pinned`
     int64_t N = 0;
     float box[6] = {0, 0, 0, 0, 0, 0};
     double box64[6] = {0, 0, 0, 0, 0, 0};   // the box of a double-precision build
@@ -189,17 +192,31 @@ int neighbors_impl(const RT *r_list, bool f64, int32_t *nlist, int32_t *n_neigh,
     P.q_count = (int32_t)q_count;
     if (q_count >= 0 && (g.variant != 1 || q_first < 0 || q_first + q_count > g.N)) return QBVH_ERR_INVALID_ARG;
     cudaError_t e;
-    // reset group_cursor and max_count (+ stats) of the previous traversal
-    e = cudaMemsetAsync(&g.buf.meta->group_cursor, 0, 2 * sizeof(int32_t), g.stream);
-    if (e != cudaSuccess) return cuda_fail(e, "memset max_count");
+    // The production kernel alone: its last warp writes {max_count, err_flags} into the pinned result words and
+    // re-arms the counters, so the launch needs no memset in front and no copy behind (two stream operations and
+    // their gaps, about 7 us).  Any other path clears the counters first and copies the result afterwards.
+    const bool self_contained = g.variant == 1 && !g.stats && g.N > 0 && g.pinned_dev != nullptr;
+    P.result_host = self_contained ? g.pinned_dev : nullptr;
+    if (!self_contained || !g.counters_armed) {
+        // group_cursor, max_count (+ warps_done, stats) of whatever ran before
+        e = cudaMemsetAsync(&g.buf.meta->group_cursor, 0, 2 * sizeof(int32_t), g.stream);
+        if (e != cudaSuccess) return cuda_fail(e, "memset max_count");
+        e = cudaMemsetAsync(&g.buf.meta->warps_done, 0, sizeof(int32_t), g.stream);
+        if (e != cudaSuccess) return cuda_fail(e, "memset warps_done");
+    }
     if (g.stats) {
         e = cudaMemsetAsync(g.buf.meta->stats, 0, sizeof(g.buf.meta->stats), g.stream);
         if (e != cudaSuccess) return cuda_fail(e, "memset stats");
     }
+    g.counters_armed = false;
     e = launch_traverse(P, g.buf, nlist, n_neigh, g.stats, g.variant, f64, g.stream);
     if (e != cudaSuccess) return cuda_fail(e, "traverse launch");
-    e = cudaMemcpyAsync(g.pinned, &g.buf.meta->max_count, 2 * sizeof(int32_t), cudaMemcpyDeviceToHost, g.stream);
-    if (e != cudaSuccess) return cuda_fail(e, "copy max_count");
+    if (self_contained) {
+        g.counters_armed = true;
+    } else {
+        e = cudaMemcpyAsync(g.pinned, &g.buf.meta->max_count, 2 * sizeof(int32_t), cudaMemcpyDeviceToHost, g.stream);
+        if (e != cudaSuccess) return cuda_fail(e, "copy max_count");
+    }
     if (g.stats) {
         e = cudaMemcpyAsync(&g.last_stats, g.buf.meta->stats, sizeof(qbvh_stats), cudaMemcpyDeviceToHost, g.stream);
         if (e != cudaSuccess) return cuda_fail(e, "copy stats");
@@ -217,6 +234,7 @@ int finish_neighbors() {
 
 int build_impl(const void *pos, bool f64, const int32_t *type, int64_t N, const float *box) {
     g.built = false;
+    g.enqueued = false;
     if (N < 0 || N >= (int64_t(1) << 30) || !box || (N > 0 && !pos)) return QBVH_ERR_INVALID_ARG;
     for (int d = 0; d < 3; ++d)
         if (!std::isfinite(box[d]) || !std::isfinite(box[3 + d]) || !(box[3 + d] > 0.0f)) return QBVH_ERR_INVALID_ARG;
@@ -226,6 +244,9 @@ int build_impl(const void *pos, bool f64, const int32_t *type, int64_t N, const 
         cudaError_t e = cudaHostAlloc(reinterpret_cast<void **>(&g.pinned), 4 * sizeof(int32_t), cudaHostAllocDefault);
         if (e != cudaSuccess) return cuda_fail(e, "cudaHostAlloc");
         g.pinned[0] = g.pinned[1] = g.pinned[2] = g.pinned[3] = 0;
+        void *dp = nullptr;
+        if (cudaHostGetDevicePointer(&dp, g.pinned, 0) == cudaSuccess) g.pinned_dev = static_cast<int32_t *>(dp);
+        else (void)cudaGetLastError();
     }
     char *w = static_cast<char *>(g.ws);
     g.buf.meta = reinterpret_cast<TreeMeta *>(w + L.meta);
@@ -280,6 +301,7 @@ int build_impl(const void *pos, bool f64, const int32_t *type, int64_t N, const 
     g.f64_built = f64;
     g.lvl_built = bp.lvl;
     g.built = true;
+    g.counters_armed = true;      // the build starts by zeroing TreeMeta
     return QBVH_OK;
 }
 
@@ -366,6 +388,19 @@ int qbvh_neighbors(const float *r_list_ij, int32_t *nlist, int32_t *n_neigh, int
     return finish_neighbors();
 }
 
+int qbvh_neighbors_enqueue(const float *r_list_ij, int32_t *nlist, int32_t *n_neigh, int32_t max_neigh) {
+    g.enqueued = false;
+    int rc = neighbors_impl(r_list_ij, false, nlist, n_neigh, max_neigh);
+    g.enqueued = rc == QBVH_OK;
+    return rc;
+}
+
+int qbvh_neighbors_result(void) {
+    if (!g.enqueued) return QBVH_ERR_NOT_BUILT;
+    g.enqueued = false;
+    return finish_neighbors();
+}
+
 int qbvh_neighbors_range(const float *r_list_ij, int32_t *nlist, int32_t *n_neigh, int32_t max_neigh, int64_t first, int64_t count) {
     if (count < 0) return QBVH_ERR_INVALID_ARG;
     int rc = neighbors_impl(r_list_ij, false, nlist, n_neigh, max_neigh, first, count);
@@ -401,6 +436,7 @@ int qbvh_count_overlaps(const float *r_list_ij, int32_t *n_overlap) {
     P.q_first = 0, P.q_count = -1;
     cudaError_t e = cudaMemsetAsync(&g.buf.meta->group_cursor, 0, 2 * sizeof(int32_t), g.stream);
     if (e != cudaSuccess) return cuda_fail(e, "memset max_count");
+    g.counters_armed = false;
     e = launch_count_overlaps(P, g.buf, n_overlap, g.stream);
     if (e != cudaSuccess) return cuda_fail(e, "count launch");
     e = cudaMemcpyAsync(g.pinned, &g.buf.meta->max_count, 2 * sizeof(int32_t), cudaMemcpyDeviceToHost, g.stream);

@@ -38,7 +38,7 @@ struct TreeMeta {
     int32_t max_count;              // max_i n_neigh[i] of the last traversal
     int32_t err_flags;              // bit 0: type id out of range; bit 1: traversal work list bound violated
     int32_t nodes_emitted;          // nodes written by the build (2N-1 without collapse)
-    int32_t pad2a_;
+    int32_t warps_done;             // warps of the running production traversal that have finished (the last one cleans up)
     unsigned long long d2h_bytes;   // list bytes the last rows_to_host_kernel wrote to host memory
     int32_t pad2_[24];
     unsigned long long stats[16];   // qbvh_stats, in order
@@ -89,6 +89,9 @@ struct TraverseParams {
     int32_t N;
     int32_t max_neigh;
     int32_t K;                         // leaf-collapse cap used by the build
+    int32_t *result_host;              // production kernel: where its last warp writes {max_count, err_flags} (pinned host
+                                       // memory, device-mapped) before it re-arms group_cursor, max_count and warps_done; nullptr: the
+                                       // host clears and copies them around the launch
     int32_t q_first, q_count;          // query sharding: only these sorted positions are queries, row = position - q_first; q_count < 0: all, row = original index
     // double-precision particle data (qbvh_neighbors_f64): r2 above is then (r + B)^2 rounded up — whatever fails it
     // in fp32 on the rounded positions cannot be a neighbor in fp64 —, r2lo = (r - B)^2 rounded down — whatever passes

@@ -873,6 +873,20 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
     wmax = __reduce_max_sync(FULL, wmax);
     if (lane == 0 && wmax > 0) atomicMax(&meta->max_count, wmax);
     if (lane == 0 && bound_violated) atomicOr(&meta->err_flags, 2);
+    if (P.result_host != nullptr && lane == 0) {
+        // The last warp to finish hands the result to the host (a write into pinned memory: no copy behind the
+        // kernel) and re-arms the counters for the next traversal of this tree (no memset in front of it).
+        __threadfence();
+        if (atomicAdd(&meta->warps_done, 1) == (int)(gridDim.x * GW_WARPS) - 1) {
+            __threadfence();
+            P.result_host[0] = atomicMax(&meta->max_count, 0);
+            P.result_host[1] = atomicOr(&meta->err_flags, 0);
+            __threadfence_system();
+            meta->max_count = 0;
+            meta->group_cursor = 0;
+            meta->warps_done = 0;
+        }
+    }
     if (STATS && lane == 0) {
         atomicAdd(&meta->stats[5], st_groups);
         atomicAdd(&meta->stats[6], st_tests);

@@ -24,7 +24,8 @@ EXPORT_KEYS_SORTED, EXPORT_PERM, EXPORT_NODES, EXPORT_PARENT, EXPORT_FRAMES, EXP
 SYMBOLS = ("qbvh_set_stream", "qbvh_set_num_types", "qbvh_workspace_bytes", "qbvh_set_workspace",
            "qbvh_set_option", "qbvh_get_option", "qbvh_build", "qbvh_neighbors", "qbvh_count_overlaps", "qbvh_staging_bytes",
            "qbvh_set_staging", "qbvh_build_host", "qbvh_neighbors_host", "qbvh_get_stats", "qbvh_debug_export",
-           "qbvh_error_string", "qbvh_padded_radius", "qbvh_set_collapse_hint", "qbvh_build_f64", "qbvh_neighbors_f64", "qbvh_last_d2h_bytes", "qbvh_neighbors_range")
+           "qbvh_error_string", "qbvh_padded_radius", "qbvh_set_collapse_hint", "qbvh_build_f64", "qbvh_neighbors_f64", "qbvh_last_d2h_bytes", "qbvh_neighbors_range",
+           "qbvh_neighbors_enqueue", "qbvh_neighbors_result")
 
 
 class QbvhStats(C.Structure):
@@ -55,6 +56,8 @@ _lib.qbvh_get_option.argtypes = [_i32]
 _lib.qbvh_set_collapse_hint.argtypes = [_vp, _i32]
 _lib.qbvh_build.argtypes = [_vp, _vp, _i64, _vp]
 _lib.qbvh_neighbors.argtypes = [_vp, _vp, _vp, _i32]
+_lib.qbvh_neighbors_enqueue.argtypes = [_vp, _vp, _vp, _i32]
+_lib.qbvh_neighbors_result.argtypes = []
 _lib.qbvh_count_overlaps.argtypes = [_vp, _vp]
 _lib.qbvh_neighbors_range.argtypes = [_vp, _vp, _vp, _i32, _i64, _i64]
 _lib.qbvh_build_f64.argtypes = [_vp, _vp, _i64, _vp]
@@ -165,6 +168,17 @@ def qbvh_neighbors(r_list_ij, nlist, n_neigh, max_neigh: int) -> int:
     """r_list_ij: host T x T; nlist, n_neigh: DEVICE int32 tensors.  Returns M = max n_neigh (overflow iff M > max_neigh)."""
     r = _r_list(r_list_ij)
     return _check(_lib.qbvh_neighbors(r.ctypes.data, _ptr(nlist), _ptr(n_neigh), max_neigh), "qbvh_neighbors")
+
+
+def qbvh_neighbors_enqueue(r_list_ij, nlist, n_neigh, max_neigh: int) -> None:
+    """qbvh_neighbors without the wait: the traversal is enqueued on the stream; take M with qbvh_neighbors_result."""
+    r = _r_list(r_list_ij)
+    _check(_lib.qbvh_neighbors_enqueue(r.ctypes.data, _ptr(nlist), _ptr(n_neigh), max_neigh), "qbvh_neighbors_enqueue")
+
+
+def qbvh_neighbors_result() -> int:
+    """Synchronises the stream; M of the last qbvh_neighbors_enqueue."""
+    return _check(_lib.qbvh_neighbors_result(), "qbvh_neighbors_result")
 
 
 def qbvh_neighbors_range(r_list_ij, nlist, n_neigh, max_neigh: int, first: int, count: int) -> int:
@@ -300,6 +314,13 @@ class NeighborList:
         self._activate()
         self.f64 = pos.dtype == self.torch.float64
         return (qbvh_build_f64 if self.f64 else qbvh_build)(pos, type, self.N, box)
+
+    def neighbors_enqueue(self, r_list) -> None:
+        """fp32 lists without the wait (qbvh_neighbors_enqueue); M comes from neighbors_result()."""
+        qbvh_neighbors_enqueue(r_list, self.nlist, self.n_neigh, self.max_neigh)
+
+    def neighbors_result(self) -> int:
+        return qbvh_neighbors_result()
 
     def neighbors(self, r_list, retry: bool = True) -> int:
         call = qbvh_neighbors_f64 if getattr(self, "f64", False) else qbvh_neighbors

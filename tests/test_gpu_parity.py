@@ -666,3 +666,34 @@ def test_cell_grid_level_choice(N, T, lvl):
     out = gpu_run(w, K=32, export=True)
     assert int(out["counts"][3]) == lvl
     compare_with_oracle(w, out, ON.neighbor_list(pos, typ, box, r), allow_overflow=True)
+
+
+def test_enqueue_result_is_qbvh_neighbors_in_two_halves():
+    """qbvh_neighbors_enqueue + qbvh_neighbors_result: same lists, counts and M as qbvh_neighbors; a result without
+    an enqueue, or after a rebuild, is refused."""
+    import torch
+    from paper_1901_08088_b200 import qbvh
+    w = W.make_config(1)
+    dev = torch.device("cuda:0")
+    qbvh.qbvh_set_option(qbvh.OPT_LEAF_COLLAPSE, 32)
+    qbvh.qbvh_set_option(qbvh.OPT_STATS, 0)
+    nl = qbvh.NeighborList(w.N, T=w.T, max_neigh=w.max_neigh, device=dev)
+    nl.build(torch.from_numpy(w.pos).to(dev), None, w.box)
+    M0 = nl.neighbors(w.r_list, retry=False)
+    ref_cnt, ref_list = nl.n_neigh.clone(), nl.nlist.clone()
+    nl.n_neigh.fill_(-1)
+    nl.nlist.fill_(-1)
+    nl.neighbors_enqueue(w.r_list)
+    assert nl.neighbors_result() == M0
+    assert torch.equal(nl.n_neigh, ref_cnt)
+    a, b = nl.nlist.cpu().numpy(), ref_list.cpu().numpy()
+    c = ref_cnt.cpu().numpy()
+    for i in range(w.N):
+        assert np.array_equal(np.sort(a[i, :c[i]]), np.sort(b[i, :c[i]]))
+    with pytest.raises(qbvh.QbvhError):
+        qbvh.qbvh_neighbors_result()                      # nothing enqueued any more
+    nl.neighbors_enqueue(w.r_list)
+    nl.build(torch.from_numpy(w.pos).to(dev), None, w.box)   # a rebuild drops the pending result
+    with pytest.raises(qbvh.QbvhError):
+        qbvh.qbvh_neighbors_result()
+    torch.cuda.synchronize()
