@@ -816,7 +816,7 @@ __global__ void __launch_bounds__(GW_WARPS * 32) traverse_group_kernel(TraverseP
                         int nkept = 0;
 #pragma unroll
                         for (int u = 0; u < GW_NB; ++u) {
-                            keep[u] = sub < (int)lf[u].y && point_in_reach(pc[u], blo, bhi, R2);
+                            keep[u] = point_in_reach(pc[u], blo, bhi, R2) & (sub < (int)lf[u].y);   // (no short circuit: no branch)
                             const uint32_t kb = __ballot_sync(FULL, keep[u]);
                             if (keep[u]) {
                                 const int slot = (thead + tcount + nkept + __popc(kb & lt_mask)) & (GW_TILE - 1);
