@@ -263,20 +263,33 @@ def run_gpu(args):
     build_bytes = N * (188.0 + (4.0 if w.type is not None else 0.0))
     trav_ms, build_ms = float(np.mean(t_trav)), float(np.mean(t_build))
     ach = trav_bytes / (trav_ms * 1e-3) / 1e9
-    # DRAM traffic of one traversal launch: a STORED ncu measurement (dram__bytes_read.sum + dram__bytes_write.sum,
-    # profiles/), valid for config 2 / fp32 at the commit named beside it; null for anything else
+    # Counters of one traversal launch that only a profiler sees: STORED ncu measurements (profiles/), valid for
+    # config 2 / fp32 at the commit named beside them; null for anything else.
     traffic = traffic_commit = None
-    tp = os.path.join(ROOT, "profiles", "traverse_traffic_bytes.txt")
+    counters = {}
+    tp = os.path.join(ROOT, "profiles", "traverse_ncu_counters.txt")
     if os.path.exists(tp) and args.config == 2 and not f64:
         try:
-            tok = open(tp).read().split()
-            traffic, traffic_commit = float(tok[0]), (tok[1] if len(tok) > 1 else None)
+            counters = dict(tok.split("=", 1) for tok in open(tp).read().split() if "=" in tok)
+            traffic, traffic_commit = float(counters["dram_bytes"]), counters.get("commit")
         except Exception:
             traffic = traffic_commit = None
+            counters = {}
     roofline = {"bound": "hbm", "kernel": "traverse_group_kernel", "achieved": ach, "peak": peak, "unit": "GB/s",
                 "frac": ach / peak, "traffic": traffic, "traffic_source": "stored ncu capture", "traffic_commit": traffic_commit,
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": trav_bytes}
-    # plain-ALU view of the same kernel: thread-instructions issued / (148 SM x 128 lanes x f)
+    # What actually bounds the kernel: warp-instruction issue.  Slots = instructions executed, the packed
+    # f32x2 ones counted twice (they hold the issue port for two cycles); peak = 4 schedulers x SMs x SM clock.
+    roofline_issue = None
+    if "inst_executed" in counters:
+        sms = torch.cuda.get_device_properties(dev).multi_processor_count
+        slots = float(counters["inst_executed"]) + float(counters.get("fp2_inst", 0))
+        clk_mhz = clocks["sm_mhz"] if clocks.get("sm_mhz") else clocks.get("sm_max_mhz") or 1965
+        ipeak = 4.0 * sms * clk_mhz * 1e6
+        roofline_issue = {"bound": "alu", "kernel": "traverse_group_kernel", "unit": "warp-instruction issue slots/s",
+                          "achieved": slots / (trav_ms * 1e-3), "peak": ipeak, "frac": slots / (trav_ms * 1e-3) / ipeak,
+                          "slots_per_launch": slots, "source": "stored ncu capture (smsp__inst_executed.sum + FADD2/FMUL2/FFMA2 once more)",
+                          "commit": traffic_commit}
     whole = (trav_bytes + build_bytes) / (ms_per_step * 1e-3) / 1e9
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": max(args.warmup, 3),
@@ -298,7 +311,7 @@ def run_gpu(args):
             "census_dist_checks_per_particle": stats["dist_checks"] / N,
             "nodes_written": int(counts[0]), "node_bytes": 16 * int(counts[0]), "node_bytes_uncollapsed": 16 * (2 * N - 1),
             "query_groups": int(counts[1]), "morton_cells": int(counts[2]), "cell_level": int(counts[3]),
-            "roofline": roofline,
+            "roofline": roofline, "roofline_issue": roofline_issue,
             "roofline_whole_path": {"bound": "hbm", "achieved": whole, "peak": peak, "unit": "GB/s", "frac": whole / peak,
                                     "algorithmic_bytes_per_step": trav_bytes + build_bytes},
             "e2e": (None if e2e_ms is None else
