@@ -41,6 +41,8 @@ extern "C" {
 #define QBVH_ERR_CUDA (-6)             /* a CUDA runtime call failed; text via qbvh_error_string(QBVH_ERR_CUDA)    */
 #define QBVH_ERR_INTERNAL (-7)         /* an internal bound was violated (the traversal's work list); the
                                           lists of that call are invalid.  Never seen; reported instead of corrupting. */
+#define QBVH_ERR_NOALLOC_LIMIT (-8)    /* qbvh_morton_keys_noalloc: N is larger than QBVH_NOALLOC_MAX_N, the size its built-in
+                                          scratch array was compiled for; use the workspace path (qbvh_build) instead   */
 
 #define QBVH_MAX_TYPES 4 /* type id lives in bits 30-31 of the 32-bit sort key above the 30-bit Morton code */
 
@@ -178,6 +180,39 @@ int qbvh_build_host(const float *pos, const int32_t *type, int64_t N, const floa
 int qbvh_neighbors_host(const float *r_list_ij, int32_t *nlist, int32_t *n_neigh, int32_t max_neigh);
 /* Bytes the last qbvh_neighbors_host call copied from the device. */
 int64_t qbvh_last_d2h_bytes(void);
+
+/* ---- for callers that cannot allocate device memory ------------------------------------------------------------
+ * Every call above needs a workspace the caller got from cudaMalloc (or from an allocator built on it).  Some callers
+ * have no such source: a plugin or callback that runs inside another GPU program and is only handed that program's
+ * buffers; code under a framework whose memory pool already owns all of the HBM, where a plain cudaMalloc fails; a
+ * latency-critical loop where cudaMalloc / cudaFree are banned because they synchronise the device.  For them, ONE
+ * entry point that allocates nothing, anywhere: step a1 of the path — the Morton keys of all particles (PAPER.md:61,
+ * §2.1: box divided into 2^10-1 bins per axis, bits interleaved along the Z-order curve) and the root box of each
+ * type's tree with its quantization step (§2.2) — e.g. to re-order particle arrays along the Z-curve or
+ * to quantize against the same frame as the tree.  Its working memory (one 96-byte record per block of 1024 particles,
+ * for the two-stage min/max reduction) is a fixed array compiled into the library: 393,472 bytes of device memory on
+ * every GPU that loads libqbvh.so, held until the process exits.  Hence:
+ *   - N <= QBVH_NOALLOC_MAX_N, otherwise QBVH_ERR_NOALLOC_LIMIT and nothing is enqueued;
+ *   - all calls (from any thread, on any stream) share that one array per GPU and the call starts by clearing the part
+ *     of it that must be zero: two calls whose device work can overlap — different streams without an ordering
+ *     between them — race on it and give wrong frames.  Calls on one stream, or ordered by events, are fine;
+ *   - the first call on each device looks up the array's device address (cudaGetSymbolAddress, with that device
+ *     current, which may also make the runtime load the module): make that first call outside any stream capture.
+ * The call uses none of the library's global state (no workspace, no qbvh_set_stream, no tree) and leaves it alone.
+ * It calls no cudaMalloc, cudaFree, cudaHostAlloc or other allocating routine; it enqueues one memset of 256 bytes and
+ * one kernel on `cuda_stream` and returns without waiting.
+ *   pos     DEVICE  N x 3 fp32 row-major, as for qbvh_build.      type  DEVICE N int32 in [0, T), or NULL (all type 0).
+ *   box     HOST    6 floats {lo_xyz, L_xyz}, as for qbvh_build.   T     number of types, 1..QBVH_MAX_TYPES.
+ *   keys    DEVICE  N uint32 out: type << 30 | 30-bit Morton code of particle i — the multiset of
+ *                   QBVH_EXPORT_KEYS_SORTED, in input order.  An out-of-range type is keyed as type 0 (as qbvh_build).
+ *   frames  DEVICE  4 x 12 floats out: per type {lo_xyz, hi_xyz, delta_xyz, 0, 0, 0}, bitwise what QBVH_EXPORT_FRAMES
+ *                   shows after qbvh_build on the same input; all zero for a type without particles.
+ *   status  DEVICE  1 int32 out: bit 0 set iff some type id was outside [0, T).
+ *   cuda_stream     a cudaStream_t (NULL: the default stream).
+ * Returns QBVH_OK, QBVH_ERR_INVALID_ARG, QBVH_ERR_NOALLOC_LIMIT or QBVH_ERR_CUDA.  N = 0 is valid (frames all zero). */
+#define QBVH_NOALLOC_MAX_N 4194304 /* 2^22 particles = 4096 block records */
+int qbvh_morton_keys_noalloc(const float *pos, const int32_t *type, int64_t N, const float *box, int32_t T,
+                             uint32_t *keys, float *frames, int32_t *status, void *cuda_stream);
 
 /* ---- inspection ----------------------------------------------------------------------------- */
 

@@ -9,7 +9,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libqbvh.so")
-SRCS = [os.path.join(CSRC, f) for f in ("api.cu", "build_kernels.cu", "traverse_kernels.cu")]
+SRCS = [os.path.join(CSRC, f) for f in ("api.cu", "build_kernels.cu", "traverse_kernels.cu", "no_alloc.cu")]
 DEPS = SRCS + [os.path.join(CSRC, "qbvh_internal.cuh"), os.path.join(os.path.dirname(HERE), "include", "qbvh.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC,-frounding-math", "-shared", "-cudart", "static"]

@@ -307,6 +307,8 @@ int build_impl(const void *pos, bool f64, const int32_t *type, int64_t N, const 
 
 }  // namespace
 
+int qbvh_record_cuda_error(cudaError_t e, const char *where) { return cuda_fail(e, where); }
+
 extern "C" {
 
 int qbvh_set_stream(void *cuda_stream) {
@@ -603,6 +605,7 @@ const char *qbvh_error_string(int code) {
         case QBVH_ERR_CUTOFF_TOO_LARGE: return "padded cutoff is not below half the shortest box length";
         case QBVH_ERR_TYPE_RANGE: return "a particle type id is outside [0, T)";
         case QBVH_ERR_INTERNAL: return "internal bound violated (traversal work list); please report";
+        case QBVH_ERR_NOALLOC_LIMIT: return "N exceeds QBVH_NOALLOC_MAX_N (4194304), the size of the built-in scratch of qbvh_morton_keys_noalloc";
         case QBVH_ERR_CUDA: return g.cuda_msg;
         default: return code > 0 ? "ok (positive return value)" : "unknown error code";
     }

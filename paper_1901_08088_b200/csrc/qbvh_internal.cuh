@@ -163,4 +163,6 @@ int traverse_warp_slots();      // warps the production traversal keeps resident
 // every row, in 16-byte pieces (qbvh_neighbors_host); max_neigh % 4 == 0, both lists 16-byte aligned
 cudaError_t launch_rows_to_host(const int32_t *dlist, const int32_t *dcnt, int32_t *hlist_dev, int64_t N, int32_t max_neigh,
                                 TreeMeta *meta, cudaStream_t st);
+// api.cu: keeps the text of a failed CUDA call for qbvh_error_string(QBVH_ERR_CUDA); returns QBVH_ERR_CUDA
+int qbvh_record_cuda_error(cudaError_t e, const char *where);
 static_assert(offsetof(TreeMeta, group_count) % 128 == 0, "the atomic counters start a 128-byte line");

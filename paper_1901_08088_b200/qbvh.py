@@ -16,6 +16,8 @@ LIB_PATH = os.path.join(_HERE, "libqbvh.so")
 
 OK = 0
 ERR_INVALID_ARG, ERR_NOT_BUILT, ERR_WORKSPACE, ERR_CUTOFF_TOO_LARGE, ERR_TYPE_RANGE, ERR_CUDA, ERR_INTERNAL = -1, -2, -3, -4, -5, -6, -7
+ERR_NOALLOC_LIMIT = -8
+NOALLOC_MAX_N = 1 << 22
 MAX_TYPES = 4
 OPT_LEAF_COLLAPSE, OPT_STATS, OPT_VARIANT, OPT_DEBUG_BUILD_TAG = 1, 2, 3, 4
 EXPORT_KEYS_SORTED, EXPORT_PERM, EXPORT_NODES, EXPORT_PARENT, EXPORT_FRAMES, EXPORT_SEGMENTS, EXPORT_SORTED_POS, EXPORT_COUNTS = range(1, 9)
@@ -25,7 +27,7 @@ SYMBOLS = ("qbvh_set_stream", "qbvh_set_num_types", "qbvh_workspace_bytes", "qbv
            "qbvh_set_option", "qbvh_get_option", "qbvh_build", "qbvh_neighbors", "qbvh_count_overlaps", "qbvh_staging_bytes",
            "qbvh_set_staging", "qbvh_build_host", "qbvh_neighbors_host", "qbvh_get_stats", "qbvh_debug_export",
            "qbvh_error_string", "qbvh_padded_radius", "qbvh_set_collapse_hint", "qbvh_build_f64", "qbvh_neighbors_f64", "qbvh_last_d2h_bytes", "qbvh_neighbors_range",
-           "qbvh_neighbors_enqueue", "qbvh_neighbors_result")
+           "qbvh_neighbors_enqueue", "qbvh_neighbors_result", "qbvh_morton_keys_noalloc")
 
 
 class QbvhStats(C.Structure):
@@ -74,6 +76,7 @@ _lib.qbvh_debug_export.argtypes = [_i32, _vp, _i64]
 _lib.qbvh_debug_export.restype = _i64
 _lib.qbvh_padded_radius.argtypes = [C.c_float, _vp]
 _lib.qbvh_padded_radius.restype = C.c_float
+_lib.qbvh_morton_keys_noalloc.argtypes = [_vp, _vp, _i64, _vp, _i32, _vp, _vp, _vp, _vp]
 _lib.qbvh_error_string.argtypes = [C.c_int]
 _lib.qbvh_error_string.restype = C.c_char_p
 
@@ -237,6 +240,15 @@ def qbvh_padded_radius(r: float, box) -> float:
     if v < 0:
         raise QbvhError(ERR_INVALID_ARG, "qbvh_padded_radius")
     return v
+
+
+def qbvh_morton_keys_noalloc(pos, type, N: int, box, T: int, keys, frames, status, cuda_stream: int | None = None) -> int:
+    """Morton keys + per-type root frames with no workspace and no allocation (include/qbvh.h): for callers that
+    cannot obtain device memory themselves.  pos, type, keys (uint32/int32 N), frames (float32 4 x 12), status
+    (int32 1): DEVICE tensors the caller already has; box: 6 host floats.  N <= NOALLOC_MAX_N.  Asynchronous."""
+    box = _host_f32(box, 6)
+    return _check(_lib.qbvh_morton_keys_noalloc(_ptr(pos), _ptr(type), N, box.ctypes.data, T, _ptr(keys), _ptr(frames),
+                                                _ptr(status), cuda_stream), "qbvh_morton_keys_noalloc")
 
 
 def qbvh_last_d2h_bytes() -> int:
