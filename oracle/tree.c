@@ -292,6 +292,13 @@ static float mul_ru(float a, float b) {
     return r;
 }
 
+/* Squared padded pruning radius, rounded UP (reading R11; "the sphere radius is padded"):
+ * the right-hand side of every sphere/box test below.  Exported so that a test can pin it against exact rationals. */
+float oracle_R2(float r, float pad_abs) {
+    float rp = oracle_r_pad(r, pad_abs);
+    return mul_ru(rp, rp);
+}
+
 /* ---------------------------------------------------------------------------
  * a7 + a8. Algorithm 1 (reconstructed per R1), one particle at
  * a time, in the paper's "accept the leaf on box overlap" mode (line 14).
@@ -325,7 +332,7 @@ int64_t oracle_traverse(const float *pos_sorted, int64_t N, const int64_t *seg, 
     float pad_abs = oracle_pad_abs(box);
     int64_t total = 0;
     float *R2 = (float *)malloc(sizeof(float) * (size_t)(T * T));
-    for (int k = 0; k < T * T; ++k) R2[k] = r_list[k] > 0.0f ? mul_ru(oracle_r_pad(r_list[k], pad_abs), oracle_r_pad(r_list[k], pad_abs)) : -1.0f;
+    for (int k = 0; k < T * T; ++k) R2[k] = r_list[k] > 0.0f ? oracle_R2(r_list[k], pad_abs) : -1.0f;
 #pragma omp parallel for schedule(dynamic, 64) reduction(+ : total)
     for (int64_t k = 0; k < N; ++k) {
         int ta = 0;
@@ -382,6 +389,69 @@ int64_t oracle_traverse(const float *pos_sorted, int64_t N, const int64_t *seg, 
             n_tests[k] = tests;
             n_images[k] = nimg;
         }
+        total += cnt;
+    }
+    free(R2);
+    return total;
+}
+
+
+/* ---------------------------------------------------------------------------
+ * The same walk on the UNquantized fp32 boxes blo/bhi of oracle_fit_quantize (what the tree was before step a6):
+ * the census against which "extra false-positive AABB tests caused by quantization" are counted (PAPER.md:85, 89,
+ * 196-198).  Count pass only.  Everything but the source of a and b is oracle_traverse's.
+ * ------------------------------------------------------------------------- */
+int64_t oracle_traverse_fp32_boxes(const float *pos_sorted, int64_t N, const int64_t *seg, int32_t T, const float *box,
+                                   const float *r_list, const float *blo, const float *bhi, const int32_t *left,
+                                   const int32_t *rope, const int32_t *roots, int32_t *n_overlap, int64_t *n_tests,
+                                   int32_t *n_images) {
+    float pad_abs = oracle_pad_abs(box);
+    int64_t total = 0;
+    float *R2 = (float *)malloc(sizeof(float) * (size_t)(T * T));
+    for (int k = 0; k < T * T; ++k) R2[k] = r_list[k] > 0.0f ? oracle_R2(r_list[k], pad_abs) : -1.0f;
+#pragma omp parallel for schedule(dynamic, 64) reduction(+ : total)
+    for (int64_t k = 0; k < N; ++k) {
+        int ta = 0;
+        while (k >= seg[ta + 1]) ++ta;
+        const float *xi = pos_sorted + 3 * k;
+        int32_t cnt = 0, nimg = 0;
+        int64_t tests = 0;
+        for (int tb = 0; tb < T; ++tb) {
+            float r2 = R2[ta * T + tb];
+            if (r2 < 0.0f || roots[tb] < 0) continue;
+            int32_t root = roots[tb];
+            uint32_t bset = 0;
+            float x[3];
+            for (int img = 0; img < 27; ++img) {                                     /* line 4 */
+                int s[3] = {img % 3 - 1, (img / 3) % 3 - 1, img / 9 - 1};
+                for (int d = 0; d < 3; ++d) x[d] = xi[d] + (float)s[d] * box[3 + d];
+                if (sphere_box(x, blo + 3 * (size_t)root, bhi + 3 * (size_t)root, r2)) bset |= 1u << img;
+            }
+            while (bset) {
+                int img = __builtin_ctz(bset);
+                bset &= bset - 1;
+                ++nimg;
+                int s[3] = {img % 3 - 1, (img / 3) % 3 - 1, img / 9 - 1};
+                for (int d = 0; d < 3; ++d) x[d] = xi[d] + (float)s[d] * box[3 + d];
+                int32_t n = root;
+                while (n >= 0) {
+                    ++tests;
+                    if (sphere_box(x, blo + 3 * (size_t)n, bhi + 3 * (size_t)n, r2)) {
+                        if (left[n] < 0) {
+                            ++cnt;
+                            n = rope[n];
+                        } else {
+                            n = left[n];
+                        }
+                    } else {
+                        n = rope[n];
+                    }
+                }
+            }
+        }
+        n_overlap[k] = cnt;
+        n_tests[k] = tests;
+        n_images[k] = nimg;
         total += cnt;
     }
     free(R2);

@@ -41,6 +41,11 @@ def lib() -> C.CDLL:
         L.oracle_pad_abs.argtypes = [_f32p]
         L.oracle_r_pad.restype = C.c_float
         L.oracle_r_pad.argtypes = [C.c_float, C.c_float]
+        L.oracle_R2.restype = C.c_float
+        L.oracle_R2.argtypes = [C.c_float, C.c_float]
+        L.oracle_traverse_fp32_boxes.restype = C.c_int64
+        L.oracle_traverse_fp32_boxes.argtypes = [_f32p, C.c_int64, _i64p, C.c_int32, _f32p, _f32p, _f32p, _f32p, _i32p, _i32p,
+                                                 _i32p, _i32p, _i64p, _i32p]
         L.oracle_traverse.restype = C.c_int64
         L.oracle_traverse.argtypes = [_f32p, C.c_int64, _i64p, C.c_int32, _f32p, _f32p, _u32p, _u32p, _i32p, _i32p,
                                       _i32p, _f32p, _i32p, _i64p, _i32p, _i64p, _i32p]
@@ -85,6 +90,13 @@ def r_pad(r: float, box) -> np.float32:
     box = np.ascontiguousarray(box, np.float32)
     pad_abs = lib().oracle_pad_abs(_p(box, C.c_float))
     return np.float32(lib().oracle_r_pad(C.c_float(r), C.c_float(pad_abs)))
+
+
+def R2_pad(r: float, box) -> np.float32:
+    """Squared padded pruning radius, rounded up: the right-hand side of the sphere/box tests of the replay."""
+    box = np.ascontiguousarray(box, np.float32)
+    pad_abs = lib().oracle_pad_abs(_p(box, C.c_float))
+    return np.float32(lib().oracle_R2(C.c_float(r), C.c_float(pad_abs)))
 
 
 @dataclass
@@ -176,3 +188,20 @@ def traverse(tree: RefTree, box, r_list, fill: bool = False):
         out["row_ptr"] = row_ptr
         out["cand"] = cand[:total]
     return out
+
+
+def traverse_fp32_boxes(tree: RefTree, box, r_list):
+    """Algorithm 1 on the tree's unquantized fp32 boxes (count pass): the census the quantized one is compared with
+    to count the extra false-positive AABB tests of quantization."""
+    box = np.ascontiguousarray(box, np.float32)
+    r_list = np.ascontiguousarray(r_list, np.float32)
+    N, T = tree.N, tree.T
+    n_overlap = np.zeros(N, np.int32)
+    n_tests = np.zeros(N, np.int64)
+    n_images = np.zeros(N, np.int32)
+    blo, bhi = np.ascontiguousarray(tree.blo, np.float32), np.ascontiguousarray(tree.bhi, np.float32)
+    total = lib().oracle_traverse_fp32_boxes(_p(tree.pos_sorted, C.c_float), N, _p(tree.seg, C.c_int64), T, _p(box, C.c_float),
+                                             _p(r_list, C.c_float), _p(blo, C.c_float), _p(bhi, C.c_float),
+                                             _p(tree.left, C.c_int32), _p(tree.rope, C.c_int32), _p(tree.roots, C.c_int32),
+                                             _p(n_overlap, C.c_int32), _p(n_tests, C.c_int64), _p(n_images, C.c_int32))
+    return {"n_overlap": n_overlap, "n_tests": n_tests, "n_images": n_images, "total": int(total)}

@@ -441,6 +441,12 @@ def test_padded_radius_exact_rational(r, lo, L):
     assert f32_to_frac(want) >= f32_to_frac(r32) * (1 + Fraction(1, 2 ** 20)) + 8 * ulp
     assert OT.r_pad(r32, box) == want
     assert np.float32(qbvh.qbvh_padded_radius(float(r32), box)) == want
+    # ... and its square, the right-hand side of every sphere/box test, is rounded UP (RN or down could prune a box the
+    # padded sphere still touches): again each side against the exact rational, not against the other
+    want2 = round_up_f32(f32_to_frac(want) ** 2)
+    assert f32_to_frac(want2) >= f32_to_frac(want) ** 2 > f32_to_frac(np.nextafter(want2, np.float32(0)))
+    assert OT.R2_pad(r32, box) == want2
+    assert np.float32(qbvh.qbvh_padded_radius_sq(float(r32), box)) == want2
     # the pad is what it is for: ulp32(M) really is the fp32 spacing at magnitude M
     M = max(abs(float(box[d])) + 2 * float(box[3 + d]) for d in range(3))
     assert float(ulp) == float(np.spacing(np.float32(M))) or float(ulp) * 2 == float(np.spacing(np.float32(M)))
@@ -471,3 +477,47 @@ def test_boundary_pairs_across_faces_and_corners_are_never_missed(lo):
         cand = t.perm[tr["cand"][tr["row_ptr"][k]:tr["row_ptr"][k + 1]]]
         missed += len(np.setdiff1d(nb[rp[i]:rp[i + 1]], cand))
     assert missed == 0
+
+
+def test_R2_pin_can_tell_the_rounding_modes_apart():
+    """The R2 pin is only worth something if some PAD_CASES row has a square that is not an fp32 number (else round
+    up = round to nearest = round down and a wrong mode would pass)."""
+    differs = 0
+    for r, lo, L in PAD_CASES:
+        box = np.array(list(lo) + list(L), np.float32)
+        want, _ = pad_exact(np.float32(r), box)
+        exact = f32_to_frac(want) ** 2
+        differs += round_up_f32(exact) != np.float32(float(exact))          # RN lands below the exact square
+    assert differs >= 2
+
+
+def test_fp32_box_census_brute_force_and_against_the_quantized_one():
+    """Algorithm 1 on the unquantized fp32 boxes (the census quantization's extra AABB tests are counted against;
+    PAPER.md:85, 89, 196-198).  Pinned by brute force — with one particle per leaf a leaf box is the particle itself, so
+    the leaf overlaps of particle i are the (j, image) with |p_j - (x_i + v)|^2 <= R2, counted here in fp64 over all N x 27
+    — and by containment: every decompressed box contains its fp32 box and the fp32 test is monotone in the box, so per
+    particle the fp32 walk visits a subset of the quantized walk's nodes and accepts a subset of its leaves."""
+    rng = np.random.default_rng(5)
+    N, L, r = 600, 9.0, 1.6
+    pos, box = W._finish(rng.random((N, 3)) * L, L)
+    rl = np.array([[r]], np.float32)
+    t = OT.build(pos, None, box)
+    f = OT.traverse_fp32_boxes(t, box, rl)
+    q = OT.traverse(t, box, rl)
+    R2 = float(OT.R2_pad(np.float32(r), box))
+    ps = t.pos_sorted.astype(np.float64)
+    Lb = box[3:].astype(np.float64)
+    cnt = np.zeros(N, np.int64)
+    near = 0
+    for img in range(27):
+        v = np.array([img % 3 - 1, (img // 3) % 3 - 1, img // 9 - 1], np.float64) * Lb
+        d2 = (((ps[:, None, :] + v[None, None, :]) - ps[None, :, :]) ** 2).sum(-1)     # [i, j]
+        cnt += (d2 <= R2).sum(1)
+        near += int((np.abs(d2 - R2) < 1e-5 * R2).sum())
+    assert near == 0                                            # no pair close enough to R2 for fp32 rounding to matter
+    assert np.array_equal(f["n_overlap"].astype(np.int64), cnt)
+    assert cnt.sum() > 10 * N                                   # self included: a real census, not an empty one
+    assert np.all(f["n_overlap"] <= q["n_overlap"]) and np.all(f["n_tests"] <= q["n_tests"]) and np.all(f["n_images"] <= q["n_images"])
+    assert q["n_tests"].sum() > f["n_tests"].sum() and q["n_overlap"].sum() >= f["n_overlap"].sum()
+    # the extra tests are a small fraction (PAPER.md:89: 10 bits per axis "sufficient"): well under 5 % here
+    assert (q["n_tests"].sum() - f["n_tests"].sum()) < 0.05 * f["n_tests"].sum()
