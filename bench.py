@@ -107,14 +107,64 @@ def reference_sample(cid: int):
     return w, f"config-{cid} recipe at reduced size N={w.N}"
 
 
-def time_oracle(w, repeats: int = 1):
+def omp_threads(n: int | None = None) -> int:
+    """Thread count of the OpenMP runtime the oracle runs on (libgomp, shared with liboracle.so); sets it when n is given."""
+    import ctypes
+    gomp = ctypes.CDLL("libgomp.so.1")
+    prev = int(gomp.omp_get_max_threads())
+    if n is not None:
+        gomp.omp_set_num_threads(int(n))
+    return prev
+
+
+def time_oracle(w, repeats: int = 1, threads: int | None = None):
+    """The oracle as it stands, timed on the host cores (all of them, or `threads`)."""
     from oracle import neighbors as ON
     best = None
-    for _ in range(repeats):
-        t = {}
-        ON.neighbor_list(w.pos, w.type, w.box, w.r_list, method="cell", with_band=False, timing=t)
-        best = t if best is None or t["seconds"] < best["seconds"] else best
+    prev = omp_threads(threads) if threads is not None else None
+    try:
+        for _ in range(repeats):
+            t = {}
+            ON.neighbor_list(w.pos, w.type, w.box, w.r_list, method="cell", with_band=False, timing=t)
+            best = t if best is None or t["seconds"] < best["seconds"] else best
+    finally:
+        if prev is not None:
+            omp_threads(prev)
     return best
+
+
+def config_keys(cid: int, w) -> dict:
+    """The workload description both arms print (identical keys and values for the same --config)."""
+    return {"workload": f"BASELINE.json configs[{cid - 1}]: {w.name}", "N": w.N, "types": w.T,
+            "r_list": [float(x) for x in np.asarray(w.r_list).reshape(-1)], "max_neigh": w.max_neigh}
+
+
+def aabb_census(w, nl, qbvh, torch, dev):
+    """'Extra false-positive AABB tests' of the quantized tree (north_star): Algorithm 1's
+    node tests and leaf overlaps per particle on the quantized one-particle-per-leaf tree — counted by the GPU census
+    (QBVH_OPT_STATS, K = 1) — against the same walk on the tree's unquantized fp32 boxes, counted by the oracle replay
+    (the library keeps no fp32 boxes).  Outside every timed region."""
+    from oracle import tree as OT
+    K0 = qbvh.qbvh_get_option(qbvh.OPT_LEAF_COLLAPSE)
+    qbvh.qbvh_set_option(qbvh.OPT_LEAF_COLLAPSE, 1)
+    qbvh.qbvh_set_option(qbvh.OPT_STATS, 1)
+    try:
+        nl.build(torch.from_numpy(w.pos).to(dev), None if w.type is None else torch.from_numpy(w.type).to(dev), w.box)
+        nl.neighbors(w.r_list, retry=False)
+        s = qbvh.qbvh_get_stats()
+    finally:
+        qbvh.qbvh_set_option(qbvh.OPT_STATS, 0)
+        qbvh.qbvh_set_option(qbvh.OPT_LEAF_COLLAPSE, K0)
+    t = OT.build(w.pos, w.type, w.box, T=w.T)
+    f = OT.traverse_fp32_boxes(t, w.box, w.r_list)
+    N = w.N
+    tq, tf = s["node_tests"] / N, float(f["n_tests"].sum()) / N
+    lq, lf = s["leaf_overlaps"] / N, float(f["n_overlap"].sum()) / N
+    return {"node_tests_per_particle_quantized": tq, "node_tests_per_particle_fp32_boxes": tf,
+            "extra_node_tests_per_particle": tq - tf, "extra_node_tests_frac": (tq - tf) / tf if tf else None,
+            "leaf_overlaps_per_particle_quantized": lq, "leaf_overlaps_per_particle_fp32_boxes": lf,
+            "extra_leaf_overlaps_per_particle": lq - lf,
+            "source": "quantized: GPU census (QBVH_OPT_STATS, leaf collapse 1); fp32 boxes: oracle replay on the same tree"}
 
 
 def run_reference(args):
@@ -134,9 +184,7 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": False,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": f"BASELINE.json configs[{args.config - 1}]: {w.name}", "N": w.N, "types": w.T,
-                       "r_list": [float(x) for x in np.asarray(w.r_list).reshape(-1)], "max_neigh": w.max_neigh,
-                       "sample": what},
+            "config": config_keys(args.config, w), "notes": {"sample": what},
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": what},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -278,27 +326,30 @@ def run_gpu(args):
     roofline = {"bound": "hbm", "kernel": "traverse_group_kernel", "achieved": ach, "peak": peak, "unit": "GB/s",
                 "frac": ach / peak, "traffic": traffic, "traffic_source": "stored ncu capture", "traffic_commit": traffic_commit,
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": trav_bytes}
-    # What actually bounds the kernel: warp-instruction issue.  Slots = instructions executed, the packed
-    # f32x2 ones counted twice (they hold the issue port for two cycles); peak = 4 schedulers x SMs x SM clock.
+    # What actually bounds the kernel is on-chip throughput, not bytes.  The profiler's own utilisation
+    # figures of the stored capture (same commit stamp), quoted as they are — no derived "issue slot" arithmetic.
     roofline_issue = None
     if "inst_executed" in counters:
-        sms = torch.cuda.get_device_properties(dev).multi_processor_count
-        slots = float(counters["inst_executed"]) + float(counters.get("fp2_inst", 0))
-        clk_mhz = clocks["sm_mhz"] if clocks.get("sm_mhz") else clocks.get("sm_max_mhz") or 1965
-        ipeak = 4.0 * sms * clk_mhz * 1e6
-        roofline_issue = {"bound": "alu", "kernel": "traverse_group_kernel", "unit": "warp-instruction issue slots/s",
-                          "achieved": slots / (trav_ms * 1e-3), "peak": ipeak, "frac": slots / (trav_ms * 1e-3) / ipeak,
-                          "slots_per_launch": slots, "source": "stored ncu capture (smsp__inst_executed.sum + FADD2/FMUL2/FFMA2 once more)",
-                          "commit": traffic_commit}
+        def num(k):
+            return float(counters[k]) if k in counters else None
+        roofline_issue = {"kernel": "traverse_group_kernel", "source": "stored ncu capture (profiles/traverse_ncu_counters.txt)",
+                          "commit": traffic_commit, "warp_instructions_per_launch": num("inst_executed"),
+                          "warp_instructions_per_particle": num("inst_executed") / N,
+                          "sm_issue_active_pct": num("issue_active_pct"),
+                          "l1tex_lsu_data_pipe_wavefronts_pct": num("lsu_data_pipe_pct"),
+                          "shared_wavefronts": num("shared_wavefronts"),
+                          "shared_bank_conflict_wavefronts": num("shared_bank_conflicts")}
+    roofline_build = {"bound": "hbm", "kernel": "build (morton_cell + cell_scan + cell_scatter + cell_tree + top_tree)",
+                      "achieved": build_bytes / (build_ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+                      "frac": build_bytes / (build_ms * 1e-3) / 1e9 / peak, "algorithmic_bytes_per_step": build_bytes}
     whole = (trav_bytes + build_bytes) / (ms_per_step * 1e-3) / 1e9
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": max(args.warmup, 3),
             "ms_per_step": ms_per_step, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64 particles / f32 tree" if f64 else "f32", "data": "synthetic",
-            "config": {"workload": f"BASELINE.json configs[{args.config - 1}]: {w.name}", "N": N, "types": T,
-                       "r_list": [float(x) for x in np.asarray(w.r_list).reshape(-1)], "max_neigh": cap,
-                       "leaf_collapse": args.leaf_collapse, "l2": "flushed between timed iterations (256 MiB memset)",
-                       "parallelism": "replicas" if world > 1 else "single GPU"},
+            "config": config_keys(args.config, w),
+            "notes": {"leaf_collapse": args.leaf_collapse, "l2": "flushed between timed iterations (256 MiB memset)",
+                      "parallelism": "replicas" if world > 1 else "single GPU"},
             "build_ms": build_ms, "traverse_ms": trav_ms,
             "build_ns_per_particle": 1e6 * build_ms / N, "traverse_ns_per_particle": 1e6 * trav_ms / N,
             "neighbors_per_particle": nn, "max_neighbors": int(M),
@@ -311,7 +362,10 @@ def run_gpu(args):
             "census_dist_checks_per_particle": stats["dist_checks"] / N,
             "nodes_written": int(counts[0]), "node_bytes": 16 * int(counts[0]), "node_bytes_uncollapsed": 16 * (2 * N - 1),
             "query_groups": int(counts[1]), "morton_cells": int(counts[2]), "cell_level": int(counts[3]),
-            "roofline": roofline, "roofline_issue": roofline_issue,
+            # how full the query groups are and how many pair checks a found neighbor costs (the decomposition's own overhead)
+            "lanes_per_group": N / max(stats["groups"], 1),
+            "candidates_per_neighbor": stats["group_dist_checks"] / max(nn * N, 1.0),
+            "roofline": roofline, "roofline_issue": roofline_issue, "roofline_build": roofline_build,
             "roofline_whole_path": {"bound": "hbm", "achieved": whole, "peak": peak, "unit": "GB/s", "frac": whole / peak,
                                     "algorithmic_bytes_per_step": trav_bytes + build_bytes},
             "e2e": (None if e2e_ms is None else
@@ -330,6 +384,11 @@ def run_gpu(args):
             t = time_oracle(ws, repeats=2)
         line["cpu_baseline"] = {"value": 1e9 * t["seconds"] / ws.N, "unit": UNIT, "cores": t["threads"],
                                 "kind": "oracle", "sample": what, "seconds": t["seconds"]}
+        if not f64 and t["seconds"] * t["threads"] <= 25.0:          # bounded: about 10-30 s of CPU work at most
+            t1 = time_oracle(ws, repeats=1, threads=1)       # "plus the 1-thread time"
+            line["cpu_baseline"].update(value_1thread=1e9 * t1["seconds"] / ws.N, seconds_1thread=t1["seconds"])
+        if not f64 and not args.no_census and N <= (1 << 21):
+            line["aabb_tests"] = aabb_census(w, nl, qbvh, torch, dev)
     if rank == 0:
         print(json.dumps(line))
     if world > 1:
@@ -400,6 +459,7 @@ def main():
     ap.add_argument("--impl", default="qbvh", choices=["qbvh", "reference"])
     ap.add_argument("--leaf-collapse", type=int, default=32)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-census", action="store_true", help="skip the quantized-vs-fp32 AABB test census (oracle replay on the host)")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg (profiling runs)")
     ap.add_argument("--variant", type=int, default=None, help="traversal kernel (QBVH_OPT_VARIANT); default: the library's")
     ap.add_argument("--sharded", action="store_true", help="extra: query sharding over the ranks (strong scaling) instead of replicas")

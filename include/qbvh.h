@@ -72,12 +72,20 @@ int qbvh_set_workspace(void *dev_ptr, int64_t bytes);
                                     ("subtree collapse"); which subtrees: qbvh_set_collapse_hint.
                                     k = 1 is exactly the paper's one-particle-per-leaf tree. Default 32.           */
 #define QBVH_OPT_STATS 2         /* 0/1: qbvh_neighbors runs the instrumented traversal and fills qbvh_get_stats
-                                    (takes effect immediately; slower — never use when timing). Default 0.        */
+                                    (takes effect immediately; slower — never use when timing). Default 0.
+                                    The census writes a row per particle, so qbvh_neighbors_range refuses to run
+                                    with it (QBVH_ERR_INVALID_ARG); under qbvh_neighbors_f64 its `neighbors` field
+                                    counts by the widened fp32 cutoff (r + 8 ulp32(M)), not by the fp64 predicate.  */
 #define QBVH_OPT_VARIANT 3       /* which traversal kernel qbvh_neighbors launches: 0 = Algorithm 1 as written, one
                                     thread per particle; 1 (default) = one warp per query group.
                                     Both produce identical lists.                                                 */
 #define QBVH_OPT_DEBUG_BUILD_TAG 4 /* testing only: v in [1, 2^18): the next qbvh_build on this workspace uses meeting-
                                     slot tag v (forward jumps only) — lets a test reach the 18-bit wrap.           */
+#define QBVH_OPT_DEBUG_SCAN_SPIN 5  /* testing only: SM clock cycles a block of the build's 128-tile cell scan (cell grid
+                                    level 6, or level 5 with >= 3 types) waits for the other blocks before it sums the
+                                    counters in front of its tile itself (default 2^18, about 130 us; 0: never wait).
+                                    Either way the result is the same; the bound only matters on a device too busy to
+                                    hold all 128 blocks at once, where an unbounded wait could hang.               */
 int qbvh_set_option(int32_t key, int32_t value);
 
 /* Hint for the build-side subtree collapse ("collapse subtrees according to an appropriate heuristic",
@@ -125,7 +133,8 @@ int qbvh_neighbors(const float *r_list_ij, int32_t *nlist, int32_t *n_neigh, int
  *                           result has been taken);
  *   qbvh_neighbors_result   synchronises the stream and returns what qbvh_neighbors would have returned for the last
  *                           enqueue (M >= 0, or QBVH_ERR_TYPE_RANGE / QBVH_ERR_INTERNAL / QBVH_ERR_CUDA);
- *                           QBVH_ERR_NOT_BUILT if nothing was enqueued since the last result.
+ *                           QBVH_ERR_NOT_BUILT if nothing was enqueued since the last result, or if another
+ *                           neighbor call (or a build) came in between: those overwrite the result words.
  * qbvh_neighbors is exactly enqueue followed by result. */
 int qbvh_neighbors_enqueue(const float *r_list_ij, int32_t *nlist, int32_t *n_neigh, int32_t max_neigh);
 int qbvh_neighbors_result(void);
@@ -134,7 +143,7 @@ int qbvh_neighbors_result(void);
  * same traversal for the particles at sorted (Z-order) positions [first, first + count) only.  Row k of nlist and
  * n_neigh[k] belong to the particle at sorted position first + k, whose original index is QBVH_EXPORT_PERM[first + k];
  * entries are ORIGINAL indices as always.  nlist: DEVICE count x max_neigh; n_neigh: DEVICE count.  Returns the
- * maximum count over the range.  Every GPU of a sharded run holds all positions (one all-gather), builds the same
+ * maximum count over the range.  Needs QBVH_OPT_VARIANT = 1 and QBVH_OPT_STATS = 0 (else QBVH_ERR_INVALID_ARG).  Every GPU of a sharded run holds all positions (one all-gather), builds the same
  * tree and calls this for its own slice (paper_1901_08088_b200/sharded.py). */
 int qbvh_neighbors_range(const float *r_list_ij, int32_t *nlist, int32_t *n_neigh, int32_t max_neigh, int64_t first, int64_t count);
 
@@ -222,6 +231,9 @@ int qbvh_morton_keys_noalloc(const float *pos, const int32_t *type, int64_t N, c
  * fp32 roundings of x_i + v_j, y - x' and the squared sum, so that no true pair is pruned.
  * Pure host arithmetic, needs no device.  box: HOST 6 floats as for qbvh_build.  Returns < 0 on bad arguments. */
 float qbvh_padded_radius(float r, const float *box);
+/* Its square rounded UP to fp32: the right-hand side d2 <= R2 of the sphere/box test of eq. 2 as the
+ * traversal kernels receive it (rounding it any other way could prune a box the padded sphere touches).  Host only. */
+float qbvh_padded_radius_sq(float r, const float *box);
 
 typedef struct qbvh_stats {
     uint64_t node_tests;    /* sphere-AABB tests of Algorithm 1 line 12 (root tests of line 4 excluded)           */
@@ -242,7 +254,9 @@ typedef struct qbvh_stats {
 int qbvh_get_stats(qbvh_stats *out);
 
 /* Debug export of build products (for parity tests of steps a1..a6).  Copies min(bytes, available) bytes into
- * HOST memory `dst` after synchronising the stream; returns the number of bytes available, or < 0. */
+ * `dst` after synchronising the stream; returns the number of bytes available, or < 0.  dst: HOST memory; for the
+ * array products (KEYS_SORTED, PERM, NODES, PARENT, FRAMES, SORTED_POS) DEVICE memory works as well (a sharded run
+ * keeps the Z-order permutation on the GPU that way). */
 #define QBVH_EXPORT_KEYS_SORTED 1 /* uint32 [N]: type << 30 | 30-bit Morton code, ascending                       */
 #define QBVH_EXPORT_PERM 2        /* uint32 [N]: original index of the particle at sorted position k              */
 #define QBVH_EXPORT_NODES 3       /* int32 [2N-1][4] = {lo, hi, left, rope}; internal node i at i (Karras

@@ -24,6 +24,7 @@ struct Context {
     bool stats = false;
     int variant = 1;
     bool built = false;
+    int scan_spin_cycles = 1 << 18;   // ~130 us at 1.9 GHz; normal waits are a few us (QBVH_OPT_DEBUG_SCAN_SPIN)
     bool enqueued = false;       // a qbvh_neighbors_enqueue whose result has not been taken
     bool counters_armed = false; // group_cursor, max_count, warps_done of the tree are zero (after a build, after a production traversal)
     int32_t *pinned_dev = nullptr;   // device-side address of `pinned`
@@ -177,8 +178,12 @@ int make_params(const RT *r_list, bool f64, TraverseParams &P) {
 template <typename RT>
 int neighbors_impl(const RT *r_list, bool f64, int32_t *nlist, int32_t *n_neigh, int32_t max_neigh, int64_t q_first = 0,
                    int64_t q_count = -1) {
+    g.enqueued = false;              // whatever was enqueued before: its result words are about to be overwritten
     if (!g.built) return QBVH_ERR_NOT_BUILT;
     if (!r_list || max_neigh < 0) return QBVH_ERR_INVALID_ARG;
+    // The census of QBVH_OPT_STATS walks once per particle and writes all N rows: a range call's buffers hold only
+    // `count` rows, so the two do not combine.
+    if (q_count >= 0 && g.stats) return QBVH_ERR_INVALID_ARG;
     if (f64 != g.f64_built) return QBVH_ERR_INVALID_ARG;          // qbvh_build_f64 pairs with qbvh_neighbors_f64
     if (f64 && g.variant != 1) return QBVH_ERR_INVALID_ARG;       // Algorithm 1 as printed (variant 0) is the fp32 path
     if (g.N > 0 && (!n_neigh || (!nlist && max_neigh > 0))) return QBVH_ERR_INVALID_ARG;
@@ -227,12 +232,20 @@ int neighbors_impl(const RT *r_list, bool f64, int32_t *nlist, int32_t *n_neigh,
 int finish_neighbors() {
     cudaError_t e = cudaStreamSynchronize(g.stream);
     if (e != cudaSuccess) return cuda_fail(e, "stream synchronize");
-    if (g.pinned[1] & 1) return QBVH_ERR_TYPE_RANGE;
-    if (g.pinned[1] & 2) return QBVH_ERR_INTERNAL;
+    const int32_t flags = g.pinned[1];
+    if (flags & 2) {
+        // the bound violation belongs to this call only: take bit 1 back out of the tree's flag word (bit 0, set by
+        // the build, stays) so that the next traversal of the same tree reports its own outcome
+        const int32_t keep = flags & 1;
+        e = cudaMemcpy(&g.buf.meta->err_flags, &keep, sizeof(keep), cudaMemcpyHostToDevice);
+        if (e != cudaSuccess) return cuda_fail(e, "clear err_flags");
+    }
+    if (flags & 1) return QBVH_ERR_TYPE_RANGE;
+    if (flags & 2) return QBVH_ERR_INTERNAL;
     return g.pinned[0];
 }
 
-int build_impl(const void *pos, bool f64, const int32_t *type, int64_t N, const float *box) {
+int build_impl(const void *pos, bool f64, const int32_t *type, int64_t N, const float *box, const double *box64 = nullptr) {
     g.built = false;
     g.enqueued = false;
     if (N < 0 || N >= (int64_t(1) << 30) || !box || (N > 0 && !pos)) return QBVH_ERR_INVALID_ARG;
@@ -269,6 +282,7 @@ int build_impl(const void *pos, bool f64, const int32_t *type, int64_t N, const 
     g.buf.entry = reinterpret_cast<int32_t *>(w + L.entry);
     g.buf.scratch = reinterpret_cast<unsigned char *>(w + L.scratch);
     std::memcpy(g.box, box, sizeof(g.box));
+    if (box64) std::memcpy(g.box64, box64, sizeof(g.box64));      // only once the arguments have been accepted
     BuildParams bp{};
     for (int d = 0; d < 3; ++d) {
         volatile float s = 1023.0f / box[3 + d];   // fp32 RN
@@ -281,6 +295,7 @@ int build_impl(const void *pos, bool f64, const int32_t *type, int64_t N, const 
     bp.K = g.K;
     bp.lvl = pick_cell_level(N, bp.T);
     bp.f64 = f64;
+    bp.scan_spin_cycles = g.scan_spin_cycles;
     for (int t = 0; t < QBVH_TMAX; ++t) bp.r_hint[t] = g.r_hint[t];
     // The meeting slots of the top-level walk carry an 18-bit build number and the cell counters are counted back to
     // zero by every build: both are cleared only when the layout moves or the number wraps.
@@ -295,7 +310,13 @@ int build_impl(const void *pos, bool f64, const int32_t *type, int64_t N, const 
     }
     bp.build_tag = ++g.build_tag;
     cudaError_t e = launch_build(pos, type, bp, g.buf, g.stream);
-    if (e != cudaSuccess) return cuda_fail(e, "build launch");
+    if (e != cudaSuccess) {
+        // some of the five launches may have run: the cell counters are not known to be back at zero and slots may
+        // carry this build's tag — the next build on this workspace clears both
+        g.build_tag = 0;
+        g.tag_N = -1;
+        return cuda_fail(e, "build launch");
+    }
     g.N = N;
     g.K_built = g.K;
     g.f64_built = f64;
@@ -355,6 +376,10 @@ int qbvh_set_option(int32_t key, int32_t value) {
             if (value < 1 || value > (int32_t)QBVH_TAG_MAX || (uint32_t)value <= g.build_tag) return QBVH_ERR_INVALID_ARG;
             if (g.build_tag != 0) g.build_tag = (uint32_t)value - 1;   // a slot area still to be cleared stays at tag 0
             return QBVH_OK;
+        case QBVH_OPT_DEBUG_SCAN_SPIN:
+            if (value < 0) return QBVH_ERR_INVALID_ARG;
+            g.scan_spin_cycles = value;
+            return QBVH_OK;
         default:
             return QBVH_ERR_INVALID_ARG;
     }
@@ -366,6 +391,7 @@ int qbvh_get_option(int32_t key) {
         case QBVH_OPT_STATS: return g.stats ? 1 : 0;
         case QBVH_OPT_VARIANT: return g.variant;
         case QBVH_OPT_DEBUG_BUILD_TAG: return (int)g.build_tag;
+        case QBVH_OPT_DEBUG_SCAN_SPIN: return g.scan_spin_cycles;
         default: return QBVH_ERR_INVALID_ARG;
     }
 }
@@ -417,8 +443,7 @@ int qbvh_build_f64(const double *pos, const int32_t *type, int64_t N, const doub
         if (!std::isfinite(box[d])) return QBVH_ERR_INVALID_ARG;
         box32[d] = (float)box[d];                     // the tree lives in fp32: Morton bins and frames from rounded values
     }
-    std::memcpy(g.box64, box, sizeof(g.box64));
-    return build_impl(pos, true, type, N, box32);
+    return build_impl(pos, true, type, N, box32, box);
 }
 
 int qbvh_neighbors_f64(const double *r_list_ij, int32_t *nlist, int32_t *n_neigh, int32_t max_neigh) {
@@ -428,6 +453,7 @@ int qbvh_neighbors_f64(const double *r_list_ij, int32_t *nlist, int32_t *n_neigh
 }
 
 int qbvh_count_overlaps(const float *r_list_ij, int32_t *n_overlap) {
+    g.enqueued = false;
     if (!g.built) return QBVH_ERR_NOT_BUILT;
     if (!r_list_ij || (g.N > 0 && !n_overlap)) return QBVH_ERR_INVALID_ARG;
     TraverseParams P{};
@@ -545,6 +571,11 @@ float qbvh_padded_radius(float r, const float *box) {
     return padded_radius(r, box);
 }
 
+float qbvh_padded_radius_sq(float r, const float *box) {
+    const float rp = qbvh_padded_radius(r, box);
+    return rp < 0.0f ? -1.0f : mul_ru(rp, rp);        // exactly what make_params stores in TraverseParams::R2
+}
+
 int qbvh_get_stats(qbvh_stats *out) {
     if (!out) return QBVH_ERR_INVALID_ARG;
     *out = g.last_stats;
@@ -590,7 +621,7 @@ int64_t qbvh_debug_export(int32_t what, void *dst, int64_t bytes) {
         return avail;
     }
     if (n > 0) {
-        e = cudaMemcpy(dst, src, (size_t)n, cudaMemcpyDeviceToHost);
+        e = cudaMemcpy(dst, src, (size_t)n, cudaMemcpyDefault);     // dst: host or device (unified addressing)
         if (e != cudaSuccess) return cuda_fail(e, "export copy");
     }
     return avail;

@@ -230,13 +230,14 @@ __device__ void finalize_block(TreeMeta *__restrict__ meta, const uint32_t *__re
 
 // One tile of SCAN_TILE cells per block.  No chain between the tiles.  Up to SCAN_DIRECT_TILES tiles every block
 // simply adds up the counters of all tiles before its own (a few hundred KB out of L2) and nothing waits for anything;
-// beyond that every block publishes its tile's total and all blocks meet at a grid-wide barrier (at most
-// SCAN_MAX_TILES = 128 blocks: all resident at once).  The kernel is a handful of dependent L2 round trips.
+// beyond that every block publishes its tile's total and the blocks meet once (at most SCAN_MAX_TILES = 128 blocks,
+// normally all resident at once; the wait is bounded and falls back to the direct sum).  The kernel is a handful of
+// dependent L2 round trips.
 constexpr int SCAN_DIRECT_TILES = 32;
 __global__ void __launch_bounds__(SCAN_THREADS) cell_scan_kernel(const uint32_t *__restrict__ cell_count,
                                                                   uint32_t *__restrict__ cell_start,
                                                                   uint32_t *__restrict__ cell_list, int ncells,
-                                                                  TreeMeta *__restrict__ meta) {
+                                                                  TreeMeta *__restrict__ meta, long long spin_cycles) {
     cudaGridDependencySynchronize();
     __shared__ unsigned long long s_warp[SCAN_THREADS / 32], s_pre[SCAN_THREADS / 32];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -282,16 +283,33 @@ __global__ void __launch_bounds__(SCAN_THREADS) cell_scan_kernel(const uint32_t 
         excl += s_pre[w];
     }
     if (ntiles > SCAN_DIRECT_TILES) {
+        // The blocks meet once: each publishes its tile's total and waits until all have.  Blocks of an ordinary launch
+        // are not promised to be resident together (a busy or partitioned device), so the wait is bounded: a block that
+        // has not seen everybody after spin_cycles adds up the counters before its tile itself, as the small grids do —
+        // the same sum, never a hang.
         volatile unsigned long long *tot = meta->scan_status;
+        __shared__ int s_met;
         if (tid == 0) {
             tot[tile] = total;
             __threadfence();
             atomicAdd(&meta->scan_arrived, 1u);
-            while (*(volatile uint32_t *)&meta->scan_arrived < (uint32_t)ntiles) {}
+            const long long t0 = clock64();
+            bool met = false;
+            while (!(met = *(volatile uint32_t *)&meta->scan_arrived >= (uint32_t)ntiles) && clock64() - t0 < spin_cycles) {}
             __threadfence();
+            s_met = met ? 1 : 0;
         }
         __syncthreads();
-        unsigned long long v = (tid < tile) ? tot[tid] : 0ull;     // ntiles <= 128 <= SCAN_THREADS
+        unsigned long long v = 0ull;
+        if (s_met) {
+            v = (tid < tile) ? tot[tid] : 0ull;     // ntiles <= 128 <= SCAN_THREADS
+        } else {
+            const uint4 *src = reinterpret_cast<const uint4 *>(cell_count);
+            for (int q = tid; q < tile * (SCAN_TILE / 4); q += SCAN_THREADS) {
+                const uint4 c = __ldcg(src + q);
+                v += value(c.x) + value(c.y) + value(c.z) + value(c.w);
+            }
+        }
 #pragma unroll
         for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, o);
         __syncthreads();
@@ -1164,7 +1182,8 @@ cudaError_t launch_build(const void *pos, const int32_t *type, const BuildParams
     fp.N = N, fp.T = p.T, fp.lvl = lvl, fp.warp_slots = traverse_warp_slots();
     for (int t = 0; t < QBVH_TMAX; ++t) fp.r_hint[t] = p.r_hint[t];
     const int tiles = (ncells + SCAN_TILE - 1) / SCAN_TILE;
-    err = launch_dependent(cell_scan_kernel, dim3(tiles), dim3(SCAN_THREADS), 0, st, b.cell_count, b.cell_start, b.cell_list, ncells, b.meta);
+    err = launch_dependent(cell_scan_kernel, dim3(tiles), dim3(SCAN_THREADS), 0, st, b.cell_count, b.cell_start, b.cell_list, ncells, b.meta,
+                           (long long)p.scan_spin_cycles);
     if (err != cudaSuccess) return err;
     err = launch_dependent(cell_scatter_kernel, dim3((N + 255) / 256), dim3(256), 0, st, b.key, b.rank, N, cell_shift, b.cell_start, b.ent,
                            b.cell_count, ncells, b.meta, fp);

@@ -152,6 +152,7 @@ struct BuildParams {
     float r_hint[QBVH_TMAX];       // <= 0: no collapse hint for that tree
     uint32_t build_tag;
     bool f64;                      // positions are double precision (qbvh_build_f64)
+    int scan_spin_cycles;          // how long a block of the 128-tile cell scan waits for the others before it sums alone
 };
 int pick_cell_level(int64_t N, int T);
 cudaError_t launch_build(const void *pos, const int32_t *type, const BuildParams &p, const BuildBuffers &b, cudaStream_t st);

@@ -19,7 +19,7 @@ ERR_INVALID_ARG, ERR_NOT_BUILT, ERR_WORKSPACE, ERR_CUTOFF_TOO_LARGE, ERR_TYPE_RA
 ERR_NOALLOC_LIMIT = -8
 NOALLOC_MAX_N = 1 << 22
 MAX_TYPES = 4
-OPT_LEAF_COLLAPSE, OPT_STATS, OPT_VARIANT, OPT_DEBUG_BUILD_TAG = 1, 2, 3, 4
+OPT_LEAF_COLLAPSE, OPT_STATS, OPT_VARIANT, OPT_DEBUG_BUILD_TAG, OPT_DEBUG_SCAN_SPIN = 1, 2, 3, 4, 5
 EXPORT_KEYS_SORTED, EXPORT_PERM, EXPORT_NODES, EXPORT_PARENT, EXPORT_FRAMES, EXPORT_SEGMENTS, EXPORT_SORTED_POS, EXPORT_COUNTS = range(1, 9)
 
 # every symbol include/qbvh.h declares
@@ -27,7 +27,7 @@ SYMBOLS = ("qbvh_set_stream", "qbvh_set_num_types", "qbvh_workspace_bytes", "qbv
            "qbvh_set_option", "qbvh_get_option", "qbvh_build", "qbvh_neighbors", "qbvh_count_overlaps", "qbvh_staging_bytes",
            "qbvh_set_staging", "qbvh_build_host", "qbvh_neighbors_host", "qbvh_get_stats", "qbvh_debug_export",
            "qbvh_error_string", "qbvh_padded_radius", "qbvh_set_collapse_hint", "qbvh_build_f64", "qbvh_neighbors_f64", "qbvh_last_d2h_bytes", "qbvh_neighbors_range",
-           "qbvh_neighbors_enqueue", "qbvh_neighbors_result", "qbvh_morton_keys_noalloc")
+           "qbvh_neighbors_enqueue", "qbvh_neighbors_result", "qbvh_morton_keys_noalloc", "qbvh_padded_radius_sq")
 
 
 class QbvhStats(C.Structure):
@@ -77,6 +77,8 @@ _lib.qbvh_debug_export.restype = _i64
 _lib.qbvh_padded_radius.argtypes = [C.c_float, _vp]
 _lib.qbvh_padded_radius.restype = C.c_float
 _lib.qbvh_morton_keys_noalloc.argtypes = [_vp, _vp, _i64, _vp, _i32, _vp, _vp, _vp, _vp]
+_lib.qbvh_padded_radius_sq.argtypes = [C.c_float, _vp]
+_lib.qbvh_padded_radius_sq.restype = C.c_float
 _lib.qbvh_error_string.argtypes = [C.c_int]
 _lib.qbvh_error_string.restype = C.c_char_p
 
@@ -251,6 +253,15 @@ def qbvh_morton_keys_noalloc(pos, type, N: int, box, T: int, keys, frames, statu
                                                 _ptr(status), cuda_stream), "qbvh_morton_keys_noalloc")
 
 
+def qbvh_padded_radius_sq(r: float, box) -> float:
+    """Host arithmetic only: the squared padded pruning radius, rounded up, as the kernels receive it."""
+    box = _host_f32(box, 6)
+    v = float(_lib.qbvh_padded_radius_sq(C.c_float(float(r)), box.ctypes.data))
+    if v < 0:
+        raise QbvhError(ERR_INVALID_ARG, "qbvh_padded_radius_sq")
+    return v
+
+
 def qbvh_last_d2h_bytes() -> int:
     return int(_lib.qbvh_last_d2h_bytes())
 
@@ -272,6 +283,13 @@ def qbvh_debug_export(what: int, N: int) -> np.ndarray:
     avail = _check(_lib.qbvh_debug_export(what, out.ctypes.data, out.nbytes), "qbvh_debug_export")
     assert avail == out.nbytes, (avail, out.nbytes)
     return out
+
+
+def qbvh_debug_export_into(what: int, dst) -> int:
+    """Array build products (EXPORT_KEYS_SORTED, PERM, NODES, PARENT, FRAMES, SORTED_POS) copied into an existing tensor
+    or array `dst`, on the host or on the device; returns the bytes available."""
+    nbytes = dst.nbytes if isinstance(dst, np.ndarray) else dst.numel() * dst.element_size()
+    return _check(_lib.qbvh_debug_export(what, _ptr(dst), nbytes), "qbvh_debug_export")
 
 
 # ---------------------------------------------------------------------------------------------------------

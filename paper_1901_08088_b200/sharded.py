@@ -59,8 +59,11 @@ class CudaBackend:
         self.torch, self.qbvh, self.device = torch, qbvh, torch.device(device)
         self.N, self.T, self.max_neigh = N, T, max_neigh
         self.inner = qbvh.NeighborList(N, T=T, max_neigh=1, device=device)     # owns the workspace; lists are per slice
+        self.perm = torch.empty(max(N, 1), dtype=torch.int32, device=self.device)   # Z-order permutation, kept on the GPU
+        self.perm_valid = False
 
     def build(self, pos, type, box):
+        self.perm_valid = False
         return self.inner.build(pos, type, box)
 
     def neighbors_range(self, r_list, first: int, count: int):
@@ -72,8 +75,10 @@ class CudaBackend:
             self.max_neigh = int((M + 7) // 8 * 8)
             nlist = torch.empty((max(count, 1), self.max_neigh), dtype=torch.int32, device=self.device)
             M = qbvh.qbvh_neighbors_range(r_list, nlist, n_neigh, self.max_neigh, first, count)
-        perm = torch.from_numpy(qbvh.qbvh_debug_export(qbvh.EXPORT_PERM, self.N)[first:first + count].astype(np.int64))
-        return perm, n_neigh[:count], nlist[:count], M
+        if not self.perm_valid:                                                # once per build, device to device
+            qbvh.qbvh_debug_export_into(qbvh.EXPORT_PERM, self.perm)
+            self.perm_valid = True
+        return self.perm[first:first + count].to(torch.int64), n_neigh[:count], nlist[:count], M
 
 
 class ShardedNeighborList:
@@ -90,25 +95,43 @@ class ShardedNeighborList:
         self.own_first, self.own_count = owned_block(self.N, self.world, self.rank)
         self.first, self.count = slice_bounds(self.N, self.world, self.rank)
         self.backend = backend if backend is not None else CudaBackend(self.N, self.T, max_neigh, device)
+        self._gather_bufs = {}
 
-    def all_gather_rows(self, local):
-        """All-gather of per-rank row blocks of unequal length (padded to the longest block: one collective)."""
+    def all_gather_rows(self, local, name="rows"):
+        """All-gather of the ranks' row blocks into ONE persistent tensor per `name` (the build's input: nothing is
+        allocated per step).  Equal blocks (world divides N): the collective writes straight into it.  Unequal blocks
+        (they differ by one row): the collective needs equal pieces, so it lands in a padded persistent buffer and the
+        blocks are copied into place."""
         torch, dist = self.torch, self.dist
         if self.world == 1:
             return local
-        longest = max(owned_block(self.N, self.world, r)[1] for r in range(self.world))
-        padded = torch.zeros((longest,) + tuple(local.shape[1:]), dtype=local.dtype, device=local.device)
-        padded[: local.shape[0]] = local
-        out = torch.empty((self.world * longest,) + tuple(local.shape[1:]), dtype=local.dtype, device=local.device)
-        dist.all_gather_into_tensor(out, padded, group=self.group)
-        chunks = [out[r * longest: r * longest + owned_block(self.N, self.world, r)[1]] for r in range(self.world)]
-        return torch.cat(chunks, dim=0)
+        key = (name, local.dtype, tuple(local.shape[1:]))
+        bufs = self._gather_bufs.get(key)
+        if bufs is None:
+            full = torch.empty((self.N,) + tuple(local.shape[1:]), dtype=local.dtype, device=local.device)
+            longest = max(owned_block(self.N, self.world, r)[1] for r in range(self.world))
+            padded = None
+            if self.N % self.world:
+                padded = (torch.zeros((longest,) + tuple(local.shape[1:]), dtype=local.dtype, device=local.device),
+                          torch.empty((self.world * longest,) + tuple(local.shape[1:]), dtype=local.dtype, device=local.device))
+            bufs = self._gather_bufs[key] = (full, longest, padded)
+        full, longest, padded = bufs
+        if padded is None:
+            dist.all_gather_into_tensor(full, local, group=self.group)
+            return full
+        mine, everyone = padded
+        mine[: local.shape[0]] = local
+        dist.all_gather_into_tensor(everyone, mine, group=self.group)
+        for r in range(self.world):
+            first, count = owned_block(self.N, self.world, r)
+            full[first:first + count] = everyone[r * longest: r * longest + count]
+        return full
 
     def build(self, pos_local, type_local, box):
         """pos_local: this rank's (own_count, 3) block.  All-gathers, then builds the full tree on every rank."""
         assert tuple(pos_local.shape) == (self.own_count, 3)
-        self.pos = self.all_gather_rows(pos_local.contiguous())
-        self.type = None if type_local is None else self.all_gather_rows(type_local.contiguous())
+        self.pos = self.all_gather_rows(pos_local.contiguous(), "pos")
+        self.type = None if type_local is None else self.all_gather_rows(type_local.contiguous(), "type")
         return self.backend.build(self.pos, self.type, box)
 
     def neighbors(self, r_list):

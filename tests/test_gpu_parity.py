@@ -46,28 +46,33 @@ def collapse_frontier(t, K, r_hint=None):
                     delta = np.float32(t.frames[tb, 6 + d])
                     rb[tb, d] = min(int(np.ceil(np.float32(r_hint[tb]) / delta)), 1023) if delta > 0 else 1
 
-    def W(n):
+    def Wv(n):                                     # swollen-volume weight of nodes n (int64 array)
         r = rb[tree_of[n]]
-        return int((ext[n, 0] + 2 * r[0]) * (ext[n, 1] + 2 * r[1]) * (ext[n, 2] + 2 * r[2]))
+        return (ext[n, 0] + 2 * r[:, 0]) * (ext[n, 1] + 2 * r[:, 1]) * (ext[n, 2] + 2 * r[:, 2])
+
+    def leaf_cost(m):
+        return Wv(m) * (C_LEAF_FIXED + C_LEAF_PER_PARTICLE * size[m])
 
     if K > 1:
-        cand = np.nonzero((np.arange(M) < N - 1) & (size >= 2) & (size <= K))[0]
-        for n in cand[np.argsort(size[cand], kind="stable")]:           # children before parents
+        internal = np.arange(M) < N - 1
+        for s in range(2, K + 1):                  # children (fewer particles) before parents; one size class at a time
+            n = np.nonzero(internal & (size == s))[0]
+            if len(n) == 0:
+                continue
             a, b = t.left[n], t.right[n]
-            ok = pend[a] and pend[b]
-            if ok and rb is not None and rb[tree_of[n], 0] >= 0:
-                leaf = lambda m: W(m) * (C_LEAF_FIXED + C_LEAF_PER_PARTICLE * int(size[m]))
-                ok = leaf(n) <= W(n) * C_NODE + leaf(a) + leaf(b)
+            ok = pend[a] & pend[b]
+            if rb is not None:
+                hinted = rb[tree_of[n], 0] >= 0
+                cheaper = leaf_cost(n) <= Wv(n) * C_NODE + leaf_cost(a) + leaf_cost(b)
+                ok &= np.where(hinted, cheaper, True)
             pend[n] = coll[n] = ok
-    # top down: a node exists iff no proper ancestor collapsed
+    # top down, level by level: a node exists iff no proper ancestor collapsed
     emitted = np.zeros(M, bool)
-    stack = [int(r) for r in t.roots if r >= 0]
-    while stack:
-        n = stack.pop()
-        emitted[n] = True
-        if n < N - 1 and not coll[n]:
-            stack.append(int(t.left[n]))
-            stack.append(int(t.right[n]))
+    frontier = np.array([int(r) for r in t.roots if r >= 0], np.int64)
+    while len(frontier):
+        emitted[frontier] = True
+        inner = frontier[(frontier < N - 1) & ~coll[frontier]]
+        frontier = np.concatenate([t.left[inner], t.right[inner]]).astype(np.int64)
     return emitted, coll
 
 
@@ -106,6 +111,19 @@ def check_build(w, K, r_hint=None):
 @pytest.mark.parametrize("cid", [1, 2, 3, 4, 5])
 def test_build_parity_small(cid, K):
     check_build(W.make_config(cid, small=True), K)
+
+
+@pytest.mark.parametrize("cid,K,hinted", [(2, 1, False), (2, 32, False), (2, 32, True), (3, 1, False), (3, 32, False),
+                                          (5, 1, False), (5, 32, False)])
+def test_build_parity_full_size(cid, K, hinted):
+    """The build the benchmark times, bit for bit against the oracle tree (steps a1..a6 + the collapse): BASELINE.json
+    sizes reach what the small cases cannot — Morton-cell levels 5 (configs 2, 3) and 6 (config 5), at level 6 the
+    128-tile scan with its grid-wide meeting point, and at K = 32 the top-down split of the nodes above the range
+    leaves (taken once N >= 32 x the resident warps of the traversal)."""
+    w = W.make_config(cid)
+    hint = np.asarray(w.r_list, np.float32).reshape(w.T, w.T).max(axis=0) if hinted else None
+    out, t = check_build(w, K, r_hint=hint)
+    assert int(out["counts"][3]) == (6 if cid == 5 else 5)
 
 
 @pytest.mark.parametrize("N", [1, 2, 3, 31, 32, 33, 255, 4095, 4096, 4097, 8193, 70001])
@@ -639,7 +657,7 @@ def test_query_sharding_slices_merge_to_the_oracle(cid, world):
     for g in range(world):
         first, count = sharded.slice_bounds(w.N, world, g)
         rows, n_neigh, nlist, M = be.neighbors_range(w.r_list, first, count)
-        parts.append((rows.numpy(), n_neigh.cpu().numpy(), nlist.cpu().numpy()))
+        parts.append((rows.cpu().numpy(), n_neigh.cpu().numpy(), nlist.cpu().numpy()))
         assert M == (int(n_neigh.max().item()) if count else 0)
     n_all, l_all = sharded.merge_slices(w.N, parts)
     out = {"M": int(n_all.max()), "max_neigh": l_all.shape[1], "nlist": l_all, "n_neigh": n_all}
@@ -648,8 +666,35 @@ def test_query_sharding_slices_merge_to_the_oracle(cid, world):
     snl = sharded.ShardedNeighborList(w.N, T=w.T, max_neigh=w.max_neigh, device=dev)
     snl.build(torch.from_numpy(w.pos).to(dev), None if w.type is None else torch.from_numpy(w.type).to(dev), w.box)
     rows, n_neigh, nlist, M = snl.neighbors(w.r_list)
-    n1, l1 = sharded.merge_slices(w.N, [(rows.numpy(), n_neigh.cpu().numpy(), nlist.cpu().numpy())])
+    n1, l1 = sharded.merge_slices(w.N, [(rows.cpu().numpy(), n_neigh.cpu().numpy(), nlist.cpu().numpy())])
     assert np.array_equal(n1, n_all)
+
+
+@pytest.mark.parametrize("K,hinted", [(8, False), (1, False), (32, True)])
+def test_query_sharding_on_other_builds(K, hinted):
+    """qbvh_neighbors_range on trees other than the default K = 32 one: smaller range leaves (other tile widths of the
+    traversal), the paper's one-particle leaves, and a build with the collapse hint."""
+    import torch
+    from paper_1901_08088_b200 import qbvh, sharded
+    w = W.make_config(3, small=True)
+    dev = torch.device("cuda:0")
+    qbvh.qbvh_set_option(qbvh.OPT_LEAF_COLLAPSE, K)
+    qbvh.qbvh_set_option(qbvh.OPT_STATS, 0)
+    qbvh.qbvh_set_collapse_hint(np.asarray(w.r_list, np.float32).reshape(w.T, w.T).max(axis=0) if hinted else None)
+    try:
+        be = sharded.CudaBackend(w.N, w.T, w.max_neigh, dev)
+        be.build(torch.from_numpy(w.pos).to(dev), torch.from_numpy(w.type).to(dev), w.box)
+        parts = []
+        for g in range(3):
+            first, count = sharded.slice_bounds(w.N, 3, g)
+            rows, n_neigh, nlist, M = be.neighbors_range(w.r_list, first, count)
+            parts.append((rows.cpu().numpy(), n_neigh.cpu().numpy(), nlist.cpu().numpy()))
+    finally:
+        qbvh.qbvh_set_collapse_hint(None)
+        qbvh.qbvh_set_option(qbvh.OPT_LEAF_COLLAPSE, 32)
+    n_all, l_all = sharded.merge_slices(w.N, parts)
+    out = {"M": int(n_all.max()), "max_neigh": l_all.shape[1], "nlist": l_all, "n_neigh": n_all}
+    compare_with_oracle(w, out, ON.neighbor_list(w.pos, w.type, w.box, w.r_list))
 
 
 @pytest.mark.parametrize("N,T,lvl", [(1, 1, 2), (3072, 1, 2), (3073, 1, 3), (200_000, 1, 5), (200_000, 4, 5), (1_600_000, 1, 6), (1_600_000, 2, 5)])

@@ -1,0 +1,130 @@
+"""-m gpu regression tests for findings of the round-2 review: argument combinations and call sequences
+that the parity tests do not reach."""
+import numpy as np
+import pytest
+
+from oracle import neighbors as ON
+from paper_1901_08088_b200 import workloads as W
+
+from gpu_util import compare_with_oracle
+
+pytestmark = pytest.mark.gpu
+
+
+def _built(w, max_neigh=None, K=32):
+    import torch
+    from paper_1901_08088_b200 import qbvh
+    dev = torch.device("cuda:0")
+    qbvh.qbvh_set_option(qbvh.OPT_LEAF_COLLAPSE, K)
+    qbvh.qbvh_set_option(qbvh.OPT_STATS, 0)
+    qbvh.qbvh_set_option(qbvh.OPT_VARIANT, 1)
+    qbvh.qbvh_set_collapse_hint(None)
+    nl = qbvh.NeighborList(w.N, T=w.T, max_neigh=w.max_neigh if max_neigh is None else max_neigh, device=dev)
+    nl.build(torch.from_numpy(w.pos).to(dev), None if w.type is None else torch.from_numpy(w.type).to(dev), w.box)
+    return nl
+
+
+def test_range_call_refuses_the_census_and_leaves_its_buffers_alone():
+    """qbvh_neighbors_range hands the library buffers of `count` rows; the census of QBVH_OPT_STATS writes a row for
+    every one of the N particles.  The combination is refused (INVALID_ARG) before anything is enqueued: guard bands
+    around the slice's buffers stay intact.  With the option off again the same call works."""
+    import torch
+    from paper_1901_08088_b200 import qbvh
+    w = W.make_config(1)
+    nl = _built(w)
+    first, count, cap, guard = 1000, 200, w.max_neigh, 4096
+    lst = torch.full((guard + count * cap + guard,), -77, dtype=torch.int32, device=nl.device)
+    cnt = torch.full((guard + count + guard,), -77, dtype=torch.int32, device=nl.device)
+    try:
+        qbvh.qbvh_set_option(qbvh.OPT_STATS, 1)
+        with pytest.raises(qbvh.QbvhError) as e:
+            qbvh.qbvh_neighbors_range(w.r_list, lst[guard:], cnt[guard:], cap, first, count)
+        assert e.value.code == qbvh.ERR_INVALID_ARG
+        torch.cuda.synchronize()
+        assert torch.all(lst == -77) and torch.all(cnt == -77)
+    finally:
+        qbvh.qbvh_set_option(qbvh.OPT_STATS, 0)
+    M = qbvh.qbvh_neighbors_range(w.r_list, lst[guard:], cnt[guard:], cap, first, count)
+    torch.cuda.synchronize()
+    assert torch.all(lst[:guard] == -77) and torch.all(lst[guard + count * cap:] == -77)
+    assert torch.all(cnt[:guard] == -77) and torch.all(cnt[guard + count:] == -77)
+    assert M == int(cnt[guard:guard + count].max().item()) > 0
+
+
+def test_a_synchronous_call_drops_a_pending_enqueue():
+    """After qbvh_neighbors_enqueue, any synchronous neighbor call overwrites the result words: a later
+    qbvh_neighbors_result must say so (NOT_BUILT) instead of returning the other call's numbers."""
+    import torch
+    from paper_1901_08088_b200 import qbvh
+    w = W.make_config(1)
+    nl = _built(w)
+    n_over = torch.zeros(w.N, dtype=torch.int32, device=nl.device)
+    for sync_call in (lambda: nl.neighbors(w.r_list, retry=False),
+                      lambda: qbvh.qbvh_count_overlaps(w.r_list, n_over),
+                      lambda: qbvh.qbvh_neighbors_range(w.r_list, nl.nlist, nl.n_neigh, nl.max_neigh, 0, 10)):
+        nl.neighbors_enqueue(w.r_list)
+        sync_call()
+        with pytest.raises(qbvh.QbvhError) as e:
+            qbvh.qbvh_neighbors_result()
+        assert e.value.code == qbvh.ERR_NOT_BUILT
+    nl.neighbors_enqueue(w.r_list)                       # and the pair still works afterwards
+    assert nl.neighbors_result() == nl.neighbors(w.r_list, retry=False)
+
+
+def test_f64_box_that_is_not_representable_in_fp32():
+    """qbvh_build_f64 with box64 != (double)(float)box64: origin and lengths that are not fp32 numbers, particles on
+    the lower faces exactly and one ulp64 below the upper faces, partners across faces and a corner at r (1 -+ eps).
+    Their fp32 roundings fall on or outside the rounded box; the lists must still be the fp64 definition's."""
+    from test_gpu_parity import gpu_run_f64
+    rng = np.random.default_rng(11)
+    lo = np.array([0.1, -1.0 / 3.0, 1000.0 / 7.0])
+    L = np.array([10.1, 9.7, 11.3])
+    box64 = np.concatenate([lo, L])
+    assert np.any(box64 != box64.astype(np.float32).astype(np.float64))
+    hi_in = np.nextafter(lo + L, -np.inf)                          # the largest coordinates inside [lo, lo + L)
+    r = 1.3
+    pts = [lo.copy(), hi_in.copy()]
+    for d in range(3):                                            # one coordinate on a face, the others inside
+        for face in (lo[d], hi_in[d]):
+            for _ in range(4):
+                p = lo + rng.random(3) * L * 0.999
+                p[d] = face
+                pts.append(p)
+    base = list(pts)
+    for b in base:                                                # partners at r (1 -+ eps): across the face for most
+        for eps in (-1e-9, 1e-9, -2e-6, 2e-6):
+            u = rng.normal(size=3)
+            u /= np.linalg.norm(u)
+            q = b + r * (1 + eps) * u
+            q = lo + np.mod(q - lo, L)
+            pts.append(np.minimum(np.maximum(q, lo), hi_in))
+    pts.extend(lo + rng.random((3000, 3)) * L)                    # a fluid around them
+    pos64 = np.ascontiguousarray(np.array(pts))
+    assert np.all(pos64 >= lo) and np.all(pos64 < lo + L)
+    p32 = pos64.astype(np.float32)
+    b32 = box64.astype(np.float32)
+    assert np.any(p32 < b32[:3]) or np.any(p32 >= b32[:3] + b32[3:])     # the case the header allows and nothing covered
+    r64 = np.array([[r]])
+    for K in (1, 32):
+        out = gpu_run_f64(pos64, None, box64, r64, 1, 64, K=K)
+        rp, nb = ON.neighbor_list_f64(pos64, None, box64, r64, method="brute")
+        w = W.Workload("f64box", p32, None, b32, r64.astype(np.float32), 64)
+        rep = compare_with_oracle(w, out, (rp, nb, np.zeros(len(nb), np.uint8)))
+        assert rep["rows_checked"] == len(pos64) and rep["pairs"] > 10000
+
+
+def test_cell_scan_without_the_meeting_point():
+    """The 128-tile scan of the build (cell grid level 6) lets its blocks meet once, with a bounded wait; a block that
+    gives up sums the counters in front of its tile itself.  Forced here (wait of 0 cycles): the build must be the same,
+    bit for bit against the oracle tree, and the default is restored afterwards."""
+    from paper_1901_08088_b200 import qbvh
+    from test_gpu_parity import check_build
+    w = W.make_config(5)
+    default = qbvh.qbvh_get_option(qbvh.OPT_DEBUG_SCAN_SPIN)
+    assert default > 0
+    try:
+        qbvh.qbvh_set_option(qbvh.OPT_DEBUG_SCAN_SPIN, 0)
+        out, t = check_build(w, 32)
+        assert int(out["counts"][3]) == 6
+    finally:
+        qbvh.qbvh_set_option(qbvh.OPT_DEBUG_SCAN_SPIN, default)

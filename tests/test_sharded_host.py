@@ -42,20 +42,23 @@ class OracleBackend:
         return torch.from_numpy(rows.astype(np.int64)), torch.from_numpy(cnt[rows].astype(np.int32)), torch.from_numpy(nlist), M
 
 
-def _workload():
+def _workload(N=1501):
     from paper_1901_08088_b200 import workloads as W
-    w = W.colloid_solvent(N=1501, n_colloid=7, seed=3)              # two types, three cutoffs, an N no world size divides
+    w = W.colloid_solvent(N=N, n_colloid=7, seed=3)                 # two types, three cutoffs; 1501: an N no world size divides
     return w
 
 
-def _worker(rank, world, port, out):
+def _worker(rank, world, port, out, N=1501):
     os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
     dist.init_process_group("gloo", rank=rank, world_size=world)
     from paper_1901_08088_b200 import sharded
-    w = _workload()
+    w = _workload(N)
     snl = sharded.ShardedNeighborList(w.N, T=w.T, max_neigh=8, device="cpu", backend=OracleBackend())
     lo, cnt = snl.own_first, snl.own_count
-    snl.build(torch.from_numpy(w.pos[lo:lo + cnt]), torch.from_numpy(w.type[lo:lo + cnt]), w.box)
+    snl.build(torch.from_numpy(w.pos[lo:lo + cnt] + 1.0), torch.from_numpy(w.type[lo:lo + cnt]), w.box)   # a first step ...
+    first_pos = snl.pos
+    snl.build(torch.from_numpy(w.pos[lo:lo + cnt]), torch.from_numpy(w.type[lo:lo + cnt]), w.box)         # ... and the next
+    assert snl.pos is first_pos                                      # gathered into the same persistent tensor, no new one per step
     gathered_ok = bool(np.array_equal(snl.pos.numpy(), w.pos) and np.array_equal(snl.type.numpy(), w.type))
     rows, n_neigh, nlist, M = snl.neighbors(w.r_list)
     out.put((rank, gathered_ok, snl.first, snl.count, rows.numpy(), n_neigh.numpy(), nlist.numpy(), M))
@@ -63,20 +66,20 @@ def _worker(rank, world, port, out):
     dist.destroy_process_group()
 
 
-@pytest.mark.parametrize("world,port", [(2, 29741), (3, 29743)])
-def test_sharded_slices_merge_to_the_full_list_gloo(world, port):
+@pytest.mark.parametrize("world,port,N", [(2, 29741, 1501), (3, 29743, 1501), (2, 29745, 1500)])   # 1500 / 2: equal blocks, gathered in place
+def test_sharded_slices_merge_to_the_full_list_gloo(world, port, N):
     from oracle import neighbors as ON
     from paper_1901_08088_b200 import sharded
     ctx = mp.get_context("spawn")
     out = ctx.Queue()
-    procs = [ctx.Process(target=_worker, args=(r, world, port, out)) for r in range(world)]
+    procs = [ctx.Process(target=_worker, args=(r, world, port, out, N)) for r in range(world)]
     for p in procs:
         p.start()
     res = sorted((out.get(timeout=180) for _ in range(world)), key=lambda t: t[0])
     for p in procs:
         p.join(timeout=60)
         assert p.exitcode == 0
-    w = _workload()
+    w = _workload(N)
     assert all(r[1] for r in res)                                               # the all-gather rebuilt pos and type
     assert [r[2] for r in res] == [sharded.slice_bounds(w.N, world, g)[0] for g in range(world)]
     assert sum(r[3] for r in res) == w.N and max(r[3] for r in res) - min(r[3] for r in res) <= 1
