@@ -248,16 +248,12 @@ def run_gpu(args):
         ev[s][0].record()
         nl.build(pos, typ, box)
         ev[s][1].record()
-        if f64:
-            nl.neighbors(r_list, retry=False)          # (the fp64 call has no enqueue form: its event follows the wait)
-            ev[s][2].record()
-        else:
-            # the traversal is enqueued, the closing event recorded behind it on the stream, and only then does the
-            # host wait for M: the events bracket the device work, not the host's wake-up after the synchronise
-            nl.neighbors_enqueue(r_list)
-            ev[s][2].record()
-            if nl.neighbors_result() > cap:
-                raise SystemExit("overflow inside the timed loop")
+        # the traversal is enqueued (fp32 or fp64 form), the closing event recorded behind it on the stream, and only then
+        # does the host wait for M: the events bracket the device work, not the host's wake-up after the synchronise
+        nl.neighbors_enqueue(r_list)
+        ev[s][2].record()
+        if nl.neighbors_result() > cap:
+            raise SystemExit("overflow inside the timed loop")
     torch.cuda.synchronize()
     wall = time.perf_counter() - wall0
     if world > 1:
@@ -421,10 +417,11 @@ def run_sharded(args):
 
     def step():
         snl.build(pos, typ, w.box)
-        return qbvh.qbvh_neighbors_range(w.r_list, nlist, n_neigh, w.max_neigh, snl.first, snl.count)
+        qbvh.qbvh_neighbors_range_enqueue(w.r_list, nlist, n_neigh, w.max_neigh, snl.first, snl.count)
 
     for _ in range(max(args.warmup, 3)):
         step()
+        qbvh.qbvh_neighbors_result()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     if world > 1:
         dist.barrier()
@@ -432,7 +429,9 @@ def run_sharded(args):
     e0.record()
     for _ in range(args.steps):
         step()
-    e1.record()
+    e1.record()                                        # behind the last traversal on the stream, before the host waits for it
+    if qbvh.qbvh_neighbors_result() > w.max_neigh:
+        raise SystemExit("overflow inside the timed loop")
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()

@@ -138,6 +138,10 @@ int qbvh_neighbors(const float *r_list_ij, int32_t *nlist, int32_t *n_neigh, int
  * qbvh_neighbors is exactly enqueue followed by result. */
 int qbvh_neighbors_enqueue(const float *r_list_ij, int32_t *nlist, int32_t *n_neigh, int32_t max_neigh);
 int qbvh_neighbors_result(void);
+/* The enqueue halves of qbvh_neighbors_f64 and qbvh_neighbors_range (declared below; same arguments, same
+ * qbvh_neighbors_result afterwards). */
+int qbvh_neighbors_f64_enqueue(const double *r_list_ij, int32_t *nlist, int32_t *n_neigh, int32_t max_neigh);
+int qbvh_neighbors_range_enqueue(const float *r_list_ij, int32_t *nlist, int32_t *n_neigh, int32_t max_neigh, int64_t first, int64_t count);
 
 /* Query sharding ("straightforwardly generalized to execute on multiple GPUs"): the
  * same traversal for the particles at sorted (Z-order) positions [first, first + count) only.  Row k of nlist and

@@ -423,6 +423,19 @@ int qbvh_neighbors_enqueue(const float *r_list_ij, int32_t *nlist, int32_t *n_ne
     return rc;
 }
 
+int qbvh_neighbors_f64_enqueue(const double *r_list_ij, int32_t *nlist, int32_t *n_neigh, int32_t max_neigh) {
+    int rc = neighbors_impl(r_list_ij, true, nlist, n_neigh, max_neigh);
+    g.enqueued = rc == QBVH_OK;
+    return rc;
+}
+
+int qbvh_neighbors_range_enqueue(const float *r_list_ij, int32_t *nlist, int32_t *n_neigh, int32_t max_neigh, int64_t first, int64_t count) {
+    if (count < 0) return QBVH_ERR_INVALID_ARG;
+    int rc = neighbors_impl(r_list_ij, false, nlist, n_neigh, max_neigh, first, count);
+    g.enqueued = rc == QBVH_OK;
+    return rc;
+}
+
 int qbvh_neighbors_result(void) {
     if (!g.enqueued) return QBVH_ERR_NOT_BUILT;
     g.enqueued = false;

@@ -27,7 +27,8 @@ SYMBOLS = ("qbvh_set_stream", "qbvh_set_num_types", "qbvh_workspace_bytes", "qbv
            "qbvh_set_option", "qbvh_get_option", "qbvh_build", "qbvh_neighbors", "qbvh_count_overlaps", "qbvh_staging_bytes",
            "qbvh_set_staging", "qbvh_build_host", "qbvh_neighbors_host", "qbvh_get_stats", "qbvh_debug_export",
            "qbvh_error_string", "qbvh_padded_radius", "qbvh_set_collapse_hint", "qbvh_build_f64", "qbvh_neighbors_f64", "qbvh_last_d2h_bytes", "qbvh_neighbors_range",
-           "qbvh_neighbors_enqueue", "qbvh_neighbors_result", "qbvh_morton_keys_noalloc", "qbvh_padded_radius_sq")
+           "qbvh_neighbors_enqueue", "qbvh_neighbors_result", "qbvh_morton_keys_noalloc", "qbvh_padded_radius_sq",
+           "qbvh_neighbors_f64_enqueue", "qbvh_neighbors_range_enqueue")
 
 
 class QbvhStats(C.Structure):
@@ -60,6 +61,8 @@ _lib.qbvh_build.argtypes = [_vp, _vp, _i64, _vp]
 _lib.qbvh_neighbors.argtypes = [_vp, _vp, _vp, _i32]
 _lib.qbvh_neighbors_enqueue.argtypes = [_vp, _vp, _vp, _i32]
 _lib.qbvh_neighbors_result.argtypes = []
+_lib.qbvh_neighbors_f64_enqueue.argtypes = [_vp, _vp, _vp, _i32]
+_lib.qbvh_neighbors_range_enqueue.argtypes = [_vp, _vp, _vp, _i32, _i64, _i64]
 _lib.qbvh_count_overlaps.argtypes = [_vp, _vp]
 _lib.qbvh_neighbors_range.argtypes = [_vp, _vp, _vp, _i32, _i64, _i64]
 _lib.qbvh_build_f64.argtypes = [_vp, _vp, _i64, _vp]
@@ -179,6 +182,21 @@ def qbvh_neighbors_enqueue(r_list_ij, nlist, n_neigh, max_neigh: int) -> None:
     """qbvh_neighbors without the wait: the traversal is enqueued on the stream; take M with qbvh_neighbors_result."""
     r = _r_list(r_list_ij)
     _check(_lib.qbvh_neighbors_enqueue(r.ctypes.data, _ptr(nlist), _ptr(n_neigh), max_neigh), "qbvh_neighbors_enqueue")
+
+
+def qbvh_neighbors_f64_enqueue(r_list_ij, nlist, n_neigh, max_neigh: int) -> None:
+    """qbvh_neighbors_f64 without the wait; M comes from qbvh_neighbors_result."""
+    r = np.ascontiguousarray(r_list_ij, dtype=np.float64)
+    if r.size != _num_types * _num_types:
+        raise ValueError(f"r_list_ij holds {r.size} values; qbvh_set_num_types({_num_types}) needs {_num_types}x{_num_types}")
+    _check(_lib.qbvh_neighbors_f64_enqueue(r.ctypes.data, _ptr(nlist), _ptr(n_neigh), max_neigh), "qbvh_neighbors_f64_enqueue")
+
+
+def qbvh_neighbors_range_enqueue(r_list_ij, nlist, n_neigh, max_neigh: int, first: int, count: int) -> None:
+    """qbvh_neighbors_range without the wait; the maximum over the range comes from qbvh_neighbors_result."""
+    r = _r_list(r_list_ij)
+    _check(_lib.qbvh_neighbors_range_enqueue(r.ctypes.data, _ptr(nlist), _ptr(n_neigh), max_neigh, first, count),
+           "qbvh_neighbors_range_enqueue")
 
 
 def qbvh_neighbors_result() -> int:
@@ -346,8 +364,9 @@ class NeighborList:
         return (qbvh_build_f64 if self.f64 else qbvh_build)(pos, type, self.N, box)
 
     def neighbors_enqueue(self, r_list) -> None:
-        """fp32 lists without the wait (qbvh_neighbors_enqueue); M comes from neighbors_result()."""
-        qbvh_neighbors_enqueue(r_list, self.nlist, self.n_neigh, self.max_neigh)
+        """Lists without the wait (qbvh_neighbors_enqueue / qbvh_neighbors_f64_enqueue); M comes from neighbors_result()."""
+        call = qbvh_neighbors_f64_enqueue if getattr(self, "f64", False) else qbvh_neighbors_enqueue
+        call(r_list, self.nlist, self.n_neigh, self.max_neigh)
 
     def neighbors_result(self) -> int:
         return qbvh_neighbors_result()

@@ -128,3 +128,30 @@ def test_cell_scan_without_the_meeting_point():
         assert int(out["counts"][3]) == 6
     finally:
         qbvh.qbvh_set_option(qbvh.OPT_DEBUG_SCAN_SPIN, default)
+
+
+def test_f64_and_range_enqueue_forms():
+    """qbvh_neighbors_f64_enqueue / qbvh_neighbors_range_enqueue + qbvh_neighbors_result give what the synchronous calls
+    give: M, counts, and the same rows as sets."""
+    import torch
+    from paper_1901_08088_b200 import qbvh
+    w = W.make_config(3, small=True)
+    nl = _built(w)
+    first, count, cap = 777, 5000, w.max_neigh
+    lst = [torch.full((count, cap), -1, dtype=torch.int32, device=nl.device) for _ in range(2)]
+    cnt = [torch.full((count,), -1, dtype=torch.int32, device=nl.device) for _ in range(2)]
+    M0 = qbvh.qbvh_neighbors_range(w.r_list, lst[0], cnt[0], cap, first, count)
+    qbvh.qbvh_neighbors_range_enqueue(w.r_list, lst[1], cnt[1], cap, first, count)
+    assert qbvh.qbvh_neighbors_result() == M0 and torch.equal(cnt[0], cnt[1])
+    a, b, c = lst[0].cpu().numpy(), lst[1].cpu().numpy(), cnt[0].cpu().numpy()
+    assert all(np.array_equal(np.sort(a[k, :c[k]]), np.sort(b[k, :c[k]])) for k in range(count))
+    pos64, box64, r64 = W.as_f64(w)
+    nl64 = qbvh.NeighborList(w.N, T=w.T, max_neigh=cap, device=nl.device)
+    nl64.build(torch.from_numpy(pos64).to(nl.device), torch.from_numpy(w.type).to(nl.device), box64)
+    M1 = nl64.neighbors(r64, retry=False)
+    ref = nl64.n_neigh.clone()
+    nl64.n_neigh.fill_(-1)
+    nl64.neighbors_enqueue(r64)                                    # the fp64 form: the object was built from fp64 positions
+    assert nl64.neighbors_result() == M1 and torch.equal(nl64.n_neigh, ref)
+    rp, nb = ON.neighbor_list_f64(pos64, w.type, box64, r64)
+    assert np.array_equal(ref.cpu().numpy()[: w.N], np.diff(rp))
