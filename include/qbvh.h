@@ -86,6 +86,15 @@ int qbvh_set_workspace(void *dev_ptr, int64_t bytes);
                                     counters in front of its tile itself (default 2^18, about 130 us; 0: never wait).
                                     Either way the result is the same; the bound only matters on a device too busy to
                                     hold all 128 blocks at once, where an unbounded wait could hang.               */
+#define QBVH_OPT_GROUP_MAX 6        /* v in [1,32], default 32: the largest query group (particles one warp of the production
+                                    traversal searches for together) the next build emits.  Smaller groups have
+                                    tighter search boxes (fewer candidates per member) but fill fewer lanes of their warp.
+                                    The lists do not depend on it.                                                 */
+#define QBVH_OPT_CELL_LEVEL 7       /* 0 (default): the build picks its Morton-cell grid (2^level cells per axis over the BOX)
+                                    from N alone, which assumes the particles fill the box; 2..6: use this level — for a
+                                    droplet or slab that occupies a small part of the box a finer grid keeps the cells small
+                                    (profiles/r03_configs.md).  Lowered if T * 8^level would exceed 2^18.  The tree and the
+                                    lists do not depend on it.                                                     */
 int qbvh_set_option(int32_t key, int32_t value);
 
 /* Hint for the build-side subtree collapse ("collapse subtrees according to an appropriate heuristic",

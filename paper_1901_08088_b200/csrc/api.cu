@@ -24,6 +24,8 @@ struct Context {
     bool stats = false;
     int variant = 1;
     bool built = false;
+    int group_cap = GROUP_MAX;   // QBVH_OPT_GROUP_MAX
+    int cell_level = 0;          // QBVH_OPT_CELL_LEVEL: 0 = chosen from N
     int scan_spin_cycles = 1 << 18;   // ~130 us at 1.9 GHz; normal waits are a few us (QBVH_OPT_DEBUG_SCAN_SPIN)
     bool enqueued = false;       // a qbvh_neighbors_enqueue whose result has not been taken
     bool counters_armed = false; // group_cursor, max_count, warps_done of the tree are zero (after a build, after a production traversal)
@@ -294,6 +296,11 @@ int build_impl(const void *pos, bool f64, const int32_t *type, int64_t N, const 
     bp.T = type ? g.T : 1;
     bp.K = g.K;
     bp.lvl = pick_cell_level(N, bp.T);
+    if (g.cell_level > 0) {          // the caller knows better (particles filling a small part of the box); still T * 8^lvl <= 2^18
+        bp.lvl = g.cell_level;
+        while (bp.lvl > CELL_LMIN && ((int64_t)bp.T << (3 * bp.lvl)) > CELL_MAX_TOTAL) --bp.lvl;
+    }
+    bp.group_cap = g.group_cap;
     bp.f64 = f64;
     bp.scan_spin_cycles = g.scan_spin_cycles;
     for (int t = 0; t < QBVH_TMAX; ++t) bp.r_hint[t] = g.r_hint[t];
@@ -376,6 +383,14 @@ int qbvh_set_option(int32_t key, int32_t value) {
             if (value < 1 || value > (int32_t)QBVH_TAG_MAX || (uint32_t)value <= g.build_tag) return QBVH_ERR_INVALID_ARG;
             if (g.build_tag != 0) g.build_tag = (uint32_t)value - 1;   // a slot area still to be cleared stays at tag 0
             return QBVH_OK;
+        case QBVH_OPT_GROUP_MAX:
+            if (value < 1 || value > GROUP_MAX) return QBVH_ERR_INVALID_ARG;
+            g.group_cap = value;
+            return QBVH_OK;
+        case QBVH_OPT_CELL_LEVEL:
+            if (value != 0 && (value < CELL_LMIN || value > CELL_LMAX)) return QBVH_ERR_INVALID_ARG;
+            g.cell_level = value;
+            return QBVH_OK;
         case QBVH_OPT_DEBUG_SCAN_SPIN:
             if (value < 0) return QBVH_ERR_INVALID_ARG;
             g.scan_spin_cycles = value;
@@ -392,6 +407,8 @@ int qbvh_get_option(int32_t key) {
         case QBVH_OPT_VARIANT: return g.variant;
         case QBVH_OPT_DEBUG_BUILD_TAG: return (int)g.build_tag;
         case QBVH_OPT_DEBUG_SCAN_SPIN: return g.scan_spin_cycles;
+        case QBVH_OPT_GROUP_MAX: return g.group_cap;
+        case QBVH_OPT_CELL_LEVEL: return g.cell_level;
         default: return QBVH_ERR_INVALID_ARG;
     }
 }

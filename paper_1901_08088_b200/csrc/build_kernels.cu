@@ -172,7 +172,7 @@ __global__ void __launch_bounds__(MORTON_THREADS) morton_cell_kernel(const PT *_
 // per-type results into segments, roots and quantization frames.
 // ------------------------------------------------------------------------------------------------------------
 struct FinalizeParams {
-    int N, T, lvl, warp_slots;
+    int N, T, lvl, warp_slots, group_cap;
     float r_hint[QBVH_TMAX];
 };
 
@@ -218,9 +218,9 @@ __device__ void finalize_block(TreeMeta *__restrict__ meta, const uint32_t *__re
     // would sweep up thousands of misses.  Groups of type t hold at most 32 rho_t / rho_max particles (>= 1).
     if (d < QBVH_TMAX) {
         const float rmax = fmaxf(fmaxf(s_rho[0], s_rho[1]), fmaxf(s_rho[2], s_rho[3]));
-        int gm = GROUP_MAX;
+        int gm = min(GROUP_MAX, max(fp.group_cap, 1));       // QBVH_OPT_GROUP_MAX (default 32)
         if (s_rho[d] > 0.0f && rmax > 0.0f)
-            gm = (int)fminf(fmaxf(floorf((float)GROUP_MAX * s_rho[d] / rmax), 1.0f), (float)GROUP_MAX);
+            gm = (int)fminf(fmaxf(floorf((float)gm * s_rho[d] / rmax), 1.0f), (float)gm);
         // Small systems (the regime of PAPER.md:186): with fewer groups than the device has resident warps the
         // traversal is one group's latency, so groups shrink (down to 4) until there is about one per warp.
         gm = min(gm, max(4, s_cnt[d] / max(fp.warp_slots, 1)));
@@ -1179,7 +1179,7 @@ cudaError_t launch_build(const void *pos, const int32_t *type, const BuildParams
     }
 #undef QBVH_MORTON
     FinalizeParams fp;
-    fp.N = N, fp.T = p.T, fp.lvl = lvl, fp.warp_slots = traverse_warp_slots();
+    fp.N = N, fp.T = p.T, fp.lvl = lvl, fp.warp_slots = traverse_warp_slots(), fp.group_cap = p.group_cap;
     for (int t = 0; t < QBVH_TMAX; ++t) fp.r_hint[t] = p.r_hint[t];
     const int tiles = (ncells + SCAN_TILE - 1) / SCAN_TILE;
     err = launch_dependent(cell_scan_kernel, dim3(tiles), dim3(SCAN_THREADS), 0, st, b.cell_count, b.cell_start, b.cell_list, ncells, b.meta,

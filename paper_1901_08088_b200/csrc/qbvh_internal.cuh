@@ -152,6 +152,7 @@ struct BuildParams {
     float r_hint[QBVH_TMAX];       // <= 0: no collapse hint for that tree
     uint32_t build_tag;
     bool f64;                      // positions are double precision (qbvh_build_f64)
+    int group_cap;                 // largest query group the build may emit (<= GROUP_MAX)
     int scan_spin_cycles;          // how long a block of the 128-tile cell scan waits for the others before it sums alone
 };
 int pick_cell_level(int64_t N, int T);

@@ -19,7 +19,7 @@ ERR_INVALID_ARG, ERR_NOT_BUILT, ERR_WORKSPACE, ERR_CUTOFF_TOO_LARGE, ERR_TYPE_RA
 ERR_NOALLOC_LIMIT = -8
 NOALLOC_MAX_N = 1 << 22
 MAX_TYPES = 4
-OPT_LEAF_COLLAPSE, OPT_STATS, OPT_VARIANT, OPT_DEBUG_BUILD_TAG, OPT_DEBUG_SCAN_SPIN = 1, 2, 3, 4, 5
+OPT_LEAF_COLLAPSE, OPT_STATS, OPT_VARIANT, OPT_DEBUG_BUILD_TAG, OPT_DEBUG_SCAN_SPIN, OPT_GROUP_MAX, OPT_CELL_LEVEL = 1, 2, 3, 4, 5, 6, 7
 EXPORT_KEYS_SORTED, EXPORT_PERM, EXPORT_NODES, EXPORT_PARENT, EXPORT_FRAMES, EXPORT_SEGMENTS, EXPORT_SORTED_POS, EXPORT_COUNTS = range(1, 9)
 
 # every symbol include/qbvh.h declares

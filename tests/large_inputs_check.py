@@ -36,15 +36,28 @@ def main():
     ap.add_argument("--r", type=float, default=1.5)
     ap.add_argument("--cap", type=int, default=32)
     ap.add_argument("--reps", type=int, default=3)
+    ap.add_argument("--cell-level", type=int, default=0, help="QBVH_OPT_CELL_LEVEL (0: chosen from N)")
+    ap.add_argument("--group-max", type=int, default=32, help="QBVH_OPT_GROUP_MAX")
+    ap.add_argument("--stats", action="store_true", help="one more, instrumented traversal: counters of the production kernel")
+    ap.add_argument("--config", type=int, default=0, help="a BASELINE.json config (full size) instead of the ideal gas")
     ap.add_argument("--no-oracle", action="store_true")
     a = ap.parse_args()
     import torch
     from paper_1901_08088_b200 import qbvh
     dev = torch.device("cuda:0")
-    pos, box = make(a.n, a.droplet, a.rho, 0)
-    r_list = np.array([[a.r]], np.float32)
+    if a.config:
+        from paper_1901_08088_b200 import workloads as W
+        w = W.make_config(a.config)
+        assert w.T == 1, "single-type configs only"
+        pos, box, r_list = w.pos, w.box, w.r_list
+        a.n, a.cap, a.r = w.N, w.max_neigh, float(w.r_list[0, 0])
+    else:
+        pos, box = make(a.n, a.droplet, a.rho, 0)
+        r_list = np.array([[a.r]], np.float32)
     qbvh.qbvh_set_option(qbvh.OPT_LEAF_COLLAPSE, 32)
     qbvh.qbvh_set_option(qbvh.OPT_STATS, 0)
+    qbvh.qbvh_set_option(qbvh.OPT_CELL_LEVEL, a.cell_level)
+    qbvh.qbvh_set_option(qbvh.OPT_GROUP_MAX, a.group_max)
     nl = qbvh.NeighborList(a.n, T=1, max_neigh=a.cap, device=dev)
     dpos = torch.from_numpy(pos).to(dev)
     tb, tt, M = [], [], 0
@@ -64,7 +77,16 @@ def main():
     out = {"N": a.n, "droplet": a.droplet, "rho": a.rho, "r": a.r, "cap": a.cap, "box_L": float(box[3]),
            "build_ms": min(tb[1:]), "traverse_ms": min(tt[1:]), "M": int(M), "nn": float(n_gpu.mean()),
            "cell_level": int(counts[3]), "cells": int(counts[2]), "groups": int(counts[1]),
-           "workspace_GB": qbvh.qbvh_workspace_bytes(a.n, 1) / 1e9}
+           "workspace_GB": qbvh.qbvh_workspace_bytes(a.n, 1) / 1e9, "group_max": a.group_max}
+    if a.stats:
+        qbvh.qbvh_set_option(qbvh.OPT_STATS, 1)
+        nl.neighbors(r_list, retry=False)
+        st = qbvh.qbvh_get_stats()
+        qbvh.qbvh_set_option(qbvh.OPT_STATS, 0)
+        out.update(lanes_per_group=a.n / max(st["groups"], 1), candidates_per_group=st["group_candidates"] / max(st["groups"], 1),
+                   dist_checks_per_particle=st["group_dist_checks"] / a.n, node_tests_per_group=st["group_node_tests"] / max(st["groups"], 1),
+                   walk_steps_per_group=st["group_walk_steps"] / max(st["groups"], 1),
+                   check_lane_slots_per_particle=32.0 * st["group_candidates"] / a.n)
     if not a.no_oracle:
         from oracle import neighbors as ON
         t0 = time.perf_counter()

@@ -155,3 +155,28 @@ def test_f64_and_range_enqueue_forms():
     assert nl64.neighbors_result() == M1 and torch.equal(nl64.n_neigh, ref)
     rp, nb = ON.neighbor_list_f64(pos64, w.type, box64, r64)
     assert np.array_equal(ref.cpu().numpy()[: w.N], np.diff(rp))
+
+
+@pytest.mark.parametrize("opt,value", [("OPT_GROUP_MAX", 16), ("OPT_GROUP_MAX", 5), ("OPT_CELL_LEVEL", 2), ("OPT_CELL_LEVEL", 6)])
+def test_group_size_and_cell_level_do_not_change_tree_or_lists(opt, value):
+    """QBVH_OPT_GROUP_MAX and QBVH_OPT_CELL_LEVEL are tuning knobs: whatever they are set to, the build products are the
+    oracle tree bit for bit and the lists the oracle's."""
+    from paper_1901_08088_b200 import qbvh
+    from test_gpu_parity import check_build
+    key = getattr(qbvh, opt)
+    default = qbvh.qbvh_get_option(key)
+    try:
+        qbvh.qbvh_set_option(key, value)
+        for cid in (2, 3):
+            w = W.make_config(cid, small=True)
+            out, t = check_build(w, 32)
+            if opt == "OPT_CELL_LEVEL":
+                lvl = value
+                while (w.T << (3 * lvl)) > (1 << 18):            # the documented cap: T * 8^level <= 2^18
+                    lvl -= 1
+                assert int(out["counts"][3]) == lvl
+            compare_with_oracle(w, out, ON.neighbor_list(w.pos, w.type, w.box, w.r_list))
+    finally:
+        qbvh.qbvh_set_option(key, default)
+    with pytest.raises(qbvh.QbvhError):
+        qbvh.qbvh_set_option(key, 33 if opt == "OPT_GROUP_MAX" else 7)
