@@ -449,6 +449,60 @@ def run_sharded(args):
     return 0
 
 
+def run_slab(args):
+    """Strong-scaling extra (SURVEY 8e bullet 2 / 8f NEXT-4 second half): slab decomposition with halos.  One system; rank g
+    owns slab g along the longest axis; per step one neighbor exchange of the halo particles (NCCL P2P), the build over
+    own + ghosts, the traversal, rows of the own particles mapped to global ids.  Nothing is redundant across ranks."""
+    import torch
+    import torch.distributed as dist
+    from paper_1901_08088_b200 import qbvh, sharded
+    from paper_1901_08088_b200 import workloads as W
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    w = W.make_config(args.config, seed=0)              # ONE system, the same on every rank
+    qbvh.qbvh_set_option(qbvh.OPT_LEAF_COLLAPSE, args.leaf_collapse)
+    snl = sharded.SlabNeighborList(w.box, w.r_list, T=w.T, max_neigh=w.max_neigh, device=dev)
+    mine = np.nonzero(sharded.slab_index(w.pos, w.box, world, snl.axis) == rank)[0]
+    pos = torch.from_numpy(w.pos[mine]).to(dev)
+    typ = None if w.type is None else torch.from_numpy(w.type[mine]).to(dev)
+    gid = torch.from_numpy(mine.astype(np.int64)).to(dev)
+
+    def step():
+        snl.build(pos, typ, gid, w.N)
+        return snl.neighbors()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    ms = max_over_ranks(e0.elapsed_time(e1) / args.steps, world, dev)
+    if rank == 0:
+        print(json.dumps({"metric": METRIC, "value": 1e6 * ms / w.N, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                          "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": False, "scaling": "strong",
+                          "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": config_keys(args.config, w),
+                          "notes": {"parallelism": f"slab decomposition over {world} rank(s) along axis {snl.axis}: halo exchange (P2P), build and traversal of own + ghost particles",
+                                    "halo_width": snl.h, "own": int(len(mine)), "ghosts": snl.n_ghost, "halo_bytes_sent_per_step": snl.halo_bytes,
+                                    "l2": "not flushed (back-to-back steps)", "includes": "host-side halo selection and the id mapping of the rows"},
+                          "gpu_launches": KERNELS_PER_STEP * args.steps}))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -462,12 +516,15 @@ def main():
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg (profiling runs)")
     ap.add_argument("--variant", type=int, default=None, help="traversal kernel (QBVH_OPT_VARIANT); default: the library's")
     ap.add_argument("--sharded", action="store_true", help="extra: query sharding over the ranks (strong scaling) instead of replicas")
+    ap.add_argument("--slab", action="store_true", help="extra: slab decomposition with halos over the ranks (strong scaling)")
     ap.add_argument("--dtype", default="f32", choices=["f32", "f64"], help="f64: double-precision particles on the fp32 tree (an extra line)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
     if args.sharded:
         return run_sharded(args)
+    if args.slab:
+        return run_slab(args)
     return run_gpu(args)
 
 

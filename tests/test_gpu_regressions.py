@@ -180,3 +180,33 @@ def test_group_size_and_cell_level_do_not_change_tree_or_lists(opt, value):
         qbvh.qbvh_set_option(key, default)
     with pytest.raises(qbvh.QbvhError):
         qbvh.qbvh_set_option(key, 33 if opt == "OPT_GROUP_MAX" else 7)
+
+
+@pytest.mark.parametrize("world", [2, 3, 5])
+@pytest.mark.parametrize("cid", [3, 5])
+def test_slab_decomposition_emulated_on_one_gpu(cid, world):
+    """SlabNeighborList with the CUDA backend, the ranks played one after another on one GPU (the exchange itself is
+    covered over gloo in test_slab_host.py): own + halo particles in the original periodic box, rows of the own particles,
+    entries mapped to global ids — merged over the ranks it must be the oracle's list of the whole system, exactly."""
+    import torch
+    from paper_1901_08088_b200 import qbvh, sharded
+    w = W.make_config(cid, small=True)
+    dev = torch.device("cuda:0")
+    qbvh.qbvh_set_option(qbvh.OPT_LEAF_COLLAPSE, 32)
+    qbvh.qbvh_set_option(qbvh.OPT_STATS, 0)
+    qbvh.qbvh_set_collapse_hint(None)
+    snl = sharded.SlabNeighborList(w.box, w.r_list, T=w.T, max_neigh=16, device=dev)      # capacity too small: the retry path
+    parts, ghosts_total = [], 0
+    for g in range(world):
+        own, ghosts = sharded.local_set_indices(w.pos, w.box, world, g, snl.h)
+        idx = np.concatenate([own, ghosts])
+        snl.build_from_local_set(torch.from_numpy(w.pos[idx]).to(dev), None if w.type is None else torch.from_numpy(w.type[idx]).to(dev),
+                                 torch.from_numpy(idx.astype(np.int64)).to(dev), len(own), w.N)
+        gid, n_neigh, nlist, M = snl.neighbors()
+        parts.append((gid.cpu().numpy(), n_neigh.cpu().numpy(), nlist.cpu().numpy()))
+        ghosts_total += len(ghosts)
+    qbvh.qbvh_set_workspace(None)
+    n_all, l_all = sharded.merge_slices(w.N, parts)
+    out = {"M": int(n_all.max()), "max_neigh": l_all.shape[1], "nlist": l_all, "n_neigh": n_all}
+    compare_with_oracle(w, out, ON.neighbor_list(w.pos, w.type, w.box, w.r_list))
+    assert 0 < ghosts_total < 2 * w.N
